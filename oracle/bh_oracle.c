@@ -1,0 +1,457 @@
+/*
+ * bh_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, single-threaded fp64 CPU Barnes-Hut written from the paper
+ * (arxiv 1509.07370, /root/reference/PAPER.md) and the readings of SURVEY.md §8(c) / DESIGN.md.
+ * It shares no code, header, table or helper with the CUDA library under paper_1509_07370_b200/.
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may
+ * call it.  Compile with:  gcc -O2 -ffp-contract=off -fPIC -shared -o libbh_oracle.so bh_oracle.c -lm
+ * (-ffp-contract=off: the key expression below must not be fused, K-rule 1).
+ *
+ * What each function follows:
+ *   orc_keys      63-bit Morton key of a point in the caller's cube.  The paper only names the
+ *                 Morton curve; the exact expression is DESIGN.md reading K1-K2.
+ *   orc_build     keys -> stable sort by (key, index) -> octree "recursively divided into eight sub
+ *                 cells ... until only one particle is left for every sub cell" (§2);
+ *                 per node total mass and centre of mass, Eq. 5, and
+ *                 delta = |com - geometric centre|.
+ *   orc_potential stack-based depth-first walk (§3.3) with the opening test
+ *                 d > l/theta (Eq. 3) or d > l/theta + delta (Eq. 4);
+ *                 a group of `group` consecutive sorted targets shares the walk and a node is used
+ *                 only if EVERY member accepts it (the all() vote).
+ *                 Phi_i = -G sum m_j/|r_i - r_j| (Eq. 2, without the printed 1/2: reading).
+ *   orc_direct    Eq. 2 written out: Phi_i = -G sum_{j != i} m_j/|r_i - r_j|.
+ *
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): keys vs closed form on 2^k grids and a per-bit
+ * interleave; tree vs a recursive brute-force partition in numpy; node counts (n-1)/7 on grids;
+ * moments vs flat sums; theta=0 walk == direct sum bit for bit in sorted order; convergence with
+ * theta; uniform-sphere and MacLaurin closed forms.  No function here is "parity unpinned".
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define ORC_MAXLEVEL 21
+#define ORC_MAC_BH86 0     /* Eq. 3 */
+#define ORC_MAC_BARNES94 1 /* Eq. 4 */
+
+typedef struct {
+    int32_t level;       /* 0 = root; 21 = bucket leaf (>= 2 cells with identical keys) */
+    uint64_t prefix;     /* key >> 3*(21-level) */
+    int64_t lo, hi;      /* sorted cell range [lo, hi) */
+    int64_t child[8];    /* per octant: -1 absent; >= 0 node index; <= -2 leaf cell with sorted slot -(c+2) */
+    double M, R[3];      /* Eq. 5 */
+    double delta;        /* |R - geometric centre| */
+    double size;         /* l = L / 2^level */
+    double centre[3];    /* geometric centre */
+} orc_node;
+
+typedef struct {
+    int64_t n;
+    double cube[4];
+    uint64_t *key;       /* sorted keys */
+    uint32_t *perm;      /* perm[s] = original index of sorted slot s */
+    double *x, *y, *z, *m; /* sorted copies */
+    orc_node *node;
+    int64_t n_nodes, cap_nodes;
+    int64_t n_clamped;
+    int32_t depth;       /* deepest internal-node level */
+} orc_tree;
+
+/* ---- keys (K1-K2) ------------------------------------------------------------------ */
+static uint64_t quantise(double v, double v0, double s, int *clamped)
+{
+    /* t = (v - v0) * s : one subtract, one multiply, round-to-nearest, no contraction */
+    double d = v - v0;
+    double t = d * s;
+    double f = floor(t);
+    if (!(f >= 0.0)) { /* negative or NaN */
+        if (clamped) *clamped = 1;
+        return 0;
+    }
+    if (f > 2097151.0) {
+        if (clamped) *clamped = 1;
+        return 2097151u;
+    }
+    return (uint64_t)f;
+}
+
+static uint64_t interleave3(uint64_t qx, uint64_t qy, uint64_t qz)
+{
+    /* bit (3k+0) = bit k of qx, (3k+1) = bit k of qy, (3k+2) = bit k of qz, k = 0..20 */
+    uint64_t key = 0;
+    for (int k = 0; k < 21; ++k) {
+        key |= ((qx >> k) & 1ull) << (3 * k + 0);
+        key |= ((qy >> k) & 1ull) << (3 * k + 1);
+        key |= ((qz >> k) & 1ull) << (3 * k + 2);
+    }
+    return key;
+}
+
+int orc_keys(const double *x, const double *y, const double *z, int64_t n, const double *cube,
+             uint64_t *keys, int64_t *n_clamped)
+{
+    if (!x || !y || !z || !cube || !keys || n < 0 || !(cube[3] > 0.0)) return -1;
+    double s = 2097152.0 / cube[3];
+    int64_t nc = 0;
+    for (int64_t i = 0; i < n; ++i) {
+        int c = 0;
+        uint64_t qx = quantise(x[i], cube[0], s, &c);
+        uint64_t qy = quantise(y[i], cube[1], s, &c);
+        uint64_t qz = quantise(z[i], cube[2], s, &c);
+        keys[i] = interleave3(qx, qy, qz);
+        nc += c;
+    }
+    if (n_clamped) *n_clamped = nc;
+    return 0;
+}
+
+/* ---- sort (S-rule): ascending key, ties by ascending original index -------------------------- */
+typedef struct { uint64_t key; uint32_t idx; } orc_kv;
+
+static int cmp_kv(const void *a, const void *b)
+{
+    const orc_kv *p = (const orc_kv *)a, *q = (const orc_kv *)b;
+    if (p->key < q->key) return -1;
+    if (p->key > q->key) return 1;
+    if (p->idx < q->idx) return -1;
+    if (p->idx > q->idx) return 1;
+    return 0;
+}
+
+int orc_sort(const uint64_t *keys, int64_t n, uint32_t *perm)
+{
+    if (!keys || !perm || n < 0) return -1;
+    orc_kv *kv = (orc_kv *)malloc(sizeof(orc_kv) * (size_t)(n > 0 ? n : 1));
+    if (!kv) return -2;
+    for (int64_t i = 0; i < n; ++i) { kv[i].key = keys[i]; kv[i].idx = (uint32_t)i; }
+    qsort(kv, (size_t)n, sizeof(orc_kv), cmp_kv);
+    for (int64_t i = 0; i < n; ++i) perm[i] = kv[i].idx;
+    free(kv);
+    return 0;
+}
+
+/* ---- tree (T-rules) and moments (M-rules) ---------------------------------------------------- */
+static int64_t new_node(orc_tree *t)
+{
+    if (t->n_nodes == t->cap_nodes) {
+        int64_t cap = t->cap_nodes ? 2 * t->cap_nodes : 1024;
+        orc_node *p = (orc_node *)realloc(t->node, sizeof(orc_node) * (size_t)cap);
+        if (!p) return -1;
+        t->node = p;
+        t->cap_nodes = cap;
+    }
+    return t->n_nodes++;
+}
+
+/* Builds the node owning sorted range [lo, hi) (hi - lo >= 2) at `level`; returns its index.
+ * the cube "is then recursively divided into eight sub cells ... until only one
+ * particle is left for every sub cell".  Single-child chains are kept (T-rule 2). */
+static int64_t build_node(orc_tree *t, int32_t level, int64_t lo, int64_t hi)
+{
+    int64_t id = new_node(t);
+    if (id < 0) return -1;
+    {
+        orc_node *nd = &t->node[id];
+        nd->level = level;
+        nd->prefix = (level == 0) ? 0 : (t->key[lo] >> (3 * (ORC_MAXLEVEL - level)));
+        nd->lo = lo;
+        nd->hi = hi;
+        for (int c = 0; c < 8; ++c) nd->child[c] = -1;
+        /* geometric centre (T-rule 4): de-interleave the prefix */
+        uint64_t px = 0, py = 0, pz = 0;
+        for (int k = 0; k < level; ++k) {
+            px |= ((nd->prefix >> (3 * k + 0)) & 1ull) << k;
+            py |= ((nd->prefix >> (3 * k + 1)) & 1ull) << k;
+            pz |= ((nd->prefix >> (3 * k + 2)) & 1ull) << k;
+        }
+        nd->size = ldexp(t->cube[3], -level);
+        nd->centre[0] = t->cube[0] + ((double)px + 0.5) * nd->size;
+        nd->centre[1] = t->cube[1] + ((double)py + 0.5) * nd->size;
+        nd->centre[2] = t->cube[2] + ((double)pz + 0.5) * nd->size;
+        nd->M = 0.0;
+        nd->R[0] = nd->R[1] = nd->R[2] = 0.0;
+        nd->delta = 0.0;
+    }
+    if (level > t->depth && level < ORC_MAXLEVEL) t->depth = level;
+
+    double M = 0.0, S[3] = {0.0, 0.0, 0.0};
+    if (level == ORC_MAXLEVEL) {
+        /* bucket leaf (T-rule 3): cells with identical keys; moments from the cells in order */
+        for (int64_t s = lo; s < hi; ++s) {
+            M += t->m[s];
+            S[0] += t->m[s] * t->x[s];
+            S[1] += t->m[s] * t->y[s];
+            S[2] += t->m[s] * t->z[s];
+        }
+    } else {
+        int shift = 3 * (ORC_MAXLEVEL - level - 1);
+        int64_t a = lo;
+        while (a < hi) {
+            int oct = (int)((t->key[a] >> shift) & 7ull);
+            int64_t b = a + 1;
+            while (b < hi && (int)((t->key[b] >> shift) & 7ull) == oct) ++b;
+            if (b - a == 1) {
+                t->node[id].child[oct] = -(a + 2); /* leaf cell, sorted slot a */
+                M += t->m[a];
+                S[0] += t->m[a] * t->x[a];
+                S[1] += t->m[a] * t->y[a];
+                S[2] += t->m[a] * t->z[a];
+            } else {
+                int64_t c = build_node(t, level + 1, a, b);
+                if (c < 0) return -1;
+                t->node[id].child[oct] = c;
+                /* Eq. 5 from the children's moments, ascending octant order (M-rule 1) */
+                M += t->node[c].M;
+                S[0] += t->node[c].M * t->node[c].R[0];
+                S[1] += t->node[c].M * t->node[c].R[1];
+                S[2] += t->node[c].M * t->node[c].R[2];
+            }
+            a = b;
+        }
+    }
+    orc_node *nd = &t->node[id];
+    nd->M = M;
+    if (M != 0.0) {
+        nd->R[0] = S[0] / M; /* Eq. 5: R = (1/M) sum m_i r_i */
+        nd->R[1] = S[1] / M;
+        nd->R[2] = S[2] / M;
+        double ex = nd->R[0] - nd->centre[0], ey = nd->R[1] - nd->centre[1], ez = nd->R[2] - nd->centre[2];
+        nd->delta = sqrt(ex * ex + ey * ey + ez * ez);
+    } else { /* M-rule 2: zero-mass node */
+        nd->R[0] = nd->centre[0];
+        nd->R[1] = nd->centre[1];
+        nd->R[2] = nd->centre[2];
+        nd->delta = 0.0;
+    }
+    return id;
+}
+
+void orc_free(orc_tree *t)
+{
+    if (!t) return;
+    free(t->key); free(t->perm); free(t->x); free(t->y); free(t->z); free(t->m); free(t->node);
+    free(t);
+}
+
+orc_tree *orc_build(const double *x, const double *y, const double *z, const double *m, int64_t n,
+                    const double *cube)
+{
+    if (!x || !y || !z || !m || !cube || n <= 0 || n >= 2147483648ll || !(cube[3] > 0.0)) return NULL;
+    orc_tree *t = (orc_tree *)calloc(1, sizeof(orc_tree));
+    if (!t) return NULL;
+    t->n = n;
+    memcpy(t->cube, cube, sizeof(double) * 4);
+    uint64_t *k0 = (uint64_t *)malloc(sizeof(uint64_t) * (size_t)n);
+    t->key = (uint64_t *)malloc(sizeof(uint64_t) * (size_t)n);
+    t->perm = (uint32_t *)malloc(sizeof(uint32_t) * (size_t)n);
+    t->x = (double *)malloc(sizeof(double) * (size_t)n);
+    t->y = (double *)malloc(sizeof(double) * (size_t)n);
+    t->z = (double *)malloc(sizeof(double) * (size_t)n);
+    t->m = (double *)malloc(sizeof(double) * (size_t)n);
+    if (!k0 || !t->key || !t->perm || !t->x || !t->y || !t->z || !t->m) { free(k0); orc_free(t); return NULL; }
+    orc_keys(x, y, z, n, cube, k0, &t->n_clamped);
+    if (orc_sort(k0, n, t->perm) != 0) { free(k0); orc_free(t); return NULL; }
+    for (int64_t s = 0; s < n; ++s) {
+        uint32_t i = t->perm[s];
+        t->key[s] = k0[i];
+        t->x[s] = x[i]; t->y[s] = y[i]; t->z[s] = z[i]; t->m[s] = m[i];
+    }
+    free(k0);
+    t->depth = 0;
+    if (n >= 2) { /* T-rule 1: root is an internal node iff n >= 2 */
+        if (build_node(t, 0, 0, n) < 0) { orc_free(t); return NULL; }
+    }
+    return t;
+}
+
+int64_t orc_num_cells(const orc_tree *t) { return t ? t->n : -1; }
+int64_t orc_num_nodes(const orc_tree *t) { return t ? t->n_nodes : -1; }  /* incl. level-21 buckets */
+int64_t orc_num_clamped(const orc_tree *t) { return t ? t->n_clamped : -1; }
+int32_t orc_depth(const orc_tree *t) { return t ? t->depth : -1; }
+
+int orc_get_sorted(const orc_tree *t, uint64_t *keys, uint32_t *perm)
+{
+    if (!t) return -1;
+    if (keys) memcpy(keys, t->key, sizeof(uint64_t) * (size_t)t->n);
+    if (perm) memcpy(perm, t->perm, sizeof(uint32_t) * (size_t)t->n);
+    return 0;
+}
+
+/* canonical order (T-rule 5): by (level, prefix) */
+typedef struct { int32_t level; uint64_t prefix; int64_t id; } orc_ord;
+static int cmp_ord(const void *a, const void *b)
+{
+    const orc_ord *p = (const orc_ord *)a, *q = (const orc_ord *)b;
+    if (p->level != q->level) return p->level < q->level ? -1 : 1;
+    if (p->prefix != q->prefix) return p->prefix < q->prefix ? -1 : 1;
+    return 0;
+}
+
+/* Fills caller arrays of length orc_num_nodes() in canonical order.  Any pointer may be NULL. */
+int orc_export_nodes(const orc_tree *t, int32_t *level, uint64_t *prefix, int64_t *lo, int64_t *hi,
+                     double *M, double *Rx, double *Ry, double *Rz, double *delta, int32_t *nchild)
+{
+    if (!t) return -1;
+    int64_t nn = t->n_nodes;
+    orc_ord *o = (orc_ord *)malloc(sizeof(orc_ord) * (size_t)(nn > 0 ? nn : 1));
+    if (!o) return -2;
+    for (int64_t i = 0; i < nn; ++i) { o[i].level = t->node[i].level; o[i].prefix = t->node[i].prefix; o[i].id = i; }
+    qsort(o, (size_t)nn, sizeof(orc_ord), cmp_ord);
+    for (int64_t i = 0; i < nn; ++i) {
+        const orc_node *nd = &t->node[o[i].id];
+        if (level) level[i] = nd->level;
+        if (prefix) prefix[i] = nd->prefix;
+        if (lo) lo[i] = nd->lo;
+        if (hi) hi[i] = nd->hi;
+        if (M) M[i] = nd->M;
+        if (Rx) Rx[i] = nd->R[0];
+        if (Ry) Ry[i] = nd->R[1];
+        if (Rz) Rz[i] = nd->R[2];
+        if (delta) delta[i] = nd->delta;
+        if (nchild) {
+            int c = 0;
+            if (nd->level == ORC_MAXLEVEL) c = (int)(nd->hi - nd->lo);
+            else for (int k = 0; k < 8; ++k) c += nd->child[k] != -1;
+            nchild[i] = c;
+        }
+    }
+    free(o);
+    return 0;
+}
+
+/* ---- walk (W-rules) ---------------------------------------------------------------------------- */
+/* A leaf cell j reached through an opened parent: every member t != j adds m_j/|r_t - r_j|
+ * (Eq. 2, j != i by sorted slot; distinct cells at zero distance are skipped, W-rule 3). */
+static void add_leaf_cell(const orc_tree *t, int64_t j, int64_t t0, int nt, double *acc)
+{
+    for (int a = 0; a < nt; ++a) {
+        int64_t s = t0 + a;
+        if (s == j) continue;
+        double dx = t->x[s] - t->x[j], dy = t->y[s] - t->y[j], dz = t->z[s] - t->z[j];
+        double d2 = dx * dx + dy * dy + dz * dz;
+        if (d2 == 0.0) continue;
+        acc[a] += t->m[j] / sqrt(d2);
+    }
+}
+
+/* Is node nd accepted by EVERY member of the group (the all() vote)?
+ * Eq. 3: d > l/theta;  Eq. 4: d > l/theta + delta;  compared as d^2 > r_c^2, strict. */
+static int group_accepts(const orc_tree *t, const orc_node *nd, double theta, int mac, int mac_fp32,
+                         int64_t t0, int nt)
+{
+    if (theta == 0.0) return 0; /* r_c = +inf: open everything */
+    if (!mac_fp32) {
+        double rc = nd->size / theta;
+        if (mac == ORC_MAC_BARNES94) rc += nd->delta;
+        double rc2 = rc * rc;
+        for (int a = 0; a < nt; ++a) {
+            int64_t s = t0 + a;
+            double dx = t->x[s] - nd->R[0], dy = t->y[s] - nd->R[1], dz = t->z[s] - nd->R[2];
+            double d2 = dx * dx + dy * dy + dz * dz;
+            if (!(d2 > rc2)) return 0;
+        }
+        return 1;
+    }
+    /* mac_fp32: the decision taken in the kernel's arithmetic type (reading W8):
+     * operands rounded to fp32, r_c = l*(1/theta) (+ delta), d2 = fma(dz,dz,fma(dy,dy,dx*dx)). */
+    float rc = (float)nd->size * (float)(1.0 / theta);
+    if (mac == ORC_MAC_BARNES94) rc = rc + (float)nd->delta;
+    float rc2 = rc * rc;
+    float nx = (float)nd->R[0], ny = (float)nd->R[1], nz = (float)nd->R[2];
+    for (int a = 0; a < nt; ++a) {
+        int64_t s = t0 + a;
+        float dx = (float)t->x[s] - nx, dy = (float)t->y[s] - ny, dz = (float)t->z[s] - nz;
+        float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+        if (!(d2 > rc2)) return 0;
+    }
+    return 1;
+}
+
+/* Walks groups [group_begin, group_end) of `group` consecutive sorted targets (W-rule 1).
+ * phi_orig: length n, ORIGINAL order; only the walked targets are written.
+ * counts (may be NULL): per walked group {accepted nodes, leaf cells summed, opened nodes}. */
+int orc_potential(const orc_tree *t, double theta, double G, int mac, int group, int mac_fp32,
+                  int64_t group_begin, int64_t group_end, double *phi_orig, int64_t *counts)
+{
+    if (!t || !phi_orig || !(theta >= 0.0) || group < 1) return -1;
+    int64_t n = t->n;
+    int64_t ngroups = (n + group - 1) / group;
+    if (group_end < 0 || group_end > ngroups) group_end = ngroups;
+    if (group_begin < 0) group_begin = 0;
+    /* stack of child references: >= 0 internal node / bucket index, <= -2 leaf cell -(slot+2).
+     * depth-first: at most 7 waiting siblings per level plus the current entry */
+    int64_t stack[8 * (ORC_MAXLEVEL + 2)];
+    double *acc = (double *)malloc(sizeof(double) * (size_t)group);
+    if (!acc) return -2;
+    for (int64_t g = group_begin; g < group_end; ++g) {
+        int64_t t0 = g * group, t1 = t0 + group;
+        if (t1 > n) t1 = n;
+        int nt = (int)(t1 - t0);
+        for (int a = 0; a < nt; ++a) acc[a] = 0.0;
+        int64_t n_acc = 0, n_leaf = 0, n_open = 0;
+        int sp = 0;
+        if (n >= 2) stack[sp++] = 0; /* root tested like any other node (W-rule 2); n = 1: Phi = 0 */
+        while (sp > 0) {
+            int64_t e = stack[--sp];
+            if (e <= -2) { /* leaf cell */
+                add_leaf_cell(t, -(e + 2), t0, nt, acc);
+                ++n_leaf;
+                continue;
+            }
+            const orc_node *nd = &t->node[e];
+            if (nd->level == ORC_MAXLEVEL) { /* bucket leaf: all its cells summed directly (T-rule 3) */
+                for (int64_t j = nd->lo; j < nd->hi; ++j) {
+                    add_leaf_cell(t, j, t0, nt, acc);
+                    ++n_leaf;
+                }
+                continue;
+            }
+            if (group_accepts(t, nd, theta, mac, mac_fp32, t0, nt)) {
+                for (int a = 0; a < nt; ++a) { /* every member adds M_N/|r_t - R_N| */
+                    int64_t s = t0 + a;
+                    double dx = t->x[s] - nd->R[0], dy = t->y[s] - nd->R[1], dz = t->z[s] - nd->R[2];
+                    acc[a] += nd->M / sqrt(dx * dx + dy * dy + dz * dz);
+                }
+                ++n_acc;
+                continue;
+            }
+            ++n_open; /* opened for the whole group: children pop in ascending octant order */
+            for (int c = 7; c >= 0; --c)
+                if (nd->child[c] != -1) stack[sp++] = nd->child[c];
+        }
+        for (int a = 0; a < nt; ++a) phi_orig[t->perm[t0 + a]] = -G * acc[a]; /* W-rule 4 */
+        if (counts) {
+            int64_t *c = counts + 3 * (g - group_begin);
+            c[0] = n_acc; c[1] = n_leaf; c[2] = n_open;
+        }
+    }
+    free(acc);
+    return 0;
+}
+
+/* ---- direct summation, Eq. 2 written out ------------------------------------------
+ * Phi_i = -G sum_{j != i} m_j/|r_i - r_j| over ALL n sources, for the listed targets (original
+ * indices; targets == NULL: all n, phi has length n).  Sources are visited in original order.
+ * Distinct cells at zero distance are skipped, as in the walk. */
+int orc_direct(const double *x, const double *y, const double *z, const double *m, int64_t n, double G,
+               const int64_t *targets, int64_t nt, double *phi)
+{
+    if (!x || !y || !z || !m || !phi || n <= 0) return -1;
+    int64_t count = targets ? nt : n;
+    for (int64_t a = 0; a < count; ++a) {
+        int64_t i = targets ? targets[a] : a;
+        if (i < 0 || i >= n) return -1;
+        double s = 0.0;
+        for (int64_t j = 0; j < n; ++j) {
+            if (j == i) continue;
+            double dx = x[i] - x[j], dy = y[i] - y[j], dz = z[i] - z[j];
+            double d2 = dx * dx + dy * dy + dz * dz;
+            if (d2 == 0.0) continue;
+            s += m[j] / sqrt(d2);
+        }
+        phi[a] = -G * s;
+    }
+    return 0;
+}

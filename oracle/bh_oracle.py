@@ -1,0 +1,155 @@
+"""ctypes wrapper of oracle/bh_oracle.c (test infrastructure; see the C file's header).
+
+Argument marshalling only -- every number comes from the C code.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "bh_oracle.c")
+_LIB = os.path.join(_HERE, "libbh_oracle.so")
+
+MAC_BH86 = 0      # Eq. 3
+MAC_BARNES94 = 1  # Eq. 4
+
+
+def build_library(force: bool = False) -> str:
+    """gcc -O2 -ffp-contract=off (K-rule 1: no FMA contraction in the key expression)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-Wall", "-fPIC", "-shared",
+                               "-o", _LIB, _SRC, "-lm"])
+    return _LIB
+
+
+_lib = None
+
+
+def _L():
+    global _lib
+    if _lib is None:
+        lib = C.CDLL(build_library())
+        dp, u64p, u32p, i64p, i32p = (C.POINTER(C.c_double), C.POINTER(C.c_uint64), C.POINTER(C.c_uint32),
+                                      C.POINTER(C.c_int64), C.POINTER(C.c_int32))
+        lib.orc_keys.argtypes = [dp, dp, dp, C.c_int64, dp, u64p, i64p]
+        lib.orc_sort.argtypes = [u64p, C.c_int64, u32p]
+        lib.orc_build.argtypes = [dp, dp, dp, dp, C.c_int64, dp]
+        lib.orc_build.restype = C.c_void_p
+        lib.orc_free.argtypes = [C.c_void_p]
+        lib.orc_free.restype = None
+        for f in ("orc_num_cells", "orc_num_nodes", "orc_num_clamped"):
+            getattr(lib, f).argtypes = [C.c_void_p]
+            getattr(lib, f).restype = C.c_int64
+        lib.orc_depth.argtypes = [C.c_void_p]
+        lib.orc_depth.restype = C.c_int32
+        lib.orc_get_sorted.argtypes = [C.c_void_p, u64p, u32p]
+        lib.orc_export_nodes.argtypes = [C.c_void_p, i32p, u64p, i64p, i64p, dp, dp, dp, dp, dp, i32p]
+        lib.orc_potential.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_int, C.c_int,
+                                      C.c_int64, C.c_int64, dp, i64p]
+        lib.orc_direct.argtypes = [dp, dp, dp, dp, C.c_int64, C.c_double, i64p, C.c_int64, dp]
+        _lib = lib
+    return _lib
+
+
+def _p(a, t):
+    return a.ctypes.data_as(C.POINTER(t))
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def keys(x, y, z, cube):
+    """63-bit Morton keys in the caller's order; returns (keys uint64[n], n_clamped)."""
+    x, y, z, cube = _f64(x), _f64(y), _f64(z), _f64(cube)
+    out = np.empty(x.shape[0], dtype=np.uint64)
+    nc = C.c_int64(0)
+    rc = _L().orc_keys(_p(x, C.c_double), _p(y, C.c_double), _p(z, C.c_double), x.shape[0],
+                       _p(cube, C.c_double), _p(out, C.c_uint64), C.byref(nc))
+    if rc != 0:
+        raise ValueError("orc_keys: invalid argument")
+    return out, int(nc.value)
+
+
+def sort_perm(k):
+    """Stable ascending (key, index) order: perm[s] = original index of sorted slot s."""
+    k = np.ascontiguousarray(k, dtype=np.uint64)
+    perm = np.empty(k.shape[0], dtype=np.uint32)
+    if _L().orc_sort(_p(k, C.c_uint64), k.shape[0], _p(perm, C.c_uint32)) != 0:
+        raise ValueError("orc_sort failed")
+    return perm
+
+
+def direct(x, y, z, m, G=1.0, targets=None):
+    """Eq. 2: Phi_i = -G sum_{j!=i} m_j/|r_i-r_j| for all i or the listed targets."""
+    x, y, z, m = _f64(x), _f64(y), _f64(z), _f64(m)
+    n = x.shape[0]
+    if targets is None:
+        phi = np.empty(n, dtype=np.float64)
+        rc = _L().orc_direct(_p(x, C.c_double), _p(y, C.c_double), _p(z, C.c_double), _p(m, C.c_double), n,
+                             G, None, 0, _p(phi, C.c_double))
+    else:
+        t = np.ascontiguousarray(targets, dtype=np.int64)
+        phi = np.empty(t.shape[0], dtype=np.float64)
+        rc = _L().orc_direct(_p(x, C.c_double), _p(y, C.c_double), _p(z, C.c_double), _p(m, C.c_double), n,
+                             G, _p(t, C.c_int64), t.shape[0], _p(phi, C.c_double))
+    if rc != 0:
+        raise ValueError("orc_direct: invalid argument")
+    return phi
+
+
+class OracleTree:
+    """keys -> sort -> octree -> monopoles for one set of cells (orc_build)."""
+
+    def __init__(self, x, y, z, m, cube):
+        x, y, z, m, cube = _f64(x), _f64(y), _f64(z), _f64(m), _f64(cube)
+        self._h = _L().orc_build(_p(x, C.c_double), _p(y, C.c_double), _p(z, C.c_double), _p(m, C.c_double),
+                                 x.shape[0], _p(cube, C.c_double))
+        if not self._h:
+            raise ValueError("orc_build: invalid argument or out of memory")
+        self.n = int(_L().orc_num_cells(self._h))
+        self.n_nodes = int(_L().orc_num_nodes(self._h))      # internal nodes + level-21 buckets
+        self.n_clamped = int(_L().orc_num_clamped(self._h))
+        self.depth = int(_L().orc_depth(self._h))
+
+    def __del__(self):
+        h = getattr(self, "_h", None)
+        if h:
+            _L().orc_free(h)
+            self._h = None
+
+    def sorted_keys_perm(self):
+        k = np.empty(self.n, dtype=np.uint64)
+        p = np.empty(self.n, dtype=np.uint32)
+        _L().orc_get_sorted(self._h, _p(k, C.c_uint64), _p(p, C.c_uint32))
+        return k, p
+
+    def nodes(self):
+        """Canonical node list (sorted by (level, prefix)) as a dict of arrays."""
+        nn = self.n_nodes
+        out = dict(level=np.empty(nn, np.int32), prefix=np.empty(nn, np.uint64), lo=np.empty(nn, np.int64),
+                   hi=np.empty(nn, np.int64), M=np.empty(nn), Rx=np.empty(nn), Ry=np.empty(nn), Rz=np.empty(nn),
+                   delta=np.empty(nn), nchild=np.empty(nn, np.int32))
+        _L().orc_export_nodes(self._h, _p(out["level"], C.c_int32), _p(out["prefix"], C.c_uint64),
+                              _p(out["lo"], C.c_int64), _p(out["hi"], C.c_int64), _p(out["M"], C.c_double),
+                              _p(out["Rx"], C.c_double), _p(out["Ry"], C.c_double), _p(out["Rz"], C.c_double),
+                              _p(out["delta"], C.c_double), _p(out["nchild"], C.c_int32))
+        return out
+
+    def potential(self, theta, G=1.0, mac=MAC_BH86, group=32, mac_fp32=False, groups=None, want_counts=False):
+        """Group walk (W-rules).  Returns phi in ORIGINAL order (NaN where not walked when `groups`
+        = (begin, end) restricts the walk) and, if asked, counts[ngroups_walked, 3] =
+        (accepted nodes, leaf cells, opened nodes)."""
+        ng = (self.n + group - 1) // group
+        gb, ge = (0, ng) if groups is None else groups
+        phi = np.full(self.n, np.nan)
+        counts = np.zeros((max(ge - gb, 0), 3), dtype=np.int64)
+        rc = _L().orc_potential(self._h, float(theta), float(G), int(mac), int(group), int(bool(mac_fp32)),
+                                gb, ge, _p(phi, C.c_double), _p(counts, C.c_int64))
+        if rc != 0:
+            raise ValueError("orc_potential: invalid argument")
+        return (phi, counts) if want_counts else phi
