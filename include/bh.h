@@ -1,0 +1,163 @@
+/*
+ * bh.h -- C ABI of libbh: Barnes-Hut gravitational potential of AMR grid cells treated as
+ * point masses, on one NVIDIA B200 (sm_100a).
+ *
+ * The method is the one of "A GPU accelerated Barnes-Hut Tree Code for FLASH4" (arXiv 1509.07370;
+ * citations below are lines of /root/reference/PAPER.md): an octree over the cells with per-node
+ * total mass and centre of mass (§2, Eq. 5), and a per-target tree
+ * walk that applies the opening criterion d > l/theta (Eq. 3) or d > l/theta + delta
+ * (Eq. 4) with one vote per warp of 32 neighbouring cells (§3.3) and
+ * accumulates Phi_i = -G sum_j m_j/|r_i - r_j| (Eq. 2; the printed factor 1/2 is not
+ * applied, reading R1).
+ *
+ * Conventions (all calls):
+ *  - Every function returns BH_OK (0) or a negative BH_ERR_* code; nothing throws, exits or
+ *    prints.  bh_strerror() names a code; bh_last_cuda_error() returns the CUDA runtime error
+ *    string recorded with the last BH_ERR_CUDA of that context.
+ *  - Pointers marked DEVICE must be device memory of the context's device; pointers marked HOST
+ *    are ordinary host memory.  The library never frees or keeps caller memory: inputs are
+ *    borrowed only for the duration stated, outputs are written on the context's stream.
+ *  - Work is enqueued on the stream given to bh_create and is complete when the caller has
+ *    synchronised that stream, except where a call is documented as synchronising itself
+ *    (bh_build reads two small scalars back; *_host calls and bh_get_stats synchronise).
+ *  - One context = one tree = one stream.  A context is not thread-safe.
+ *  - There is no CPU fallback: without a CUDA device every compute call fails with BH_ERR_CUDA.
+ */
+#ifndef BH_H_
+#define BH_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct bh_ctx bh_ctx;
+
+/* ---- status codes ------------------------------------------------------------------------- */
+#define BH_OK               0
+#define BH_ERR_INVALID_ARG -1   /* null pointer, n <= 0, n >= 2^31, L <= 0, theta < 0 or NaN, bad option */
+#define BH_ERR_NOT_BUILT   -2   /* bh_potential / export / direct before a successful bh_build */
+#define BH_ERR_CUDA        -3   /* a CUDA runtime call failed; see bh_last_cuda_error() */
+#define BH_ERR_OOM         -4   /* device or host allocation failed */
+#define BH_ERR_TOO_LARGE   -5   /* bh_potential_direct over all n with n above BH_DIRECT_ALL_MAX; or n + nodes >= 2^32 */
+
+/* ---- options (bh_set_option) ---------------------------------------------------------------- */
+#define BH_OPT_MAC    1   /* opening criterion */
+#define BH_MAC_BH86     0 /*   Eq. 3:  accept iff d > l/theta          (default) */
+#define BH_MAC_BARNES94 1 /*   Eq. 4:  accept iff d > l/theta + delta              */
+#define BH_OPT_GROUP  2   /* how many consecutive Morton-sorted targets share one walk and one vote */
+                          /*   32 (default): the paper's warp vote; 1: per-target lists  */
+
+#define BH_MAX_LEVEL 21               /* 21 key bits per dimension -> 63-bit keys */
+#define BH_DIRECT_ALL_MAX (1 << 18)   /* largest n for bh_potential_direct with targets == NULL */
+
+/* ---- statistics ----------------------------------------------------------------------------- */
+typedef struct bh_stats {
+    int64_t n;                 /* cells of the last build                                            */
+    int64_t n_nodes;           /* internal nodes incl. level-21 bucket leaves                          */
+    int64_t n_slots;           /* records of the walk array: 1 (root) + sum of child counts           */
+    int32_t depth;             /* deepest internal-node level below 21 (0 = root only)                */
+    int32_t sort_passes;       /* 8-bit radix passes the last build executed                           */
+    int64_t n_clamped;         /* cells with a coordinate outside the cube (clamped into the edge cell) */
+    int64_t max_bucket;        /* largest number of cells sharing one 63-bit key (1 = no bucket leaves) */
+    int64_t n_accepted;        /* last walk: sum over groups of internal nodes accepted                */
+    int64_t n_leaf;            /* last walk: sum over groups of leaf cells summed directly            */
+    int64_t n_opened;          /* last walk: sum over groups of internal nodes opened                 */
+    int64_t n_exact_tests;     /* last walk: nodes whose vote needed the per-target test (diagnostic)  */
+    double  interactions;      /* last walk: sum over TARGETS of (accepted + leaf) of their group     */
+    /* device time in ms of the passes of the last bh_build / bh_potential (CUDA events) */
+    float ms_keys, ms_sort, ms_permute, ms_topology, ms_moments, ms_build_total;
+    float ms_walk;
+} bh_stats;
+
+/* ---- life cycle ----------------------------------------------------------------------------- */
+
+/* Creates a context on CUDA device `device`.  `cuda_stream` is a cudaStream_t passed as void*
+ * (NULL = the legacy default stream), e.g. torch.cuda.current_stream().cuda_stream; the caller
+ * keeps ownership of the stream and must keep it alive until bh_destroy. */
+int bh_create(bh_ctx** out, int device, void* cuda_stream);
+
+/* Frees every internal buffer (synchronises the stream first). NULL is accepted. */
+int bh_destroy(bh_ctx* ctx);
+
+const char* bh_strerror(int code);
+const char* bh_last_cuda_error(const bh_ctx* ctx);
+
+int bh_set_option(bh_ctx* ctx, int key, int value);
+
+/* ---- the hot path --------------------------------------------------------------------------- */
+
+/* bh_build: octree with monopole moments over n point masses (§2; Eq. 5).
+ *   x, y, z, m : DEVICE, const double[n] each (SoA, "arrays with a one-dimensional layout",
+ *                PAPER.md:96): cell centres and cell masses, caller's ("original") order.
+ *                Borrowed until the stream has passed this call; the context keeps sorted copies.
+ *   n          : 1 <= n < 2^31.
+ *   cube       : HOST, const double[4] = {x0, y0, z0, L}: the root cube [x0,x0+L) x ....
+ *                L > 0.  A coordinate outside the cube is clamped into the edge cell and counted
+ *                (bh_stats.n_clamped); NaN coordinates quantise to 0.
+ * Steps, all on the device: 63-bit Morton keys (DESIGN.md K-rules) -> stable LSD radix sort of
+ * (key, index) -> permutation of the cells into sorted order -> octree topology from the sorted
+ * keys (one cell per leaf, single-child chains kept, identical keys form a level-21 bucket leaf;
+ * DESIGN.md T-rules) -> bottom-up level-by-level M, R (Eq. 5), delta = |R - geometric centre|
+ * in fp64 (DESIGN.md M-rules).
+ * Synchronises the stream twice internally to read back (a) which key bits vary and (b) the node
+ * count per level; everything else is asynchronous. */
+int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, const double* m,
+             int64_t n, const double cube[4]);
+
+/* bh_potential: Phi_i = -G sum_j m_j/|r_i - r_j| over the nodes and leaf cells the group walk of
+ * PAPER.md:176-178 selects (DESIGN.md W-rules).
+ *   theta : >= 0; theta = 0 opens every node (the result is then the direct sum in fp32 terms).
+ *   G     : gravitational constant.
+ *   phi   : DEVICE, double[n], ORIGINAL cell order; every element is written.
+ * fp32 arithmetic for distances and m/d, accumulated in short fp32 blocks that are flushed into
+ * fp64 sums.  The opening decision of a node is taken in fp32 exactly as DESIGN.md W8 states. */
+int bh_potential(bh_ctx* ctx, double theta, double G, double* phi);
+
+/* bh_potential_direct: Eq. 2 written out in fp64,
+ * Phi_i = -G sum_{j != i} m_j/|r_i - r_j| over ALL n cells of the last build.
+ *   targets : DEVICE, const int64_t[nt] original cell indices in [0, n), or NULL for all n cells
+ *             (then phi has n elements and n must be <= BH_DIRECT_ALL_MAX, else BH_ERR_TOO_LARGE).
+ *             Out-of-range indices make their phi element NaN.
+ *   phi     : DEVICE, double[nt] (or double[n]); phi[a] belongs to targets[a].
+ * Pairs of distinct cells at zero distance are skipped. */
+int bh_potential_direct(bh_ctx* ctx, double G, const int64_t* targets, int64_t nt, double* phi);
+
+/* One call with HOST buffers: copies x, y, z, m (double[n] each, pageable or pinned) to the
+ * device, runs bh_build and bh_potential, copies phi (double[n]) back, synchronises. */
+int bh_solve_host(bh_ctx* ctx, const double* x, const double* y, const double* z, const double* m,
+                  int64_t n, const double cube[4], double theta, double G, double* phi);
+
+/* ---- parity / reporting --------------------------------------------------------------------- */
+
+/* Sizes of the last build (HOST outputs, any may be NULL). */
+int bh_tree_sizes(const bh_ctx* ctx, int64_t* n, int64_t* n_nodes, int64_t* n_slots);
+
+/* bh_export_tree: copies the tree of the last build into caller DEVICE buffers (any may be NULL).
+ *   keys[n]  : sorted 63-bit Morton keys            perm[n] : original index of sorted slot s
+ * and, for the n_nodes internal nodes (incl. level-21 buckets) in CANONICAL order = ascending
+ * (level, prefix) (T5):
+ *   level[i] (int32), prefix[i] (uint64 = key >> 3*(21-level)), lo[i], hi[i] (int64: sorted cell
+ *   range [lo, hi)), nchild[i] (int32; for a bucket the number of cells), M[i], Rx[i], Ry[i],
+ *   Rz[i], delta[i] (double). */
+int bh_export_tree(bh_ctx* ctx, uint64_t* keys, uint32_t* perm, int32_t* level, uint64_t* prefix,
+                   int64_t* lo, int64_t* hi, int32_t* nchild, double* M, double* Rx, double* Ry,
+                   double* Rz, double* delta);
+
+/* Per-group counts of the last bh_potential: DEVICE int64[3 * ngroups], ngroups =
+ * ceil(n / group), group g at [3g..3g+2] = {internal nodes accepted, leaf cells summed, internal
+ * nodes opened}; same definition as the oracle's counters (W6). */
+int bh_last_group_counts(bh_ctx* ctx, int64_t* counts);
+
+/* Interactions evaluated for each target in the last bh_potential (accepted + leaf of its group;
+ * the target's own cell is counted as evaluated-and-masked): DEVICE uint32[n], original order. */
+int bh_last_interactions(bh_ctx* ctx, uint32_t* per_target);
+
+/* Synchronises the stream and fills *out (HOST). */
+int bh_get_stats(bh_ctx* ctx, bh_stats* out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BH_H_ */

@@ -1,0 +1,215 @@
+"""ctypes binding of libbh (include/bh.h).  Same names as the C ABI; marshalling only."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+from . import build as _build
+
+BH_MAC_BH86 = 0       # Eq. 3
+BH_MAC_BARNES94 = 1   # Eq. 4
+BH_OPT_MAC = 1
+BH_OPT_GROUP = 2
+BH_DIRECT_ALL_MAX = 1 << 18
+
+EXPORTED_SYMBOLS = (
+    "bh_create", "bh_destroy", "bh_strerror", "bh_last_cuda_error", "bh_set_option", "bh_build", "bh_potential",
+    "bh_potential_direct", "bh_solve_host", "bh_tree_sizes", "bh_export_tree", "bh_last_group_counts",
+    "bh_last_interactions", "bh_get_stats",
+)
+
+
+class Stats(C.Structure):
+    _fields_ = [("n", C.c_int64), ("n_nodes", C.c_int64), ("n_slots", C.c_int64), ("depth", C.c_int32),
+                ("sort_passes", C.c_int32), ("n_clamped", C.c_int64), ("max_bucket", C.c_int64),
+                ("n_accepted", C.c_int64), ("n_leaf", C.c_int64), ("n_opened", C.c_int64),
+                ("n_exact_tests", C.c_int64), ("interactions", C.c_double),
+                ("ms_keys", C.c_float), ("ms_sort", C.c_float), ("ms_permute", C.c_float),
+                ("ms_topology", C.c_float), ("ms_moments", C.c_float), ("ms_build_total", C.c_float),
+                ("ms_walk", C.c_float)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+class BHError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libbh error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib_path() -> str:
+    return _build.LIB
+
+
+def lib():
+    """Loads (building first if needed) libbh.so.  Raises if it cannot be built: no fallback."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = C.CDLL(path)
+        vp, dp, i64, i32 = C.c_void_p, C.c_void_p, C.c_int64, C.c_int
+        L.bh_create.argtypes = [C.POINTER(vp), i32, vp]
+        L.bh_destroy.argtypes = [vp]
+        L.bh_strerror.argtypes = [i32]
+        L.bh_strerror.restype = C.c_char_p
+        L.bh_last_cuda_error.argtypes = [vp]
+        L.bh_last_cuda_error.restype = C.c_char_p
+        L.bh_set_option.argtypes = [vp, i32, i32]
+        L.bh_build.argtypes = [vp, dp, dp, dp, dp, i64, C.POINTER(C.c_double)]
+        L.bh_potential.argtypes = [vp, C.c_double, C.c_double, dp]
+        L.bh_potential_direct.argtypes = [vp, C.c_double, dp, i64, dp]
+        L.bh_solve_host.argtypes = [vp, dp, dp, dp, dp, i64, C.POINTER(C.c_double), C.c_double, C.c_double, dp]
+        L.bh_tree_sizes.argtypes = [vp, C.POINTER(i64), C.POINTER(i64), C.POINTER(i64)]
+        L.bh_export_tree.argtypes = [vp] + [dp] * 12
+        L.bh_last_group_counts.argtypes = [vp, dp]
+        L.bh_last_interactions.argtypes = [vp, dp]
+        L.bh_get_stats.argtypes = [vp, C.POINTER(Stats)]
+        for name in EXPORTED_SYMBOLS:
+            if name not in ("bh_strerror", "bh_last_cuda_error"):
+                getattr(L, name).restype = i32
+        _lib = L
+    return _lib
+
+
+def _cube(c):
+    return (C.c_double * 4)(*[float(v) for v in c])
+
+
+class Context:
+    """One tree on one CUDA stream (bh_create ... bh_destroy).  Tensors are torch CUDA tensors."""
+
+    def __init__(self, device: int = 0, stream=None):
+        import torch
+        self._torch = torch
+        self._L = lib()
+        self._h = C.c_void_p()
+        self.device = int(device)
+        if stream is None:
+            stream = torch.cuda.current_stream(self.device)
+        self.stream = stream
+        self._check(self._L.bh_create(C.byref(self._h), self.device, C.c_void_p(stream.cuda_stream)))
+        self.n = 0
+
+    # -- helpers ------------------------------------------------------------------------------------
+    def _check(self, rc):
+        if rc != 0:
+            msg = self._L.bh_strerror(rc).decode()
+            if self._h:
+                extra = self._L.bh_last_cuda_error(self._h).decode()
+                if extra:
+                    msg += " [" + extra + "]"
+            raise BHError(rc, msg)
+
+    def _dev(self, t, dtype):
+        torch = self._torch
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+            raise TypeError(f"expected a contiguous CUDA tensor of dtype {dtype}")
+        return C.c_void_p(t.data_ptr())
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.bh_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- the C ABI, same names ----------------------------------------------------------------------
+    def set_option(self, key: int, value: int):
+        self._check(self._L.bh_set_option(self._h, int(key), int(value)))
+
+    def set_mac(self, mac: int):
+        self.set_option(BH_OPT_MAC, mac)
+
+    def set_group(self, group: int):
+        self.set_option(BH_OPT_GROUP, group)
+
+    def build(self, x, y, z, m, cube):
+        f64 = self._torch.float64
+        n = x.numel()
+        for t in (y, z, m):
+            if t.numel() != n:
+                raise ValueError("x, y, z, m must have the same length")
+        self._check(self._L.bh_build(self._h, self._dev(x, f64), self._dev(y, f64), self._dev(z, f64),
+                                     self._dev(m, f64), n, _cube(cube)))
+        self.n = n
+
+    def potential(self, theta: float, G: float = 1.0, out=None):
+        torch = self._torch
+        if out is None:
+            out = torch.empty(self.n, dtype=torch.float64, device=f"cuda:{self.device}")
+        self._check(self._L.bh_potential(self._h, float(theta), float(G), self._dev(out, torch.float64)))
+        return out
+
+    def potential_direct(self, G: float = 1.0, targets=None, out=None):
+        torch = self._torch
+        nt = self.n if targets is None else targets.numel()
+        if out is None:
+            out = torch.empty(nt, dtype=torch.float64, device=f"cuda:{self.device}")
+        tp = C.c_void_p(0) if targets is None else self._dev(targets, torch.int64)
+        self._check(self._L.bh_potential_direct(self._h, float(G), tp, nt, self._dev(out, torch.float64)))
+        return out
+
+    def solve_host(self, x, y, z, m, cube, theta: float, G: float = 1.0, out=None):
+        """numpy / CPU-tensor float64 inputs; returns (or fills) a host float64 array."""
+        import numpy as np
+        arrs = []
+        for a in (x, y, z, m):
+            if hasattr(a, "numpy"):
+                a = a.numpy()
+            a = np.ascontiguousarray(a, dtype=np.float64)
+            arrs.append(a)
+        n = arrs[0].shape[0]
+        if out is None:
+            out = np.empty(n, dtype=np.float64)
+        o = out.numpy() if hasattr(out, "numpy") else out
+        self._check(self._L.bh_solve_host(self._h, *[C.c_void_p(a.ctypes.data) for a in arrs], n, _cube(cube),
+                                          float(theta), float(G), C.c_void_p(o.ctypes.data)))
+        self.n = n
+        return out
+
+    def tree_sizes(self):
+        n, nn, ns = C.c_int64(), C.c_int64(), C.c_int64()
+        self._check(self._L.bh_tree_sizes(self._h, C.byref(n), C.byref(nn), C.byref(ns)))
+        return n.value, nn.value, ns.value
+
+    def export_tree(self):
+        """Returns dict of CUDA tensors: keys, perm and the canonical node list."""
+        torch = self._torch
+        n, nn, _ = self.tree_sizes()
+        dev = f"cuda:{self.device}"
+        out = dict(
+            keys=torch.empty(n, dtype=torch.int64, device=dev), perm=torch.empty(n, dtype=torch.int32, device=dev),
+            level=torch.empty(nn, dtype=torch.int32, device=dev), prefix=torch.empty(nn, dtype=torch.int64, device=dev),
+            lo=torch.empty(nn, dtype=torch.int64, device=dev), hi=torch.empty(nn, dtype=torch.int64, device=dev),
+            nchild=torch.empty(nn, dtype=torch.int32, device=dev), M=torch.empty(nn, dtype=torch.float64, device=dev),
+            Rx=torch.empty(nn, dtype=torch.float64, device=dev), Ry=torch.empty(nn, dtype=torch.float64, device=dev),
+            Rz=torch.empty(nn, dtype=torch.float64, device=dev), delta=torch.empty(nn, dtype=torch.float64, device=dev))
+        order = ("keys", "perm", "level", "prefix", "lo", "hi", "nchild", "M", "Rx", "Ry", "Rz", "delta")
+        self._check(self._L.bh_export_tree(self._h, *[C.c_void_p(out[k].data_ptr()) for k in order]))
+        return out
+
+    def last_group_counts(self, group: int = 32):
+        torch = self._torch
+        ng = (self.n + group - 1) // group
+        out = torch.empty((ng, 3), dtype=torch.int64, device=f"cuda:{self.device}")
+        self._check(self._L.bh_last_group_counts(self._h, C.c_void_p(out.data_ptr())))
+        return out
+
+    def last_interactions(self):
+        torch = self._torch
+        out = torch.empty(self.n, dtype=torch.int32, device=f"cuda:{self.device}")
+        self._check(self._L.bh_last_interactions(self._h, C.c_void_p(out.data_ptr())))
+        return out
+
+    def get_stats(self) -> Stats:
+        s = Stats()
+        self._check(self._L.bh_get_stats(self._h, C.byref(s)))
+        return s

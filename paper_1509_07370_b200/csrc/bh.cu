@@ -1,0 +1,540 @@
+// bh.cu -- host side of libbh: the C ABI declared in include/bh.h.
+// Every step of the path runs in the kernels of keys.cuh / sort.cuh / scan.cuh / tree.cuh /
+// walk.cuh / direct.cuh; this file owns buffers, launches and the two scalar read-backs of bh_build.
+#include "../../include/bh.h"
+
+#include <math.h>
+#include <new>
+#include <stdio.h>
+#include <string.h>
+
+#include "common.cuh"
+#include "direct.cuh"
+#include "keys.cuh"
+#include "scan.cuh"
+#include "sort.cuh"
+#include "tree.cuh"
+#include "walk.cuh"
+
+using namespace bh;
+
+namespace {
+
+struct DevBuf {                 // grow-only device buffer
+    void* p = nullptr;
+    size_t cap = 0;
+    cudaError_t ensure(size_t bytes)
+    {
+        if (bytes <= cap) return cudaSuccess;
+        if (p) { cudaError_t e = cudaFree(p); p = nullptr; cap = 0; if (e != cudaSuccess) return e; }
+        size_t want = bytes + bytes / 16 + 256;
+        cudaError_t e = cudaMalloc(&p, want);
+        if (e != cudaSuccess) { p = nullptr; return e; }
+        cap = want;
+        return cudaSuccess;
+    }
+    void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
+    template <typename T> T* as() const { return reinterpret_cast<T*>(p); }
+};
+
+struct DeviceScalars {          // small device-resident results read back by the host
+    KeyReduce keyred;
+    u32 level_hist[kNumLevels];
+    u32 max_bucket;
+    u32 walk_overflow;
+    unsigned long long totals[5];
+};
+
+enum { EV_B0, EV_KEYS, EV_SORT, EV_PERM, EV_TOPO, EV_MOM, EV_W0, EV_W1, EV_COUNT };
+
+}  // namespace
+
+struct bh_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    int mac = BH_MAC_BH86;
+    int group = 32;
+    bool built = false;
+    bool walked = false;
+    int walk_group = 32;
+    char cuda_msg[256] = {0};
+
+    // problem
+    i64 n = 0, nn = 0, nslots = 0;
+    int depth = 0, maxlevel = 0, sort_passes = 0;
+    i64 n_clamped = 0, max_bucket = 1;
+    double cube[4] = {0, 0, 0, 1};
+    i64 level_base[kNumLevels + 1] = {0};
+
+    // per cell
+    DevBuf keysA, keysB, idxA, idxB;      // ping-pong (key, index)
+    u64* keys = nullptr;                  // sorted keys (one of keysA/keysB)
+    u32* idx = nullptr;                   // perm: original index of sorted slot
+    DevBuf leaf64, leafrec, slot_of, clev, pre_base;
+    // sort / scan scratch
+    DevBuf hist, scan_scratch;
+    // per node (pre-order, then canonical order)
+    DevBuf nkey, npre, nlo, bkey, bpre, bfs_of, blo, bhi, nchild, cstart, child_base, node_slot, mom, delta64;
+    // per slot
+    DevBuf rec, aux, slot_src;
+    // walk
+    DevBuf gcount;
+    DevBuf scalars;                       // DeviceScalars
+    DeviceScalars* h_scalars = nullptr;   // pinned host mirror
+    DevBuf stage[4];                      // bh_solve_host staging (x, y, z, m) and phi
+    DevBuf stage_phi;
+
+    cudaEvent_t ev[EV_COUNT] = {nullptr};
+    bool ev_build = false, ev_walk = false;
+};
+
+namespace {
+
+int cuda_fail(bh_ctx* c, cudaError_t e, const char* where)
+{
+    if (c) snprintf(c->cuda_msg, sizeof(c->cuda_msg), "%s: %s", where, cudaGetErrorString(e));
+    cudaGetLastError();   // clear sticky-free errors
+    return e == cudaErrorMemoryAllocation ? BH_ERR_OOM : BH_ERR_CUDA;
+}
+
+#define BH_CUDA(call)                                                    \
+    do {                                                                 \
+        cudaError_t e__ = (call);                                        \
+        if (e__ != cudaSuccess) return cuda_fail(ctx, e__, #call);       \
+    } while (0)
+
+inline unsigned blocks_for(i64 n, int threads) { return (unsigned)((n + threads - 1) / threads); }
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+int persistent_grid(const bh_ctx* ctx, int per_sm)
+{
+    int sms = 148;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, ctx->device);
+    return sms * per_sm;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* bh_strerror(int code)
+{
+    switch (code) {
+        case BH_OK: return "ok";
+        case BH_ERR_INVALID_ARG: return "invalid argument";
+        case BH_ERR_NOT_BUILT: return "no tree: call bh_build first";
+        case BH_ERR_CUDA: return "CUDA runtime error (see bh_last_cuda_error)";
+        case BH_ERR_OOM: return "out of memory";
+        case BH_ERR_TOO_LARGE: return "problem too large for this call";
+        default: return "unknown error code";
+    }
+}
+
+const char* bh_last_cuda_error(const bh_ctx* ctx) { return ctx ? ctx->cuda_msg : ""; }
+
+int bh_create(bh_ctx** out, int device, void* cuda_stream)
+{
+    if (!out) return BH_ERR_INVALID_ARG;
+    *out = nullptr;
+    int count = 0;
+    cudaError_t e = cudaGetDeviceCount(&count);
+    if (e != cudaSuccess) { cudaGetLastError(); return BH_ERR_CUDA; }   // no CPU fallback
+    if (device < 0 || device >= count) return BH_ERR_INVALID_ARG;
+    bh_ctx* ctx = new (std::nothrow) bh_ctx;
+    if (!ctx) return BH_ERR_OOM;
+    ctx->device = device;
+    ctx->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    int rc = BH_OK;
+    do {
+        if ((e = cudaSetDevice(device)) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaSetDevice"); break; }
+        int major = 0;
+        cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device);
+        if (major != 10) {
+            snprintf(ctx->cuda_msg, sizeof(ctx->cuda_msg), "device %d is sm_%d0; libbh is built for sm_100a only",
+                     device, major);
+            rc = BH_ERR_CUDA;
+            break;
+        }
+        for (int i = 0; i < EV_COUNT; ++i)
+            if ((e = cudaEventCreate(&ctx->ev[i])) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaEventCreate"); break; }
+        if (rc) break;
+        if ((e = ctx->scalars.ensure(sizeof(DeviceScalars))) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaMalloc"); break; }
+        if ((e = cudaMallocHost(&ctx->h_scalars, sizeof(DeviceScalars))) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaMallocHost"); break; }
+        if ((e = cudaFuncSetAttribute(radix_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)sizeof(SortSmem))) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(sort)"); break; }
+        if ((e = cudaFuncSetAttribute(walk_group32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      227 * 1024)) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(walk)"); break; }
+    } while (0);
+    if (rc != BH_OK) { bh_destroy(ctx); return rc; }
+    *out = ctx;
+    return BH_OK;
+}
+
+int bh_destroy(bh_ctx* ctx)
+{
+    if (!ctx) return BH_OK;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    DevBuf* all[] = {&ctx->keysA, &ctx->keysB, &ctx->idxA, &ctx->idxB, &ctx->leaf64, &ctx->leafrec, &ctx->slot_of,
+                     &ctx->clev, &ctx->pre_base, &ctx->hist, &ctx->scan_scratch, &ctx->nkey, &ctx->npre, &ctx->nlo,
+                     &ctx->bkey, &ctx->bpre, &ctx->bfs_of, &ctx->blo, &ctx->bhi, &ctx->nchild, &ctx->cstart,
+                     &ctx->child_base, &ctx->node_slot, &ctx->mom, &ctx->delta64, &ctx->rec, &ctx->aux,
+                     &ctx->slot_src, &ctx->gcount, &ctx->scalars, &ctx->stage[0], &ctx->stage[1], &ctx->stage[2],
+                     &ctx->stage[3], &ctx->stage_phi};
+    for (DevBuf* b : all) b->release();
+    if (ctx->h_scalars) cudaFreeHost(ctx->h_scalars);
+    for (int i = 0; i < EV_COUNT; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+    delete ctx;
+    return BH_OK;
+}
+
+int bh_set_option(bh_ctx* ctx, int key, int value)
+{
+    if (!ctx) return BH_ERR_INVALID_ARG;
+    if (key == BH_OPT_MAC && (value == BH_MAC_BH86 || value == BH_MAC_BARNES94)) { ctx->mac = value; return BH_OK; }
+    if (key == BH_OPT_GROUP && (value == 32 || value == 1)) { ctx->group = value; return BH_OK; }
+    return BH_ERR_INVALID_ARG;
+}
+
+int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, const double* m, int64_t n,
+             const double cube[4])
+{
+    if (!ctx || !x || !y || !z || !m || !cube) return BH_ERR_INVALID_ARG;
+    if (n <= 0 || n >= 2147483648LL || !(cube[3] > 0.0) || !isfinite(cube[0]) || !isfinite(cube[1]) ||
+        !isfinite(cube[2]) || !isfinite(cube[3]))
+        return BH_ERR_INVALID_ARG;
+    ctx->built = false;
+    ctx->walked = false;
+    BH_CUDA(cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    DeviceScalars* ds = ctx->scalars.as<DeviceScalars>();
+    ctx->n = n;
+    memcpy(ctx->cube, cube, sizeof(double) * 4);
+
+    // ---- buffers that depend on n only ----
+    BH_CUDA(ctx->keysA.ensure(sizeof(u64) * n));
+    BH_CUDA(ctx->keysB.ensure(sizeof(u64) * n));
+    BH_CUDA(ctx->idxA.ensure(sizeof(u32) * n));
+    BH_CUDA(ctx->idxB.ensure(sizeof(u32) * n));
+    BH_CUDA(ctx->leaf64.ensure(sizeof(double4) * n));
+    BH_CUDA(ctx->leafrec.ensure(sizeof(float4) * n));
+    BH_CUDA(ctx->slot_of.ensure(sizeof(u32) * n));
+    BH_CUDA(ctx->clev.ensure((size_t)n + 16));
+    BH_CUDA(ctx->pre_base.ensure(sizeof(u32) * (n + 4)));
+    BH_CUDA(ctx->hist.ensure(sizeof(u32) * (sort_hist_elems(n) + 4)));
+    BH_CUDA(ctx->scan_scratch.ensure(sizeof(u32) * (scan_scratch_elems(n > (i64)sort_hist_elems(n) ? n : (i64)sort_hist_elems(n)) + 4)));
+
+    BH_CUDA(cudaMemsetAsync(ds, 0, sizeof(DeviceScalars), st));
+    {   // key_and starts as all ones
+        const u64 ones = ~0ULL;
+        BH_CUDA(cudaMemcpyAsync(&ds->keyred.key_and, &ones, sizeof(u64), cudaMemcpyHostToDevice, st));
+    }
+    BH_CUDA(cudaEventRecord(ctx->ev[EV_B0], st));
+
+    // ---- a1: Morton keys ----
+    const double s = 2097152.0 / cube[3];      // K1: s = 2^21 / L in fp64
+    {
+        const int grid = persistent_grid(ctx, 8);
+        if (aligned16(x) && aligned16(y) && aligned16(z))
+            morton_keys_kernel<2><<<grid, 256, 0, st>>>(x, y, z, n, cube[0], cube[1], cube[2], s,
+                                                        ctx->keysA.as<u64>(), ctx->idxA.as<u32>(), &ds->keyred);
+        else
+            morton_keys_kernel<1><<<grid, 256, 0, st>>>(x, y, z, n, cube[0], cube[1], cube[2], s,
+                                                        ctx->keysA.as<u64>(), ctx->idxA.as<u32>(), &ds->keyred);
+        BH_CUDA(cudaGetLastError());
+    }
+    BH_CUDA(cudaEventRecord(ctx->ev[EV_KEYS], st));
+
+    // read-back 1: which key bits vary (decides the radix passes) and the clamp count
+    BH_CUDA(cudaMemcpyAsync(&ctx->h_scalars->keyred, &ds->keyred, sizeof(KeyReduce), cudaMemcpyDeviceToHost, st));
+    BH_CUDA(cudaStreamSynchronize(st));
+    ctx->n_clamped = (i64)ctx->h_scalars->keyred.n_clamped;
+    const SortPlan plan = make_sort_plan(ctx->h_scalars->keyred.key_or ^ ctx->h_scalars->keyred.key_and);
+    ctx->sort_passes = plan.npasses;
+
+    // ---- a2: radix sort of (key, index) ----
+    u64* k0 = ctx->keysA.as<u64>(); u64* k1 = ctx->keysB.as<u64>();
+    u32* v0 = ctx->idxA.as<u32>();  u32* v1 = ctx->idxB.as<u32>();
+    for (int p = 0; p < plan.npasses; ++p) {
+        BH_CUDA(radix_pass(k0, v0, k1, v1, n, plan.shift[p], plan.mask[p], ctx->hist.as<u32>(),
+                           ctx->scan_scratch.as<u32>(), st));
+        u64* tk = k0; k0 = k1; k1 = tk;
+        u32* tv = v0; v0 = v1; v1 = tv;
+    }
+    ctx->keys = k0;
+    ctx->idx = v0;
+    BH_CUDA(cudaEventRecord(ctx->ev[EV_SORT], st));
+
+    // ---- a3: permute ----
+    permute_kernel<<<blocks_for(n, 256), 256, 0, st>>>(ctx->idx, x, y, z, m, n, ctx->leaf64.as<double4>(),
+                                                       ctx->leafrec.as<float4>(), ctx->slot_of.as<u32>());
+    BH_CUDA(cudaGetLastError());
+    BH_CUDA(cudaEventRecord(ctx->ev[EV_PERM], st));
+
+    // ---- a4: topology ----
+    ctx->nn = 0; ctx->nslots = 0; ctx->depth = 0; ctx->maxlevel = 0; ctx->max_bucket = 1;
+    for (int l = 0; l <= kNumLevels; ++l) ctx->level_base[l] = 0;
+    if (n >= 2) {
+        u32* cnt = ctx->pre_base.as<u32>();
+        node_count_kernel<<<persistent_grid(ctx, 8), 256, 0, st>>>(ctx->keys, n, cnt, ctx->clev.as<signed char>(),
+                                                                    ds->level_hist);
+        BH_CUDA(cudaGetLastError());
+        // read-back 2: nodes per level (sizes every node / slot array)
+        BH_CUDA(cudaMemcpyAsync(ctx->h_scalars->level_hist, ds->level_hist, sizeof(u32) * kNumLevels,
+                                cudaMemcpyDeviceToHost, st));
+        BH_CUDA(exclusive_scan_u32(cnt, cnt, n, ctx->scan_scratch.as<u32>(), nullptr, st));
+        BH_CUDA(cudaStreamSynchronize(st));
+        i64 nn = 0;
+        for (int l = 0; l < kNumLevels; ++l) {
+            ctx->level_base[l] = nn;
+            const i64 c = ctx->h_scalars->level_hist[l];
+            if (c) { ctx->maxlevel = l; if (l < kMaxLevel) ctx->depth = l; }
+            nn += c;
+        }
+        ctx->level_base[kNumLevels] = nn;
+        ctx->nn = nn;
+        ctx->nslots = n + nn;
+        if (ctx->nslots >= 4294967296LL) return BH_ERR_TOO_LARGE;
+
+        BH_CUDA(ctx->nkey.ensure(sizeof(u64) * nn));
+        BH_CUDA(ctx->npre.ensure(sizeof(u32) * nn));
+        BH_CUDA(ctx->nlo.ensure(sizeof(u32) * nn));
+        BH_CUDA(ctx->bkey.ensure(sizeof(u64) * nn));
+        BH_CUDA(ctx->bpre.ensure(sizeof(u32) * nn));
+        BH_CUDA(ctx->bfs_of.ensure(sizeof(u32) * nn));
+        BH_CUDA(ctx->blo.ensure(sizeof(u32) * nn));
+        BH_CUDA(ctx->bhi.ensure(sizeof(u32) * nn));
+        BH_CUDA(ctx->nchild.ensure(sizeof(u32) * (nn + 4)));
+        BH_CUDA(ctx->cstart.ensure(sizeof(u32) * 8 * nn));
+        BH_CUDA(ctx->child_base.ensure(sizeof(u32) * (nn + 4)));
+        BH_CUDA(ctx->node_slot.ensure(sizeof(u32) * nn));
+        BH_CUDA(ctx->mom.ensure(sizeof(double4) * nn));
+        BH_CUDA(ctx->delta64.ensure(sizeof(double) * nn));
+        BH_CUDA(ctx->rec.ensure(sizeof(float4) * ctx->nslots));
+        BH_CUDA(ctx->aux.ensure(sizeof(WalkAux) * ctx->nslots));
+        BH_CUDA(ctx->slot_src.ensure(sizeof(int) * ctx->nslots));
+        BH_CUDA(ctx->hist.ensure(sizeof(u32) * (sort_hist_elems(nn) + 4)));
+        BH_CUDA(ctx->scan_scratch.ensure(sizeof(u32) * (scan_scratch_elems(nn > (i64)sort_hist_elems(nn) ? nn : (i64)sort_hist_elems(nn)) + 4)));
+
+        node_emit_kernel<<<blocks_for(n, 256), 256, 0, st>>>(ctx->clev.as<signed char>(), cnt, n, ctx->nkey.as<u64>(),
+                                                             ctx->npre.as<u32>(), ctx->nlo.as<u32>());
+        BH_CUDA(cudaGetLastError());
+        // pre-order -> canonical (level, prefix) order: one stable counting pass on the level
+        BH_CUDA(radix_pass(ctx->nkey.as<u64>(), ctx->npre.as<u32>(), ctx->bkey.as<u64>(), ctx->bpre.as<u32>(), nn, 0,
+                           0xffu, ctx->hist.as<u32>(), ctx->scan_scratch.as<u32>(), st));
+        node_children_kernel<<<blocks_for(nn, 256), 256, 0, st>>>(
+            ctx->keys, n, ctx->bkey.as<u64>(), ctx->bpre.as<u32>(), ctx->nlo.as<u32>(), nn, ctx->bfs_of.as<u32>(),
+            ctx->blo.as<u32>(), ctx->bhi.as<u32>(), ctx->nchild.as<u32>(), ctx->cstart.as<u32>(), &ds->max_bucket);
+        BH_CUDA(cudaGetLastError());
+        BH_CUDA(exclusive_scan_u32(ctx->nchild.as<u32>(), ctx->child_base.as<u32>(), nn, ctx->scan_scratch.as<u32>(),
+                                   nullptr, st));
+        slot_fill_kernel<<<blocks_for(nn * 8, 256), 256, 0, st>>>(
+            ctx->bkey.as<u64>(), ctx->bpre.as<u32>(), ctx->blo.as<u32>(), ctx->bhi.as<u32>(), ctx->nchild.as<u32>(),
+            ctx->cstart.as<u32>(), ctx->child_base.as<u32>(), cnt, ctx->bfs_of.as<u32>(), nn,
+            ctx->leafrec.as<float4>(), ctx->slot_src.as<int>(), ctx->node_slot.as<u32>(), ctx->rec.as<float4>(),
+            ctx->aux.as<WalkAux>());
+        BH_CUDA(cudaGetLastError());
+        BH_CUDA(cudaEventRecord(ctx->ev[EV_TOPO], st));
+
+        // ---- a5: moments, deepest level first ----
+        for (int l = ctx->maxlevel; l >= 0; --l) {
+            const i64 b0 = ctx->level_base[l], b1 = ctx->level_base[l + 1];
+            if (b1 == b0) continue;
+            moments_kernel<<<blocks_for(b1 - b0, 128), 128, 0, st>>>(
+                b0, b1, l, ctx->keys, ctx->blo.as<u32>(), ctx->nchild.as<u32>(), ctx->child_base.as<u32>(),
+                ctx->slot_src.as<int>(), ctx->node_slot.as<u32>(), ctx->leaf64.as<double4>(), ctx->mom.as<double4>(),
+                ctx->delta64.as<double>(), ctx->rec.as<float4>(), ctx->aux.as<WalkAux>(), cube[0], cube[1], cube[2],
+                cube[3]);
+            BH_CUDA(cudaGetLastError());
+        }
+    } else {
+        BH_CUDA(cudaEventRecord(ctx->ev[EV_TOPO], st));
+    }
+    BH_CUDA(cudaEventRecord(ctx->ev[EV_MOM], st));
+    ctx->ev_build = true;
+    ctx->built = true;
+    return BH_OK;
+}
+
+int bh_potential(bh_ctx* ctx, double theta, double G, double* phi)
+{
+    if (!ctx || !phi || !(theta >= 0.0) || isnan(G)) return BH_ERR_INVALID_ARG;
+    if (!ctx->built) return BH_ERR_NOT_BUILT;
+    BH_CUDA(cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    const i64 n = ctx->n;
+    if (ctx->group != 32) {
+        snprintf(ctx->cuda_msg, sizeof(ctx->cuda_msg), "BH_OPT_GROUP=1 walk is not built yet");
+        return BH_ERR_INVALID_ARG;
+    }
+    const i64 ngroups = (n + 31) / 32;
+    BH_CUDA(ctx->gcount.ensure(sizeof(uint4) * ngroups));
+    BH_CUDA(cudaEventRecord(ctx->ev[EV_W0], st));
+    if (n == 1) {   // T-rule 1: a lone cell has no tree; Phi = 0
+        BH_CUDA(cudaMemsetAsync(phi, 0, sizeof(double), st));
+        BH_CUDA(cudaMemsetAsync(ctx->gcount.p, 0, sizeof(uint4), st));
+    } else {
+        WalkParams P;
+        P.rec = ctx->rec.as<float4>();
+        P.aux = ctx->aux.as<WalkAux>();
+        P.leafrec = ctx->leafrec.as<float4>();
+        P.idx = ctx->idx;
+        P.phi = phi;
+        P.gcount = ctx->gcount.as<uint4>();
+        P.n = n;
+        P.ngroups = ngroups;
+        P.inv_theta = (float)(1.0 / theta);
+        P.mac = ctx->mac;
+        P.negG = -G;
+        i64 cap = (i64)kStackPerLevel * (ctx->maxlevel + 2) + 32;
+        cap = (cap + 1) & ~1LL;
+        const size_t smem = walk_smem_per_warp((int)cap) * kWalkWarps;
+        if (smem > 227 * 1024) return BH_ERR_TOO_LARGE;
+        P.stack_cap = (int)cap;
+        walk_group32_kernel<<<blocks_for(ngroups, kWalkWarps), kWalkWarps * 32, smem, st>>>(P);
+        BH_CUDA(cudaGetLastError());
+    }
+    BH_CUDA(cudaEventRecord(ctx->ev[EV_W1], st));
+    ctx->ev_walk = true;
+    ctx->walked = true;
+    ctx->walk_group = 32;
+    return BH_OK;
+}
+
+int bh_potential_direct(bh_ctx* ctx, double G, const int64_t* targets, int64_t nt, double* phi)
+{
+    if (!ctx || !phi || isnan(G)) return BH_ERR_INVALID_ARG;
+    if (!ctx->built) return BH_ERR_NOT_BUILT;
+    if (!targets) {
+        if (ctx->n > BH_DIRECT_ALL_MAX) return BH_ERR_TOO_LARGE;
+        nt = ctx->n;
+    } else if (nt < 0) return BH_ERR_INVALID_ARG;
+    if (nt == 0) return BH_OK;
+    BH_CUDA(cudaSetDevice(ctx->device));
+    direct_kernel<<<blocks_for(nt, kDirectThreads), kDirectThreads, 0, ctx->stream>>>(
+        ctx->leaf64.as<double4>(), ctx->n, ctx->slot_of.as<u32>(), reinterpret_cast<const i64*>(targets), nt, -G, phi);
+    BH_CUDA(cudaGetLastError());
+    return BH_OK;
+}
+
+int bh_solve_host(bh_ctx* ctx, const double* x, const double* y, const double* z, const double* m, int64_t n,
+                  const double cube[4], double theta, double G, double* phi)
+{
+    if (!ctx || !x || !y || !z || !m || !cube || !phi || n <= 0 || n >= 2147483648LL) return BH_ERR_INVALID_ARG;
+    BH_CUDA(cudaSetDevice(ctx->device));
+    const double* src[4] = {x, y, z, m};
+    for (int k = 0; k < 4; ++k) {
+        BH_CUDA(ctx->stage[k].ensure(sizeof(double) * n));
+        BH_CUDA(cudaMemcpyAsync(ctx->stage[k].p, src[k], sizeof(double) * n, cudaMemcpyHostToDevice, ctx->stream));
+    }
+    BH_CUDA(ctx->stage_phi.ensure(sizeof(double) * n));
+    int rc = bh_build(ctx, ctx->stage[0].as<double>(), ctx->stage[1].as<double>(), ctx->stage[2].as<double>(),
+                      ctx->stage[3].as<double>(), n, cube);
+    if (rc != BH_OK) return rc;
+    rc = bh_potential(ctx, theta, G, ctx->stage_phi.as<double>());
+    if (rc != BH_OK) return rc;
+    BH_CUDA(cudaMemcpyAsync(phi, ctx->stage_phi.p, sizeof(double) * n, cudaMemcpyDeviceToHost, ctx->stream));
+    BH_CUDA(cudaStreamSynchronize(ctx->stream));
+    return BH_OK;
+}
+
+int bh_tree_sizes(const bh_ctx* ctx, int64_t* n, int64_t* n_nodes, int64_t* n_slots)
+{
+    if (!ctx) return BH_ERR_INVALID_ARG;
+    if (!ctx->built) return BH_ERR_NOT_BUILT;
+    if (n) *n = ctx->n;
+    if (n_nodes) *n_nodes = ctx->nn;
+    if (n_slots) *n_slots = ctx->nslots;
+    return BH_OK;
+}
+
+int bh_export_tree(bh_ctx* ctx, uint64_t* keys, uint32_t* perm, int32_t* level, uint64_t* prefix, int64_t* lo,
+                   int64_t* hi, int32_t* nchild, double* M, double* Rx, double* Ry, double* Rz, double* delta)
+{
+    if (!ctx) return BH_ERR_INVALID_ARG;
+    if (!ctx->built) return BH_ERR_NOT_BUILT;
+    BH_CUDA(cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    if (keys) BH_CUDA(cudaMemcpyAsync(keys, ctx->keys, sizeof(u64) * ctx->n, cudaMemcpyDeviceToDevice, st));
+    if (perm) BH_CUDA(cudaMemcpyAsync(perm, ctx->idx, sizeof(u32) * ctx->n, cudaMemcpyDeviceToDevice, st));
+    if (ctx->nn > 0) {
+        export_nodes_kernel<<<blocks_for(ctx->nn, 256), 256, 0, st>>>(
+            ctx->nn, ctx->keys, ctx->bkey.as<u64>(), ctx->blo.as<u32>(), ctx->bhi.as<u32>(), ctx->nchild.as<u32>(),
+            ctx->mom.as<double4>(), ctx->delta64.as<double>(), level, reinterpret_cast<u64*>(prefix),
+            reinterpret_cast<i64*>(lo), reinterpret_cast<i64*>(hi), nchild, M, Rx, Ry, Rz, delta);
+        BH_CUDA(cudaGetLastError());
+    }
+    return BH_OK;
+}
+
+int bh_last_group_counts(bh_ctx* ctx, int64_t* counts)
+{
+    if (!ctx || !counts) return BH_ERR_INVALID_ARG;
+    if (!ctx->walked) return BH_ERR_NOT_BUILT;
+    BH_CUDA(cudaSetDevice(ctx->device));
+    const i64 ng = (ctx->n + ctx->walk_group - 1) / ctx->walk_group;
+    group_counts_export_kernel<<<blocks_for(ng, 256), 256, 0, ctx->stream>>>(ctx->gcount.as<uint4>(), ng,
+                                                                             reinterpret_cast<i64*>(counts));
+    BH_CUDA(cudaGetLastError());
+    return BH_OK;
+}
+
+int bh_last_interactions(bh_ctx* ctx, uint32_t* per_target)
+{
+    if (!ctx || !per_target) return BH_ERR_INVALID_ARG;
+    if (!ctx->walked) return BH_ERR_NOT_BUILT;
+    BH_CUDA(cudaSetDevice(ctx->device));
+    per_target_counts_kernel<<<blocks_for(ctx->n, 256), 256, 0, ctx->stream>>>(ctx->gcount.as<uint4>(), ctx->idx,
+                                                                               ctx->n, ctx->walk_group, per_target);
+    BH_CUDA(cudaGetLastError());
+    return BH_OK;
+}
+
+int bh_get_stats(bh_ctx* ctx, bh_stats* out)
+{
+    if (!ctx || !out) return BH_ERR_INVALID_ARG;
+    memset(out, 0, sizeof(*out));
+    if (!ctx->built) return BH_ERR_NOT_BUILT;
+    BH_CUDA(cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    DeviceScalars* ds = ctx->scalars.as<DeviceScalars>();
+    if (ctx->walked) {
+        const i64 ng = (ctx->n + ctx->walk_group - 1) / ctx->walk_group;
+        BH_CUDA(cudaMemsetAsync(ds->totals, 0, sizeof(ds->totals), st));
+        group_counts_total_kernel<<<persistent_grid(ctx, 2), 256, 0, st>>>(ctx->gcount.as<uint4>(), ng, ctx->n,
+                                                                          ctx->walk_group, ds->totals);
+        BH_CUDA(cudaGetLastError());
+        BH_CUDA(cudaMemcpyAsync(ctx->h_scalars->totals, ds->totals, sizeof(ds->totals), cudaMemcpyDeviceToHost, st));
+    }
+    BH_CUDA(cudaMemcpyAsync(&ctx->h_scalars->max_bucket, &ds->max_bucket, sizeof(u32), cudaMemcpyDeviceToHost, st));
+    BH_CUDA(cudaStreamSynchronize(st));
+    ctx->max_bucket = ctx->h_scalars->max_bucket > 1 ? ctx->h_scalars->max_bucket : 1;
+    out->n = ctx->n;
+    out->n_nodes = ctx->nn;
+    out->n_slots = ctx->nslots;
+    out->depth = ctx->depth;
+    out->sort_passes = ctx->sort_passes;
+    out->n_clamped = ctx->n_clamped;
+    out->max_bucket = ctx->max_bucket;
+    if (ctx->walked) {
+        out->n_accepted = (i64)ctx->h_scalars->totals[0];
+        out->n_leaf = (i64)ctx->h_scalars->totals[1];
+        out->n_opened = (i64)ctx->h_scalars->totals[2];
+        out->n_exact_tests = (i64)ctx->h_scalars->totals[3];
+        out->interactions = (double)ctx->h_scalars->totals[4];
+    }
+    if (ctx->ev_build) {
+        cudaEventElapsedTime(&out->ms_keys, ctx->ev[EV_B0], ctx->ev[EV_KEYS]);
+        cudaEventElapsedTime(&out->ms_sort, ctx->ev[EV_KEYS], ctx->ev[EV_SORT]);
+        cudaEventElapsedTime(&out->ms_permute, ctx->ev[EV_SORT], ctx->ev[EV_PERM]);
+        cudaEventElapsedTime(&out->ms_topology, ctx->ev[EV_PERM], ctx->ev[EV_TOPO]);
+        cudaEventElapsedTime(&out->ms_moments, ctx->ev[EV_TOPO], ctx->ev[EV_MOM]);
+        cudaEventElapsedTime(&out->ms_build_total, ctx->ev[EV_B0], ctx->ev[EV_MOM]);
+    }
+    if (ctx->ev_walk) cudaEventElapsedTime(&out->ms_walk, ctx->ev[EV_W0], ctx->ev[EV_W1]);
+    cudaGetLastError();
+    return BH_OK;
+}
+
+}  // extern "C"
