@@ -1,0 +1,332 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the Barnes-Hut hot path (bh_build + bh_potential) on B200.
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: 63-bit Morton keys ->
+radix sort -> permute -> octree topology -> monopole moments -> group tree walk -> Phi scattered to
+the original order.  Workload at N=1: BASELINE.json configs[3], the 256^3 turbulent medium
+(16,777,216 cells, theta = 0.5) -- the configuration the north-star's 40 % FP32 / 60 % HBM bars are
+stated on.  `value` = cells/s of build+walk with inputs resident in HBM; the walk's interactions/s
+and the roofline of the dominant kernel (the walk) are reported beside it.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+
+N > 1 (torchrun): the path is scoped to one GPU: every rank
+runs an independent replica of the workload ("replicas only", weak scaling, no collective on the data
+path); time = max over ranks.
+--impl reference: the fp64 CPU oracle (oracle/), as it stands, on the host cores, on a bounded
+sample of the same workload per step.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+FLOPS_PER_INTERACTION = 13          # north-star convention (BASELINE.json)
+FP32_LANES_PER_SM = 128
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return float(d.get("hbm_gbs", 6650.0)), float(d.get("sm_max_mhz", 1965.0)), "measured"
+    return 6650.0, 1965.0, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.lines = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [t.strip() for t in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for k, nm in enumerate(names):
+                if f[3 + k].lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def build_bytes_per_cell(n, n_nodes, sort_passes):
+    """Algorithmic HBM bytes of bh_build per cell."""
+    keys = 36.0
+    sort = sort_passes * (8.0 + 24.0)                # classic pass: histogram read + read/write of 12 B
+    permute = 84.0 + 4.0
+    topo = 8.0 + 5.0 + (n_nodes / n) * 24.0
+    mom = 32.0 + (n_nodes / n) * 72.0
+    return keys + sort + permute + topo + mom
+
+
+def oracle_step(w, orc, n_sample_groups, phi_buf):
+    """One pass of the oracle as it stands: full build, then the group walk on `n_sample_groups`
+    groups taken as 16 evenly spaced contiguous runs; walk time is extrapolated linearly to all
+    groups (groups are independent).  Returns (t_build, t_walk_extrapolated, interactions_sampled,
+    targets_sampled)."""
+    import numpy as np
+    t0 = time.perf_counter()
+    ot = orc.OracleTree(w.x, w.y, w.z, w.m, w.cube)
+    t_build = time.perf_counter() - t0
+    ng = (w.n + 31) // 32
+    ns = min(n_sample_groups, ng)
+    runs = 16 if ns >= 64 else 1
+    per = max(ns // runs, 1)
+    inter = 0
+    targets = 0
+    t_walk = 0.0
+    for r in range(runs):
+        g0 = min((ng // runs) * r + (ng // runs - per) // 2, ng - per)
+        t1 = time.perf_counter()
+        _, cnt = ot.potential(w.theta, w.G, group=32, groups=(g0, g0 + per), want_counts=True, out=phi_buf)
+        t_walk += time.perf_counter() - t1
+        members = np.minimum(32, w.n - 32 * np.arange(g0, g0 + per))
+        inter += int(((cnt[:, 0] + cnt[:, 1]) * members).sum())
+        targets += int(members.sum())
+    walked = runs * per
+    del ot
+    return t_build, t_walk * (ng / walked), inter, targets, walked
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores; rank 0 only."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import numpy as np
+    import bh_workloads as wl
+    import oracle as orc
+    orc.build_library()
+    w = wl.by_name(args.workload)
+    w.theta = args.theta
+    phi_buf = np.full(w.n, np.nan)
+    times = []
+    inter = tg = walked = 0
+    for it in range(args.warmup + args.steps):
+        tb, tw, inter, tg, walked = oracle_step(w, orc, args.ref_groups, phi_buf)
+        if it >= args.warmup:
+            times.append((tb, tw))
+    tb = sum(t[0] for t in times) / len(times)
+    tw = sum(t[1] for t in times) / len(times)
+    value = w.n / (tb + tw)
+    ng = (w.n + 31) // 32
+    sample = (f"full fp64 build of {w.n} cells + group walk of {walked} of {ng} groups (16 evenly spaced runs), "
+              f"walk time scaled by {ng / walked:.1f}; single thread")
+    line = {
+        "impl": "reference", "metric": "cells_per_s_build_plus_walk", "value": value, "unit": "cells/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": (tb + tw) * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "n_cells": w.n, "theta": w.theta, "group": 32, "mac": "eq3"},
+        "walk_interactions_per_s": (inter / tg) * w.n / tw,
+        "cpu_baseline": {"value": value, "unit": "cells/s", "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "cells/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import bh_workloads as wl
+    import paper_1509_07370_b200 as bh
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: libbh has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+
+    hbm_gbs, sm_max_mhz, peak_src = _peaks()
+    w = wl.by_name(args.workload)
+    w.theta = args.theta
+    n = w.n
+    dev = f"cuda:{local}"
+    host = [torch.from_numpy(np.ascontiguousarray(a)).pin_memory() for a in (w.x, w.y, w.z, w.m)]
+    d = [t.to(dev, non_blocking=False) for t in host]
+    phi = torch.empty(n, dtype=torch.float64, device=dev)
+    ctx = bh.Context(local)
+
+    def step():
+        ctx.build(d[0], d[1], d[2], d[3], w.cube)
+        ctx.potential(w.theta, w.G, out=phi)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    st = ctx.get_stats()
+    launches_per_step = st.launches_build + st.launches_walk
+
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    sampler = ClockSampler(local)
+    sampler.start()
+    if dist:
+        dist.barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for k in range(args.steps):
+        ev[k][0].record()
+        ctx.build(d[0], d[1], d[2], d[3], w.cube)
+        ev[k][1].record()
+        ctx.potential(w.theta, w.G, out=phi)
+        ev[k][2].record()
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    elapsed = time.perf_counter() - t0
+    clocks = sampler.stop()
+    dev_total = ev[0][0].elapsed_time(ev[-1][2]) / 1e3          # device time first event -> last event
+    t_build = sum(e[0].elapsed_time(e[1]) for e in ev) / args.steps / 1e3
+    t_walk = sum(e[1].elapsed_time(e[2]) for e in ev) / args.steps / 1e3
+    t = torch.tensor([dev_total, elapsed], dtype=torch.float64, device=dev)
+    if dist:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dev_total, elapsed = float(t[0]), float(t[1])
+    st = ctx.get_stats()
+
+    # ---- e2e: the public host-buffer call, copies inside the timed region ----
+    e2e_steps = max(1, min(args.steps, 5))
+    phi_host = torch.empty(n, dtype=torch.float64).pin_memory()
+    hx = [t.numpy() for t in host]
+    ctx.solve_host(hx[0], hx[1], hx[2], hx[3], w.cube, w.theta, w.G, out=phi_host.numpy())
+    if dist:
+        dist.barrier()
+    torch.cuda.synchronize()
+    t1 = time.perf_counter()
+    for _ in range(e2e_steps):
+        ctx.solve_host(hx[0], hx[1], hx[2], hx[3], w.cube, w.theta, w.G, out=phi_host.numpy())
+    torch.cuda.synchronize()
+    e2e_t = time.perf_counter() - t1
+    te = torch.tensor([e2e_t], dtype=torch.float64, device=dev)
+    if dist:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_t = float(te[0])
+
+    if rank != 0:
+        if dist:
+            dist.destroy_process_group()
+        return 0
+
+    inter = st.interactions
+    fp32_peak_tflops = st_sms(local) * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
+    walk_tflops = inter * FLOPS_PER_INTERACTION / t_walk / 1e12
+    bpc = build_bytes_per_cell(n, st.n_nodes, st.sort_passes)
+    line = {
+        "metric": "cells_per_s_build_plus_walk", "value": world * n * args.steps / dev_total, "unit": "cells/s",
+        "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": dev_total / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": w.name, "n_cells": n, "theta": w.theta, "group": 32, "mac": "eq3", "G": w.G,
+                   "l2": "inputs_exceed_l2 (4 x %.0f MB fp64 arrays re-read every step)" % (n * 8 / 1e6),
+                   "parallelism": "replicas x%d" % world, "timing": "cuda events, max over ranks",
+                   "wall_ms_per_step": elapsed / args.steps * 1e3},
+        "walk_interactions_per_s": world * inter / t_walk,
+        "interactions_per_target": inter / n,
+        "ms_build": t_build * 1e3, "ms_walk": t_walk * 1e3,
+        "build_passes_ms": {"keys": st.ms_keys, "sort": st.ms_sort, "permute": st.ms_permute,
+                            "topology": st.ms_topology, "moments": st.ms_moments},
+        "tree": {"n_nodes": st.n_nodes, "depth": st.depth, "sort_passes": st.sort_passes,
+                 "exact_tests_per_group": st.n_exact_tests / ((n + 31) // 32)},
+        "roofline": {"bound": "alu", "kernel": "walk_group32_kernel", "achieved": walk_tflops, "peak": fp32_peak_tflops,
+                     "unit": "TFLOP/s", "frac": walk_tflops / fp32_peak_tflops, "traffic": None,
+                     "peak_source": "nominal FP32: %d SMs x 128 lanes x 2 x %.0f MHz (sm_max_mhz, MEASURED_PEAKS.json %s); "
+                                    "13 flops/interaction" % (st_sms(local), sm_max_mhz, peak_src),
+                     "build_hbm": {"achieved": bpc * n / t_build / 1e9, "peak": hbm_gbs, "unit": "GB/s",
+                                   "frac": bpc * n / t_build / 1e9 / hbm_gbs, "bytes_per_cell": bpc,
+                                   "peak_source": peak_src}},
+        "clocks": clocks,
+        "e2e": {"value": world * n * e2e_steps / e2e_t, "unit": "cells/s", "h2d_bytes_per_step": 4 * 8 * n,
+                "d2h_bytes_per_step": 8 * n, "steps": e2e_steps, "api": "bh_solve_host (pinned host buffers)"},
+        "gpu_launches": launches_per_step * args.steps,
+    }
+    if not args.no_cpu_baseline and world == 1:
+        import oracle as orc
+        orc.build_library()
+        phi_buf = np.full(n, np.nan)
+        tb, tw, oi, otg, walked = oracle_step(w, orc, args.ref_groups, phi_buf)
+        ng = (n + 31) // 32
+        line["cpu_baseline"] = {
+            "value": n / (tb + tw), "unit": "cells/s", "cores": 1, "kind": "oracle",
+            "sample": f"full fp64 build ({tb:.1f} s) + group walk of {walked} of {ng} groups "
+                      f"(16 evenly spaced runs), walk time scaled by {ng / walked:.1f} to {tw:.1f} s",
+            "walk_interactions_per_s": (oi / otg) * n / tw, "host_cpus": os.cpu_count()}
+    print(json.dumps(line))
+    if dist:
+        dist.destroy_process_group()
+    return 0
+
+
+def st_sms(index):
+    import torch
+    return torch.cuda.get_device_properties(index).multi_processor_count
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="turb256")
+    ap.add_argument("--theta", type=float, default=0.5)
+    ap.add_argument("--ref-groups", type=int, default=4096, help="groups the oracle walks per step (sample)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

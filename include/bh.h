@@ -69,6 +69,8 @@ typedef struct bh_stats {
     /* device time in ms of the passes of the last bh_build / bh_potential (CUDA events) */
     float ms_keys, ms_sort, ms_permute, ms_topology, ms_moments, ms_build_total;
     float ms_walk;
+    int32_t launches_build;    /* kernels the last bh_build launched                                   */
+    int32_t launches_walk;     /* kernels the last bh_potential launched                               */
 } bh_stats;
 
 /* ---- life cycle ----------------------------------------------------------------------------- */

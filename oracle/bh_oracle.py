@@ -140,13 +140,14 @@ class OracleTree:
                               _p(out["delta"], C.c_double), _p(out["nchild"], C.c_int32))
         return out
 
-    def potential(self, theta, G=1.0, mac=MAC_BH86, group=32, mac_fp32=False, groups=None, want_counts=False):
+    def potential(self, theta, G=1.0, mac=MAC_BH86, group=32, mac_fp32=False, groups=None, want_counts=False,
+                  out=None):
         """Group walk (W-rules).  Returns phi in ORIGINAL order (NaN where not walked when `groups`
         = (begin, end) restricts the walk) and, if asked, counts[ngroups_walked, 3] =
-        (accepted nodes, leaf cells, opened nodes)."""
+        (accepted nodes, leaf cells, opened nodes).  `out`: reuse a float64[n] buffer (marshalling only)."""
         ng = (self.n + group - 1) // group
         gb, ge = (0, ng) if groups is None else groups
-        phi = np.full(self.n, np.nan)
+        phi = np.full(self.n, np.nan) if out is None else out
         counts = np.zeros((max(ge - gb, 0), 3), dtype=np.int64)
         rc = _L().orc_potential(self._h, float(theta), float(G), int(mac), int(group), int(bool(mac_fp32)),
                                 gb, ge, _p(phi, C.c_double), _p(counts, C.c_int64))

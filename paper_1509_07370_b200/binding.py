@@ -26,7 +26,7 @@ class Stats(C.Structure):
                 ("n_exact_tests", C.c_int64), ("interactions", C.c_double),
                 ("ms_keys", C.c_float), ("ms_sort", C.c_float), ("ms_permute", C.c_float),
                 ("ms_topology", C.c_float), ("ms_moments", C.c_float), ("ms_build_total", C.c_float),
-                ("ms_walk", C.c_float)]
+                ("ms_walk", C.c_float), ("launches_build", C.c_int32), ("launches_walk", C.c_int32)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

@@ -86,6 +86,7 @@ struct bh_ctx {
 
     cudaEvent_t ev[EV_COUNT] = {nullptr};
     bool ev_build = false, ev_walk = false;
+    int launches_build = 0, launches_walk = 0;
 };
 
 namespace {
@@ -206,6 +207,7 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
         return BH_ERR_INVALID_ARG;
     ctx->built = false;
     ctx->walked = false;
+    ctx->launches_build = 0;
     BH_CUDA(cudaSetDevice(ctx->device));
     cudaStream_t st = ctx->stream;
     DeviceScalars* ds = ctx->scalars.as<DeviceScalars>();
@@ -244,6 +246,7 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
                                                         ctx->keysA.as<u64>(), ctx->idxA.as<u32>(), &ds->keyred);
         BH_CUDA(cudaGetLastError());
     }
+    ctx->launches_build += 1;
     BH_CUDA(cudaEventRecord(ctx->ev[EV_KEYS], st));
 
     // read-back 1: which key bits vary (decides the radix passes) and the clamp count
@@ -259,6 +262,7 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
     for (int p = 0; p < plan.npasses; ++p) {
         BH_CUDA(radix_pass(k0, v0, k1, v1, n, plan.shift[p], plan.mask[p], ctx->hist.as<u32>(),
                            ctx->scan_scratch.as<u32>(), st));
+        ctx->launches_build += 5;   // histogram + 3 scan kernels + scatter
         u64* tk = k0; k0 = k1; k1 = tk;
         u32* tv = v0; v0 = v1; v1 = tv;
     }
@@ -270,6 +274,7 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
     permute_kernel<<<blocks_for(n, 256), 256, 0, st>>>(ctx->idx, x, y, z, m, n, ctx->leaf64.as<double4>(),
                                                        ctx->leafrec.as<float4>(), ctx->slot_of.as<u32>());
     BH_CUDA(cudaGetLastError());
+    ctx->launches_build += 1;
     BH_CUDA(cudaEventRecord(ctx->ev[EV_PERM], st));
 
     // ---- a4: topology ----
@@ -335,6 +340,7 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
             ctx->leafrec.as<float4>(), ctx->slot_src.as<int>(), ctx->node_slot.as<u32>(), ctx->rec.as<float4>(),
             ctx->aux.as<WalkAux>());
         BH_CUDA(cudaGetLastError());
+        ctx->launches_build += 1 + 3 + 1 + 5 + 1 + 3 + 1;   // count, scan, emit, level pass, children, scan, fill
         BH_CUDA(cudaEventRecord(ctx->ev[EV_TOPO], st));
 
         // ---- a5: moments, deepest level first ----
@@ -347,6 +353,7 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
                 ctx->delta64.as<double>(), ctx->rec.as<float4>(), ctx->aux.as<WalkAux>(), cube[0], cube[1], cube[2],
                 cube[3]);
             BH_CUDA(cudaGetLastError());
+            ctx->launches_build += 1;
         }
     } else {
         BH_CUDA(cudaEventRecord(ctx->ev[EV_TOPO], st));
@@ -370,6 +377,7 @@ int bh_potential(bh_ctx* ctx, double theta, double G, double* phi)
     }
     const i64 ngroups = (n + 31) / 32;
     BH_CUDA(ctx->gcount.ensure(sizeof(uint4) * ngroups));
+    ctx->launches_walk = 0;
     BH_CUDA(cudaEventRecord(ctx->ev[EV_W0], st));
     if (n == 1) {   // T-rule 1: a lone cell has no tree; Phi = 0
         BH_CUDA(cudaMemsetAsync(phi, 0, sizeof(double), st));
@@ -394,6 +402,7 @@ int bh_potential(bh_ctx* ctx, double theta, double G, double* phi)
         P.stack_cap = (int)cap;
         walk_group32_kernel<<<blocks_for(ngroups, kWalkWarps), kWalkWarps * 32, smem, st>>>(P);
         BH_CUDA(cudaGetLastError());
+        ctx->launches_walk = 1;
     }
     BH_CUDA(cudaEventRecord(ctx->ev[EV_W1], st));
     ctx->ev_walk = true;
@@ -533,6 +542,8 @@ int bh_get_stats(bh_ctx* ctx, bh_stats* out)
         cudaEventElapsedTime(&out->ms_build_total, ctx->ev[EV_B0], ctx->ev[EV_MOM]);
     }
     if (ctx->ev_walk) cudaEventElapsedTime(&out->ms_walk, ctx->ev[EV_W0], ctx->ev[EV_W1]);
+    out->launches_build = ctx->launches_build;
+    out->launches_walk = ctx->launches_walk;
     cudaGetLastError();
     return BH_OK;
 }

@@ -33,8 +33,8 @@ def test_strerror_and_stats_layout():
     L = pkg.lib()
     assert L.bh_strerror(0) == b"ok"
     assert b"invalid" in L.bh_strerror(-1)
-    # struct bh_stats: 3*8 + 2*4 + 6*8 + 8 + 7*4 (+4 pad) bytes
-    assert C.sizeof(pkg.Stats) == 120
+    # struct bh_stats: 3*8 + 2*4 + 6*8 + 8 + 7*4 + 2*4 (+4 pad) bytes
+    assert C.sizeof(pkg.Stats) == 128
 
 
 def test_no_cpu_fallback_without_device():
