@@ -164,7 +164,7 @@ int bh_create(bh_ctx** out, int device, void* cuda_stream)
         if ((e = cudaMallocHost(&ctx->h_scalars, sizeof(DeviceScalars))) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaMallocHost"); break; }
         if ((e = cudaFuncSetAttribute(radix_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       (int)sizeof(SortSmem))) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(sort)"); break; }
-        if ((e = cudaFuncSetAttribute(walk_group32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        if ((e = cudaFuncSetAttribute(walk_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       227 * 1024)) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(walk)"); break; }
     } while (0);
     if (rc != BH_OK) { bh_destroy(ctx); return rc; }
@@ -371,11 +371,8 @@ int bh_potential(bh_ctx* ctx, double theta, double G, double* phi)
     BH_CUDA(cudaSetDevice(ctx->device));
     cudaStream_t st = ctx->stream;
     const i64 n = ctx->n;
-    if (ctx->group != 32) {
-        snprintf(ctx->cuda_msg, sizeof(ctx->cuda_msg), "BH_OPT_GROUP=1 walk is not built yet");
-        return BH_ERR_INVALID_ARG;
-    }
-    const i64 ngroups = (n + 31) / 32;
+    const int group = ctx->group;
+    const i64 ngroups = (n + group - 1) / group;
     BH_CUDA(ctx->gcount.ensure(sizeof(uint4) * ngroups));
     ctx->launches_walk = 0;
     BH_CUDA(cudaEventRecord(ctx->ev[EV_W0], st));
@@ -395,19 +392,25 @@ int bh_potential(bh_ctx* ctx, double theta, double G, double* phi)
         P.inv_theta = (float)(1.0 / theta);
         P.mac = ctx->mac;
         P.negG = -G;
-        i64 cap = (i64)kStackPerLevel * (ctx->maxlevel + 2) + 32;
-        cap = (cap + 1) & ~1LL;
-        const size_t smem = walk_smem_per_warp((int)cap) * kWalkWarps;
-        if (smem > 227 * 1024) return BH_ERR_TOO_LARGE;
-        P.stack_cap = (int)cap;
-        walk_group32_kernel<<<blocks_for(ngroups, kWalkWarps), kWalkWarps * 32, smem, st>>>(P);
+        P.stack_cap = 0;
+        if (group == 32) {
+            i64 cap = (i64)kStackPerLevel * (ctx->maxlevel + 2) + 32;
+            cap = (cap + 1) & ~1LL;
+            const size_t smem = walk_smem_per_warp((int)cap) * kWalkWarps;
+            if (smem > 227 * 1024) return BH_ERR_TOO_LARGE;
+            P.stack_cap = (int)cap;
+            const i64 npairs = (ngroups + 1) / 2;
+            walk_pair_kernel<<<blocks_for(npairs, kWalkWarps), kWalkWarps * 32, smem, st>>>(P);
+        } else {
+            walk_single_kernel<<<blocks_for(n, 128), 128, 0, st>>>(P);
+        }
         BH_CUDA(cudaGetLastError());
         ctx->launches_walk = 1;
     }
     BH_CUDA(cudaEventRecord(ctx->ev[EV_W1], st));
     ctx->ev_walk = true;
     ctx->walked = true;
-    ctx->walk_group = 32;
+    ctx->walk_group = group;
     return BH_OK;
 }
 

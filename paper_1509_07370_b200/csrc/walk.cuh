@@ -1,34 +1,46 @@
 // walk.cuh -- steps a6 + a7: the group tree walk (§3.3) and the scatter of Phi.
 //
-// What is kept from the paper's kernel: one warp owns 32 neighbouring (Morton-consecutive) target
-// cells; the traversal stack lives in shared memory and is shared by the warp; a node is used only
-// if EVERY lane accepts it (the all() vote), otherwise the whole warp opens it;
-// potentials are accumulated in registers.
+// What is kept from the paper's kernel: 32 neighbouring (Morton-consecutive) target cells form a
+// group that shares one traversal; the traversal stack lives in shared memory; a node is used only
+// if EVERY member of the group accepts it (the all() vote), otherwise the whole
+// group opens it; potentials are accumulated in registers.
 // What differs (the paper's design is for a Fermi C2075, where lane 0 alone walks the tree):
-//  * The traversal is lane-parallel: each step pops up to 4 opened nodes and tests their <= 32
-//    children at once, one child per lane.  The vote of DESIGN.md W2 ("all members pass
-//    d^2 > r_c^2") is decided without touching the members whenever the group's bounding box
-//    proves it: fp32 rounding is monotone, so the fp32 d^2 evaluated at the box's nearest (farthest)
-//    point bounds every member's fp32 d^2 from below (above).  Only nodes between the two bounds
-//    take the per-member test + __all_sync vote.
-//  * Accepted nodes and leaf cells are appended to two interaction lists in shared memory, stored
-//    as pairs (x0,x1,y0,y1 | z0,z1,m0,m1), and evaluated with lane = target using packed
-//    fp32x2 arithmetic (FADD2/FMUL2/FFMA2, sm_100) and one MUFU.RSQ per interaction.
+//  * One warp walks TWO adjacent groups A = 2w, B = 2w+1 at once (lane = one target of A and one of
+//    B).  The two groups keep their own votes -- every decision below is taken per group, so the
+//    result is the one of DESIGN.md W1-W4 -- but they share the traversal: a stack entry carries
+//    the set of groups that still need the subtree, and a node both groups accept (about 3/4 of
+//    all list entries on the grid workloads) is fetched from shared memory once and evaluated for
+//    both targets with packed fp32x2 arithmetic (FADD2/FFMA2, sm_100; one MUFU.RSQ per interaction).
+//  * The traversal is lane-parallel: each step pops up to 4 stack entries and tests their <= 32
+//    children at once, one child per lane.  The vote ("all members have d^2 > r_c^2") is decided
+//    without touching the members whenever the group's bounding box proves it: fp32 rounding is
+//    monotone, so the fp32 d^2 evaluated at the box's nearest (farthest) point bounds every
+//    member's fp32 d^2 from below (above).  Only nodes between the two bounds take the per-member
+//    test + __all_sync vote.
+//  * Accepted nodes and leaf cells go to interaction lists in shared memory: U2 (both groups,
+//    float4 records, packed across the two targets), UA / UB (one group only, SoA, packed across
+//    two entries), and C (leaf cells inside a group's bounding box -- the only ones that can be a
+//    target's own cell or coincide with it -- evaluated with the zero-distance mask of W3).
 //  * Partial sums are fp32 over one list flush (<= 128 entries, 4 accumulators) and are flushed
 //    into an fp64 sum per target, which keeps the summation error near 1e-7 relative.
 //  * Phi is written straight to the original cell order (step a7 is fused: no extra pass).
 // ALU-bound: 13 flops per interaction by the north-star convention; MUFU (16 rsqrt/clk/SM) is the
 // co-limiter.
+// BH_OPT_GROUP = 1 (W5, the textbook per-target walk) is walk_single_kernel below.
 #pragma once
 #include "common.cuh"
 #include "tree.cuh"
 
 namespace bh {
 
-constexpr int kWalkWarps = 8;                 // warps (= groups) per CTA
-constexpr int kListCap = 128;                 // entries per interaction list (per warp)
-constexpr int kListFlushAt = kListCap - 32;   // a traversal step appends <= 32 entries
+constexpr int kWalkWarps = 8;                 // warps (= group pairs) per CTA
+constexpr int kU2Cap = 128;                   // entries of the both-groups list (float4 each)
+constexpr int kU1Cap = 64;                    // entries of each one-group list (SoA x,y,z,m)
+constexpr int kCCap = 64;                     // entries of the checked list (float4 + group mask)
+constexpr int kStepMax = 32;                  // a traversal step appends <= 32 entries to any list
 constexpr int kStackPerLevel = 36;            // stack entries a level can leave behind (<= 3 + 32)
+constexpr u32 kCountMask = 0x3fffffffu;       // stack entry .y = child count | group set << 30
+constexpr float kTinyD2 = 1.0e-36f;           // keeps d^2 of the unchecked lists off zero
 
 struct WalkParams {
     const float4* rec;        // [n_slots] (x, y, z, m) of every node / leaf-cell slot
@@ -47,7 +59,8 @@ struct WalkParams {
 
 __host__ __device__ inline size_t walk_smem_per_warp(int stack_cap)
 {
-    return (size_t)stack_cap * sizeof(uint2) + 2 * (size_t)kListCap * 16;
+    return (size_t)kU2Cap * 16 + 2 * (size_t)kU1Cap * 16 + (size_t)kCCap * 16 + (size_t)kCCap * 4 +
+           (size_t)stack_cap * sizeof(uint2);
 }
 
 __device__ __forceinline__ float rsqrt_approx(float v)
@@ -57,58 +70,113 @@ __device__ __forceinline__ float rsqrt_approx(float v)
     return r;
 }
 
-// Evaluates `cnt` list entries for this lane's target.  List layout per PAIR p (8 floats):
-// x[2p], x[2p+1], y[2p], y[2p+1], z[2p], z[2p+1], m[2p], m[2p+1].  The list is padded to a multiple
-// of 4 entries with zero-mass far-away dummies by the caller.  CHECKED: skip pairs at zero distance
-// (the target's own cell and coincident cells, W3).
-template <bool CHECKED>
-__device__ __forceinline__ double eval_list(const float* __restrict__ list, int cnt, float2 npx, float2 npy,
-                                            float2 npz)
+__device__ __forceinline__ float2 splat2(float v) { return make_float2(v, v); }
+
+// ---- U2: entries both groups take; packed across the lane's two targets -------------------------
+// np* = (-p_A, -p_B).  The list is padded to a multiple of 4 entries by the caller.
+__device__ __forceinline__ void u2_body(const float4 v, const float2 npx, const float2 npy, const float2 npz,
+                                        float2& s)
 {
-    float2 s0 = make_float2(0.f, 0.f), s1 = make_float2(0.f, 0.f);
-    const int nquads = (cnt + 3) >> 2;
-    const float4* L4 = reinterpret_cast<const float4*>(list);
+    const float2 dx = __fadd2_rn(splat2(v.x), npx);
+    const float2 dy = __fadd2_rn(splat2(v.y), npy);
+    const float2 dz = __fadd2_rn(splat2(v.z), npz);
+    float2 d2 = __ffma2_rn(dx, dx, splat2(kTinyD2));
+    d2 = __ffma2_rn(dy, dy, d2);
+    d2 = __ffma2_rn(dz, dz, d2);
+    const float2 r = make_float2(rsqrt_approx(d2.x), rsqrt_approx(d2.y));
+    s = __ffma2_rn(splat2(v.w), r, s);
+}
+
+__device__ __forceinline__ void eval_u2(const float4* __restrict__ L, int cnt, const float2 npx, const float2 npy,
+                                        const float2 npz, double& accA, double& accB)
+{
+    float2 s0 = splat2(0.f), s1 = splat2(0.f), s2 = splat2(0.f), s3 = splat2(0.f);
+    const int nq = (cnt + 3) >> 2;
     #pragma unroll 2
-    for (int q = 0; q < nquads; ++q) {
-        const float4 a0 = L4[4 * q + 0], b0 = L4[4 * q + 1];
-        const float4 a1 = L4[4 * q + 2], b1 = L4[4 * q + 3];
-        float2 dx0 = __fadd2_rn(make_float2(a0.x, a0.y), npx);
-        float2 dy0 = __fadd2_rn(make_float2(a0.z, a0.w), npy);
-        float2 dz0 = __fadd2_rn(make_float2(b0.x, b0.y), npz);
-        float2 dx1 = __fadd2_rn(make_float2(a1.x, a1.y), npx);
-        float2 dy1 = __fadd2_rn(make_float2(a1.z, a1.w), npy);
-        float2 dz1 = __fadd2_rn(make_float2(b1.x, b1.y), npz);
-        float2 d0 = __fmul2_rn(dx0, dx0);
-        float2 d1 = __fmul2_rn(dx1, dx1);
+    for (int q = 0; q < nq; ++q) {
+        const float4 v0 = L[4 * q + 0], v1 = L[4 * q + 1], v2 = L[4 * q + 2], v3 = L[4 * q + 3];
+        u2_body(v0, npx, npy, npz, s0);
+        u2_body(v1, npx, npy, npz, s1);
+        u2_body(v2, npx, npy, npz, s2);
+        u2_body(v3, npx, npy, npz, s3);
+    }
+    accA += ((double)s0.x + (double)s1.x) + ((double)s2.x + (double)s3.x);
+    accB += ((double)s0.y + (double)s1.y) + ((double)s2.y + (double)s3.y);
+}
+
+// ---- UA / UB: entries one group takes; SoA lists, packed across two entries --------------------
+// np = (-p, -p, -p) of the one target.  Padded to a multiple of 4 entries by the caller.
+__device__ __forceinline__ double eval_u1(const float* __restrict__ L, int cnt, const float npx, const float npy,
+                                          const float npz)
+{
+    const float4* X = reinterpret_cast<const float4*>(L);
+    const float4* Y = reinterpret_cast<const float4*>(L + kU1Cap);
+    const float4* Z = reinterpret_cast<const float4*>(L + 2 * kU1Cap);
+    const float4* M = reinterpret_cast<const float4*>(L + 3 * kU1Cap);
+    float2 s0 = splat2(0.f), s1 = splat2(0.f);
+    const int nq = (cnt + 3) >> 2;
+    #pragma unroll 2
+    for (int q = 0; q < nq; ++q) {
+        const float4 x = X[q], y = Y[q], z = Z[q], m = M[q];
+        const float2 dx0 = __fadd2_rn(make_float2(x.x, x.y), splat2(npx));
+        const float2 dx1 = __fadd2_rn(make_float2(x.z, x.w), splat2(npx));
+        const float2 dy0 = __fadd2_rn(make_float2(y.x, y.y), splat2(npy));
+        const float2 dy1 = __fadd2_rn(make_float2(y.z, y.w), splat2(npy));
+        const float2 dz0 = __fadd2_rn(make_float2(z.x, z.y), splat2(npz));
+        const float2 dz1 = __fadd2_rn(make_float2(z.z, z.w), splat2(npz));
+        float2 d0 = __ffma2_rn(dx0, dx0, splat2(kTinyD2));
+        float2 d1 = __ffma2_rn(dx1, dx1, splat2(kTinyD2));
         d0 = __ffma2_rn(dy0, dy0, d0);
         d1 = __ffma2_rn(dy1, dy1, d1);
         d0 = __ffma2_rn(dz0, dz0, d0);
         d1 = __ffma2_rn(dz1, dz1, d1);
-        float2 r0 = make_float2(rsqrt_approx(d0.x), rsqrt_approx(d0.y));
-        float2 r1 = make_float2(rsqrt_approx(d1.x), rsqrt_approx(d1.y));
-        if (CHECKED) {
-            r0.x = d0.x >= 1.17549435e-38f ? r0.x : 0.f;
-            r0.y = d0.y >= 1.17549435e-38f ? r0.y : 0.f;
-            r1.x = d1.x >= 1.17549435e-38f ? r1.x : 0.f;
-            r1.y = d1.y >= 1.17549435e-38f ? r1.y : 0.f;
-        }
-        s0 = __ffma2_rn(make_float2(b0.z, b0.w), r0, s0);
-        s1 = __ffma2_rn(make_float2(b1.z, b1.w), r1, s1);
+        const float2 r0 = make_float2(rsqrt_approx(d0.x), rsqrt_approx(d0.y));
+        const float2 r1 = make_float2(rsqrt_approx(d1.x), rsqrt_approx(d1.y));
+        s0 = __ffma2_rn(make_float2(m.x, m.y), r0, s0);
+        s1 = __ffma2_rn(make_float2(m.z, m.w), r1, s1);
     }
     return ((double)s0.x + (double)s0.y) + ((double)s1.x + (double)s1.y);
 }
 
-__device__ __forceinline__ void list_store(float* list, int e, float4 r)
+// ---- C: leaf cells inside a group's bounding box; zero-distance pairs are skipped (W3) ----------
+__device__ __forceinline__ void eval_c(const float4* __restrict__ L, const u32* __restrict__ Lm, int cnt,
+                                       const float2 npx, const float2 npy, const float2 npz, double& accA,
+                                       double& accB)
 {
-    float* p = list + (e >> 1) * 8 + (e & 1);
-    p[0] = r.x; p[2] = r.y; p[4] = r.z; p[6] = r.w;
+    float2 s = splat2(0.f);
+    for (int e = 0; e < cnt; ++e) {
+        const float4 v = L[e];
+        const u32 mk = Lm[e];
+        const float2 dx = __fadd2_rn(splat2(v.x), npx);
+        const float2 dy = __fadd2_rn(splat2(v.y), npy);
+        const float2 dz = __fadd2_rn(splat2(v.z), npz);
+        float2 d2 = __fmul2_rn(dx, dx);
+        d2 = __ffma2_rn(dy, dy, d2);
+        d2 = __ffma2_rn(dz, dz, d2);
+        float2 r = make_float2(rsqrt_approx(d2.x), rsqrt_approx(d2.y));
+        r.x = (d2.x >= 1.17549435e-38f && (mk & 1u)) ? r.x : 0.f;
+        r.y = (d2.y >= 1.17549435e-38f && (mk & 2u)) ? r.y : 0.f;
+        s = __ffma2_rn(splat2(v.w), r, s);
+    }
+    accA += (double)s.x;
+    accB += (double)s.y;
 }
 
-// pads [cnt, roundup4(cnt)) with zero-mass entries far away (finite d^2, no NaN)
-__device__ __forceinline__ void list_pad(float* list, int cnt)
+__device__ __forceinline__ void u1_store(float* L, int e, float4 r)
+{
+    L[e] = r.x; L[kU1Cap + e] = r.y; L[2 * kU1Cap + e] = r.z; L[3 * kU1Cap + e] = r.w;
+}
+
+// zero-mass entries far away (finite d^2, no NaN) up to the next multiple of 4
+__device__ __forceinline__ void u2_pad(float4* L, int cnt)
 {
     const int e = cnt + (int)lane_id();
-    if (e < ((cnt + 3) & ~3)) list_store(list, e, make_float4(3.0e18f, 3.0e18f, 3.0e18f, 0.f));
+    if (e < ((cnt + 3) & ~3)) L[e] = make_float4(3.0e18f, 3.0e18f, 3.0e18f, 0.f);
+}
+__device__ __forceinline__ void u1_pad(float* L, int cnt)
+{
+    const int e = cnt + (int)lane_id();
+    if (e < ((cnt + 3) & ~3)) u1_store(L, e, make_float4(3.0e18f, 3.0e18f, 3.0e18f, 0.f));
 }
 
 __device__ __forceinline__ float warp_min(float v)
@@ -124,66 +192,95 @@ __device__ __forceinline__ float warp_max(float v)
     return v;
 }
 
-__global__ void __launch_bounds__(kWalkWarps * 32)
-walk_group32_kernel(const WalkParams P)
+// fp32 d^2 at the nearest / farthest point of the box [lo, hi] from q, with the rounding sequence
+// of W8 (monotone in every |component|, so they bound every member's fp32 d^2).
+__device__ __forceinline__ void box_d2(const float qx, const float qy, const float qz, const float xl, const float xh,
+                                       const float yl, const float yh, const float zl, const float zh,
+                                       float& d2min, float& d2max)
+{
+    const float ax = __fsub_rn(xl, qx), bx = __fsub_rn(xh, qx);
+    const float ay = __fsub_rn(yl, qy), by = __fsub_rn(yh, qy);
+    const float az = __fsub_rn(zl, qz), bz = __fsub_rn(zh, qz);
+    const float nx = fmaxf(0.f, fmaxf(ax, -bx)), fx = fmaxf(-ax, bx);
+    const float ny = fmaxf(0.f, fmaxf(ay, -by)), fy = fmaxf(-ay, by);
+    const float nz = fmaxf(0.f, fmaxf(az, -bz)), fz = fmaxf(-az, bz);
+    d2min = __fmaf_rn(nz, nz, __fmaf_rn(ny, ny, __fmul_rn(nx, nx)));
+    d2max = __fmaf_rn(fz, fz, __fmaf_rn(fy, fy, __fmul_rn(fx, fx)));
+}
+
+__global__ void __launch_bounds__(kWalkWarps * 32, 3)
+walk_pair_kernel(const WalkParams P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5;
     const u32 lane = lane_id();
-    const i64 g = (i64)blockIdx.x * kWalkWarps + warp;
-    if (g >= P.ngroups) return;                       // whole warp leaves; no block-level sync below
+    const i64 pr = (i64)blockIdx.x * kWalkWarps + warp;       // pair of groups (2 pr, 2 pr + 1)
+    const i64 gA = 2 * pr, gB = gA + 1;
+    if (gA >= P.ngroups) return;                      // whole warp leaves; no block-level sync below
 
     unsigned char* my = smem_raw + (size_t)warp * walk_smem_per_warp(P.stack_cap);
-    float* nlist = reinterpret_cast<float*>(my);                       // accepted internal nodes
-    float* llist = nlist + kListCap * 4;                               // leaf cells
-    uint2* stack = reinterpret_cast<uint2*>(llist + kListCap * 4);     // (first child slot, count)
+    float4* U2 = reinterpret_cast<float4*>(my);                         // both groups
+    float* UA = reinterpret_cast<float*>(U2 + kU2Cap);                  // group A only (SoA)
+    float* UB = UA + 4 * kU1Cap;                                        // group B only (SoA)
+    float4* C = reinterpret_cast<float4*>(UB + 4 * kU1Cap);             // checked leaf cells
+    u32* Cm = reinterpret_cast<u32*>(C + kCCap);                        //   and the groups they serve
+    uint2* stack = reinterpret_cast<uint2*>(Cm + kCCap);                // (first child slot, count | groups << 30)
 
-    // ---- the 32 targets of this group (W-rule 1): sorted slots [32g, 32g+32) ----
-    const i64 s = g * 32 + lane;
-    const int nt = (int)min((i64)32, P.n - g * 32);
-    const bool live = (int)lane < nt;
-    const float4 tp = __ldg(P.leafrec + (live ? s : g * 32));
-    const float px = tp.x, py = tp.y, pz = tp.z;
-    // bounding box of the live targets
-    const float bxl = warp_min(px), bxh = warp_max(px);
-    const float byl = warp_min(py), byh = warp_max(py);
-    const float bzl = warp_min(pz), bzh = warp_max(pz);
-    const float2 npx = make_float2(-px, -px), npy = make_float2(-py, -py), npz = make_float2(-pz, -pz);
+    // ---- the targets (W-rule 1): group g = sorted slots [32g, 32g+32) ----
+    const bool hasB = gB < P.ngroups;
+    const int ntA = (int)min((i64)32, P.n - gA * 32);
+    const int ntB = hasB ? (int)min((i64)32, P.n - gB * 32) : 0;
+    const bool liveA = (int)lane < ntA, liveB = (int)lane < ntB;
+    const i64 sA = gA * 32 + lane, sB = gB * 32 + lane;
+    const float4 tA = __ldg(P.leafrec + (liveA ? sA : gA * 32));
+    const float4 tB = __ldg(P.leafrec + (liveB ? sB : (hasB ? gB * 32 : gA * 32)));
+    // bounding boxes of the live targets of each group
+    const float axl = warp_min(tA.x), axh = warp_max(tA.x);
+    const float ayl = warp_min(tA.y), ayh = warp_max(tA.y);
+    const float azl = warp_min(tA.z), azh = warp_max(tA.z);
+    const float bxl = warp_min(tB.x), bxh = warp_max(tB.x);
+    const float byl = warp_min(tB.y), byh = warp_max(tB.y);
+    const float bzl = warp_min(tB.z), bzh = warp_max(tB.z);
+    const float2 npx = make_float2(-tA.x, -tB.x), npy = make_float2(-tA.y, -tB.y), npz = make_float2(-tA.z, -tB.z);
 
-    double acc = 0.0;
-    int n_node = 0, n_leaf = 0;                 // list fill (warp-uniform)
-    u32 c_acc = 0, c_leaf = 0, c_open = 0, c_exact = 0;
+    double accA = 0.0, accB = 0.0;
+    int nU2 = 0, nUA = 0, nUB = 0, nC = 0;          // list fill (warp-uniform)
+    u32 cAccA = 0, cLeafA = 0, cOpenA = 0, cExA = 0;  // per-lane partial counters, reduced at the end
+    u32 cAccB = 0, cLeafB = 0, cOpenB = 0, cExB = 0;
     int sp = 0;
     if (P.n >= 2) {                             // root is tested like any other node (W-rule 2)
-        if (lane == 0) stack[0] = make_uint2(0u, 1u);
+        if (lane == 0) stack[0] = make_uint2(0u, 1u | ((hasB ? 3u : 1u) << 30));
         sp = 1;
     }
     __syncwarp();
 
     const u32 lt = lanemask_lt();
     const int sub = lane >> 3, j = lane & 7;
+    const float inv_theta = P.inv_theta;
+    const bool mac94 = P.mac == 1;
     while (sp > 0) {
-        // ---- pop up to 4 opened nodes; lane (sub, j) takes child j of entry sub ----
+        // ---- pop up to 4 entries; lane (sub, j) takes child j of entry sub ----
         int npop = sp < 4 ? sp : 4;
         uint2 e = make_uint2(0u, 0u);
         if (sub < npop) e = stack[sp - 1 - sub];
         u32 jj = (u32)j;
-        if (__any_sync(0xffffffffu, e.y > 8u)) {
+        if (__any_sync(0xffffffffu, (e.y & kCountMask) > 8u)) {
             // rare: a bucket of > 8 coincident cells is near the top; serve the top entry alone,
             // 32 children per step, shrinking it in place while more than 32 remain
             e = stack[sp - 1];
             jj = lane;
             npop = 1;
             __syncwarp();
-            if (e.y > 32u) {
+            if ((e.y & kCountMask) > 32u) {
                 if (lane == 0) stack[sp - 1] = make_uint2(e.x + 32u, e.y - 32u);
-                e.y = 32u;
+                e.y = (e.y & ~kCountMask) | 32u;
                 npop = 0;
             }
         }
         sp -= npop;
         __syncwarp();
-        const bool have = jj < e.y;
+        const u32 msk = e.y >> 30;
+        const bool have = jj < (e.y & kCountMask);
         const u32 slot = e.x + jj;
         float4 r = make_float4(0.f, 0.f, 0.f, 0.f);
         WalkAux a; a.size = 0.f; a.delta = 0.f; a.first = 0u; a.count = 0u;
@@ -193,27 +290,22 @@ walk_group32_kernel(const WalkParams P)
             a.size = __uint_as_float(t.x); a.delta = __uint_as_float(t.y); a.first = t.z; a.count = t.w;
         }
         const bool internal = have && a.count > 0u;
-        const bool is_leaf = have && a.count == 0u;
+        const bool leaf = have && a.count == 0u;
+        const bool wA = (msk & 1u) != 0u, wB = (msk & 2u) != 0u;
         // ---- opening test (W-rule 2, fp32 decision W8): r_c = l*(1/theta) [+ delta] ----
-        float rc = __fmul_rn(a.size, P.inv_theta);
-        if (P.mac == 1) rc = __fadd_rn(rc, a.delta);
+        float rc = __fmul_rn(a.size, inv_theta);
+        if (mac94) rc = __fadd_rn(rc, a.delta);
         const float rc2 = __fmul_rn(rc, rc);
-        bool accept = false, amb = false;
-        if (internal) {
-            const float ax = __fsub_rn(bxl, r.x), bx = __fsub_rn(bxh, r.x);
-            const float ay = __fsub_rn(byl, r.y), by = __fsub_rn(byh, r.y);
-            const float az = __fsub_rn(bzl, r.z), bz = __fsub_rn(bzh, r.z);
-            const float nx = fmaxf(0.f, fmaxf(ax, -bx)), fx = fmaxf(-ax, bx);
-            const float ny = fmaxf(0.f, fmaxf(ay, -by)), fy = fmaxf(-ay, by);
-            const float nz = fmaxf(0.f, fmaxf(az, -bz)), fz = fmaxf(-az, bz);
-            const float d2min = __fmaf_rn(nz, nz, __fmaf_rn(ny, ny, __fmul_rn(nx, nx)));
-            const float d2max = __fmaf_rn(fz, fz, __fmaf_rn(fy, fy, __fmul_rn(fx, fx)));
-            accept = d2min > rc2;                    // every member passes
-            amb = !accept && (d2max > rc2);          // some member might pass, some might not
-        }
-        // ---- nodes the box cannot decide: per-member test + vote ----
-        u32 am = __ballot_sync(0xffffffffu, amb);
-        c_exact += __popc(am);
+        float d2minA, d2maxA, d2minB, d2maxB;
+        box_d2(r.x, r.y, r.z, axl, axh, ayl, ayh, azl, azh, d2minA, d2maxA);
+        box_d2(r.x, r.y, r.z, bxl, bxh, byl, byh, bzl, bzh, d2minB, d2maxB);
+        bool accA_ = internal && wA && d2minA > rc2;                  // every member of A passes
+        bool accB_ = internal && wB && d2minB > rc2;
+        const bool ambA = internal && wA && !accA_ && d2maxA > rc2;   // some member might pass, some not
+        const bool ambB = internal && wB && !accB_ && d2maxB > rc2;
+        cExA += ambA; cExB += ambB;
+        // ---- nodes a box cannot decide: per-member test + vote ----
+        u32 am = __ballot_sync(0xffffffffu, ambA || ambB);
         while (am) {
             const int src = __ffs(am) - 1;
             am &= am - 1;
@@ -221,56 +313,147 @@ walk_group32_kernel(const WalkParams P)
             const float qy = __shfl_sync(0xffffffffu, r.y, src);
             const float qz = __shfl_sync(0xffffffffu, r.z, src);
             const float q2 = __shfl_sync(0xffffffffu, rc2, src);
-            const float dx = __fsub_rn(px, qx), dy = __fsub_rn(py, qy), dz = __fsub_rn(pz, qz);
-            const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-            const bool ok = __all_sync(0xffffffffu, !live || d2 > q2);
-            if ((int)lane == src) accept = ok;
+            const float2 dx = __fadd2_rn(splat2(qx), npx), dy = __fadd2_rn(splat2(qy), npy),
+                         dz = __fadd2_rn(splat2(qz), npz);
+            const float2 d2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
+            const bool okA = __all_sync(0xffffffffu, !liveA || d2.x > q2);
+            const bool okB = __all_sync(0xffffffffu, !liveB || d2.y > q2);
+            if ((int)lane == src) {
+                if (ambA) accA_ = okA;
+                if (ambB) accB_ = okB;
+            }
         }
-        const bool open = internal && !accept;
-        // ---- append accepted nodes and leaf cells to the lists; push opened nodes ----
-        const u32 m_acc = __ballot_sync(0xffffffffu, internal && accept);
-        const u32 m_leaf = __ballot_sync(0xffffffffu, is_leaf);
-        const u32 m_open = __ballot_sync(0xffffffffu, open);
-        if (internal && accept) list_store(nlist, n_node + __popc(m_acc & lt), r);
-        if (is_leaf) list_store(llist, n_leaf + __popc(m_leaf & lt), r);
-        const bool bucket = open && !(a.size < __int_as_float(0x7f800000));
-        if (open) stack[sp + __popc(m_open & lt)] = make_uint2(a.first, a.count);
-        sp += __popc(m_open);
-        n_node += __popc(m_acc);
-        n_leaf += __popc(m_leaf);
-        c_acc += __popc(m_acc);
-        c_leaf += __popc(m_leaf);
-        c_open += __popc(m_open) - __popc(__ballot_sync(0xffffffffu, bucket));
+        const bool opA = internal && wA && !accA_, opB = internal && wB && !accB_;
+        const u32 om = (opA ? 1u : 0u) | (opB ? 2u : 0u);               // groups that open the node
+        // leaf cells inside a group's box may be a target's own cell or coincide with one
+        const bool danger = leaf && ((wA && !(d2minA > 0.f)) || (wB && !(d2minB > 0.f)));
+        const u32 um = internal ? ((accA_ ? 1u : 0u) | (accB_ ? 2u : 0u)) : ((leaf && !danger) ? msk : 0u);
+        const bool toU2 = um == 3u, toUA = um == 1u, toUB = um == 2u;
+        // ---- append to the lists; push opened nodes ----
+        const u32 bU2 = __ballot_sync(0xffffffffu, toU2);
+        const u32 bUA = __ballot_sync(0xffffffffu, toUA);
+        const u32 bUB = __ballot_sync(0xffffffffu, toUB);
+        const u32 bC = __ballot_sync(0xffffffffu, danger);
+        const u32 bOp = __ballot_sync(0xffffffffu, om != 0u);
+        if (toU2) U2[nU2 + __popc(bU2 & lt)] = r;
+        if (toUA) u1_store(UA, nUA + __popc(bUA & lt), r);
+        if (toUB) u1_store(UB, nUB + __popc(bUB & lt), r);
+        if (danger) { const int k = nC + __popc(bC & lt); C[k] = r; Cm[k] = msk; }
+        if (om) stack[sp + __popc(bOp & lt)] = make_uint2(a.first, a.count | (om << 30));
+        sp += __popc(bOp);
+        nU2 += __popc(bU2); nUA += __popc(bUA); nUB += __popc(bUB); nC += __popc(bC);
+        const bool bucket = internal && !(a.size < __int_as_float(0x7f800000));
+        cAccA += accA_; cAccB += accB_;
+        cLeafA += leaf && wA; cLeafB += leaf && wB;
+        cOpenA += opA && !bucket; cOpenB += opB && !bucket;
         __syncwarp();
         // ---- evaluate a list before the next step could overflow it ----
-        if (n_node > kListFlushAt) {
-            list_pad(nlist, n_node);
+        if (nU2 > kU2Cap - kStepMax) {
+            u2_pad(U2, nU2);
             __syncwarp();
-            acc += eval_list<false>(nlist, n_node, npx, npy, npz);
-            n_node = 0;
-            __syncwarp();
-        }
-        if (n_leaf > kListFlushAt) {
-            list_pad(llist, n_leaf);
-            __syncwarp();
-            acc += eval_list<true>(llist, n_leaf, npx, npy, npz);
-            n_leaf = 0;
+            eval_u2(U2, nU2, npx, npy, npz, accA, accB);
+            nU2 = 0;
             __syncwarp();
         }
+        if (nUA > kU1Cap - kStepMax) {
+            u1_pad(UA, nUA);
+            __syncwarp();
+            accA += eval_u1(UA, nUA, npx.x, npy.x, npz.x);
+            nUA = 0;
+            __syncwarp();
+        }
+        if (nUB > kU1Cap - kStepMax) {
+            u1_pad(UB, nUB);
+            __syncwarp();
+            accB += eval_u1(UB, nUB, npx.y, npy.y, npz.y);
+            nUB = 0;
+            __syncwarp();
+        }
+        if (nC > kCCap - kStepMax) {
+            eval_c(C, Cm, nC, npx, npy, npz, accA, accB);
+            nC = 0;
+            __syncwarp();
+        }
     }
-    if (n_node > 0) {
-        list_pad(nlist, n_node);
+    if (nU2 > 0) {
+        u2_pad(U2, nU2);
         __syncwarp();
-        acc += eval_list<false>(nlist, n_node, npx, npy, npz);
+        eval_u2(U2, nU2, npx, npy, npz, accA, accB);
     }
-    if (n_leaf > 0) {
-        list_pad(llist, n_leaf);
+    if (nUA > 0) {
+        u1_pad(UA, nUA);
         __syncwarp();
-        acc += eval_list<true>(llist, n_leaf, npx, npy, npz);
+        accA += eval_u1(UA, nUA, npx.x, npy.x, npz.x);
     }
+    if (nUB > 0) {
+        u1_pad(UB, nUB);
+        __syncwarp();
+        accB += eval_u1(UB, nUB, npx.y, npy.y, npz.y);
+    }
+    if (nC > 0) eval_c(C, Cm, nC, npx, npy, npz, accA, accB);
     // ---- a7: Phi_t = -G * sum, written in the original cell order (W-rule 4) ----
-    if (live) P.phi[__ldg(P.idx + s)] = P.negG * acc;
-    if (lane == 0) P.gcount[g] = make_uint4(c_acc, c_leaf, c_open, c_exact);
+    if (liveA) P.phi[__ldg(P.idx + sA)] = P.negG * accA;
+    if (liveB) P.phi[__ldg(P.idx + sB)] = P.negG * accB;
+    cAccA = __reduce_add_sync(0xffffffffu, cAccA); cLeafA = __reduce_add_sync(0xffffffffu, cLeafA);
+    cOpenA = __reduce_add_sync(0xffffffffu, cOpenA); cExA = __reduce_add_sync(0xffffffffu, cExA);
+    cAccB = __reduce_add_sync(0xffffffffu, cAccB); cLeafB = __reduce_add_sync(0xffffffffu, cLeafB);
+    cOpenB = __reduce_add_sync(0xffffffffu, cOpenB); cExB = __reduce_add_sync(0xffffffffu, cExB);
+    if (lane == 0) {
+        P.gcount[gA] = make_uint4(cAccA, cLeafA, cOpenA, cExA);
+        if (hasB) P.gcount[gB] = make_uint4(cAccB, cLeafB, cOpenB, cExB);
+    }
+}
+
+// ---- BH_OPT_GROUP = 1 (W5): every target walks alone --------------------------------------------
+// The textbook per-particle Barnes-Hut: one thread per target, depth-first with a private stack of
+// sibling runs (one entry per level), the same fp32 decision (W8) and the same zero-distance rule
+// (W3).  A check / comparison mode, not tuned: threads of a warp diverge.
+constexpr int kSingleStack = 3 * (kMaxLevel + 2);
+
+__global__ void __launch_bounds__(128)
+walk_single_kernel(const WalkParams P)
+{
+    const i64 s = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= P.n) return;
+    const float4 tp = __ldg(P.leafrec + s);
+    u32 st_first[kSingleStack], st_count[kSingleStack];
+    int sp = 0;
+    if (P.n >= 2) { st_first[0] = 0u; st_count[0] = 1u; sp = 1; }
+    double acc = 0.0;
+    float part = 0.f;
+    int npart = 0;
+    u32 c_acc = 0, c_leaf = 0, c_open = 0;
+    while (sp > 0) {
+        const u32 slot = st_first[sp - 1];
+        if (--st_count[sp - 1] == 0u) --sp; else ++st_first[sp - 1];
+        const float4 r = __ldg(P.rec + slot);
+        const uint4 t = __ldg(reinterpret_cast<const uint4*>(P.aux + slot));
+        const float size = __uint_as_float(t.x), delta = __uint_as_float(t.y);
+        const u32 first = t.z, count = t.w;
+        const float dx = __fsub_rn(tp.x, r.x), dy = __fsub_rn(tp.y, r.y), dz = __fsub_rn(tp.z, r.z);
+        const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+        bool use;
+        if (count == 0u) {                       // leaf cell: summed unless at zero distance (W3)
+            ++c_leaf;
+            use = d2 >= 1.17549435e-38f;
+        } else {
+            float rc = __fmul_rn(size, P.inv_theta);
+            if (P.mac == 1) rc = __fadd_rn(rc, delta);
+            use = d2 > __fmul_rn(rc, rc);
+            if (use) ++c_acc;
+            else {
+                if (size < __int_as_float(0x7f800000)) ++c_open;
+                st_first[sp] = first; st_count[sp] = count; ++sp;
+            }
+        }
+        if (use) {
+            part = __fmaf_rn(r.w, rsqrt_approx(d2), part);
+            if (++npart == 32) { acc += (double)part; part = 0.f; npart = 0; }
+        }
+    }
+    acc += (double)part;
+    P.phi[__ldg(P.idx + s)] = P.negG * acc;
+    P.gcount[s] = make_uint4(c_acc, c_leaf, c_open, 0u);
 }
 
 // per-target interaction counts / int64 group counts from the uint4 group counters

@@ -124,6 +124,23 @@ def test_phi_vs_oracle(bh, oracle, w, theta, mac):
     assert np.array_equal(inter[perm], np.repeat(ocnt[:, 0] + ocnt[:, 1], 32)[: w.n])
 
 
+@pytest.mark.parametrize("theta", [0.5, 1.0])
+@pytest.mark.parametrize("w", [CASES[1], CASES[3], CASES[4], CASES[6]], ids=lambda w: w.name)
+def test_group1_walk(bh, oracle, w, theta):
+    """BH_OPT_GROUP = 1 (W5): every target walks alone -- the textbook per-particle BH."""
+    ctx = _build(bh, w)
+    ctx.set_group(1)
+    phi = ctx.potential(theta, w.G).cpu().numpy()
+    cnt = ctx.last_group_counts(group=1).cpu().numpy()
+    ot = oracle.OracleTree(w.x, w.y, w.z, w.m, w.cube)
+    ref, ocnt = ot.potential(theta, w.G, group=1, mac_fp32=True, want_counts=True)
+    assert np.array_equal(cnt, ocnt)
+    _phi_check(phi, ref)
+    ctx.set_group(32)                                   # and back: the pair walk on the same tree
+    ref32 = ot.potential(theta, w.G, group=32, mac_fp32=True)
+    _phi_check(ctx.potential(theta, w.G).cpu().numpy(), ref32)
+
+
 @pytest.mark.parametrize("w", [CASES[1], CASES[4]], ids=lambda w: w.name)
 def test_theta_zero_is_direct_sum(bh, oracle, w):
     ctx = _build(bh, w)
