@@ -57,6 +57,9 @@ struct bh_ctx {
     bool built = false;
     bool walked = false;
     int walk_group = 32;
+    bool counts_valid = false;            // gcount holds the counters of the last walk
+    double walk_theta = 0.0;              // arguments of the last bh_potential (the count pass repeats its walk)
+    int walk_mac = BH_MAC_BH86;
     char cuda_msg[256] = {0};
 
     // problem
@@ -164,8 +167,10 @@ int bh_create(bh_ctx** out, int device, void* cuda_stream)
         if ((e = cudaMallocHost(&ctx->h_scalars, sizeof(DeviceScalars))) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaMallocHost"); break; }
         if ((e = cudaFuncSetAttribute(radix_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       (int)sizeof(SortSmem))) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(sort)"); break; }
-        if ((e = cudaFuncSetAttribute(walk_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        if ((e = cudaFuncSetAttribute(walk_pair_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       227 * 1024)) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(walk)"); break; }
+        if ((e = cudaFuncSetAttribute(walk_pair_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      227 * 1024)) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(walk count)"); break; }
     } while (0);
     if (rc != BH_OK) { bh_destroy(ctx); return rc; }
     *out = ctx;
@@ -364,53 +369,88 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
     return BH_OK;
 }
 
+}  // extern "C" (reopened below)
+
+namespace {
+
+// Launches the walk of the last build on the context's stream.  count_only: the traversal of
+// walk_pair_kernel<true> (same decisions, no arithmetic on masses), filling ctx->gcount.
+int launch_walk(bh_ctx* ctx, double theta, double G, double* phi, int group, int mac, bool count_only)
+{
+    cudaStream_t st = ctx->stream;
+    const i64 n = ctx->n;
+    const i64 ngroups = (n + group - 1) / group;
+    BH_CUDA(ctx->gcount.ensure(sizeof(uint4) * ngroups));
+    if (n == 1) {   // T-rule 1: a lone cell has no tree; Phi = 0
+        if (!count_only) BH_CUDA(cudaMemsetAsync(phi, 0, sizeof(double), st));
+        BH_CUDA(cudaMemsetAsync(ctx->gcount.p, 0, sizeof(uint4), st));
+        return BH_OK;
+    }
+    WalkParams P;
+    P.rec = ctx->rec.as<float4>();
+    P.aux = ctx->aux.as<WalkAux>();
+    P.leafrec = ctx->leafrec.as<float4>();
+    P.idx = ctx->idx;
+    P.phi = phi;
+    P.gcount = ctx->gcount.as<uint4>();
+    P.n = n;
+    P.ngroups = ngroups;
+    P.inv_theta = (float)(1.0 / theta);
+    P.mac = mac;
+    P.negG = -G;
+    P.stack_cap = 0;
+    if (group == 32) {
+        i64 cap = (i64)kStackPerLevel * (ctx->maxlevel + 2) + 32;
+        cap = (cap + 1) & ~1LL;
+        const size_t smem = walk_smem_per_warp((int)cap) * kWalkWarps;
+        if (smem > 227 * 1024) return BH_ERR_TOO_LARGE;
+        P.stack_cap = (int)cap;
+        const i64 npairs = (ngroups + 1) / 2;
+        if (count_only)
+            walk_pair_kernel<true><<<blocks_for(npairs, kWalkWarps), kWalkWarps * 32, smem, st>>>(P);
+        else
+            walk_pair_kernel<false><<<blocks_for(npairs, kWalkWarps), kWalkWarps * 32, smem, st>>>(P);
+    } else {
+        walk_single_kernel<<<blocks_for(n, 128), 128, 0, st>>>(P);   // counts as it goes
+    }
+    BH_CUDA(cudaGetLastError());
+    return BH_OK;
+}
+
+// The per-group counters (W6) are not kept by the hot kernel: the first call that asks for them
+// repeats the walk of the last bh_potential in count-only mode.
+int ensure_counts(bh_ctx* ctx)
+{
+    if (ctx->counts_valid) return BH_OK;
+    int rc = launch_walk(ctx, ctx->walk_theta, 0.0, nullptr, ctx->walk_group, ctx->walk_mac, true);
+    if (rc == BH_OK) ctx->counts_valid = true;
+    return rc;
+}
+
+}  // namespace
+
+extern "C" {
+
 int bh_potential(bh_ctx* ctx, double theta, double G, double* phi)
 {
     if (!ctx || !phi || !(theta >= 0.0) || isnan(G)) return BH_ERR_INVALID_ARG;
     if (!ctx->built) return BH_ERR_NOT_BUILT;
     BH_CUDA(cudaSetDevice(ctx->device));
     cudaStream_t st = ctx->stream;
-    const i64 n = ctx->n;
     const int group = ctx->group;
-    const i64 ngroups = (n + group - 1) / group;
-    BH_CUDA(ctx->gcount.ensure(sizeof(uint4) * ngroups));
     ctx->launches_walk = 0;
+    ctx->walked = false;
     BH_CUDA(cudaEventRecord(ctx->ev[EV_W0], st));
-    if (n == 1) {   // T-rule 1: a lone cell has no tree; Phi = 0
-        BH_CUDA(cudaMemsetAsync(phi, 0, sizeof(double), st));
-        BH_CUDA(cudaMemsetAsync(ctx->gcount.p, 0, sizeof(uint4), st));
-    } else {
-        WalkParams P;
-        P.rec = ctx->rec.as<float4>();
-        P.aux = ctx->aux.as<WalkAux>();
-        P.leafrec = ctx->leafrec.as<float4>();
-        P.idx = ctx->idx;
-        P.phi = phi;
-        P.gcount = ctx->gcount.as<uint4>();
-        P.n = n;
-        P.ngroups = ngroups;
-        P.inv_theta = (float)(1.0 / theta);
-        P.mac = ctx->mac;
-        P.negG = -G;
-        P.stack_cap = 0;
-        if (group == 32) {
-            i64 cap = (i64)kStackPerLevel * (ctx->maxlevel + 2) + 32;
-            cap = (cap + 1) & ~1LL;
-            const size_t smem = walk_smem_per_warp((int)cap) * kWalkWarps;
-            if (smem > 227 * 1024) return BH_ERR_TOO_LARGE;
-            P.stack_cap = (int)cap;
-            const i64 npairs = (ngroups + 1) / 2;
-            walk_pair_kernel<<<blocks_for(npairs, kWalkWarps), kWalkWarps * 32, smem, st>>>(P);
-        } else {
-            walk_single_kernel<<<blocks_for(n, 128), 128, 0, st>>>(P);
-        }
-        BH_CUDA(cudaGetLastError());
-        ctx->launches_walk = 1;
-    }
+    int rc = launch_walk(ctx, theta, G, phi, group, ctx->mac, false);
+    if (rc != BH_OK) return rc;
+    ctx->launches_walk = ctx->n > 1 ? 1 : 0;
     BH_CUDA(cudaEventRecord(ctx->ev[EV_W1], st));
     ctx->ev_walk = true;
     ctx->walked = true;
     ctx->walk_group = group;
+    ctx->walk_theta = theta;
+    ctx->walk_mac = ctx->mac;
+    ctx->counts_valid = group != 32 || ctx->n == 1;   // the per-target walk and n = 1 fill gcount themselves
     return BH_OK;
 }
 
@@ -485,6 +525,7 @@ int bh_last_group_counts(bh_ctx* ctx, int64_t* counts)
     if (!ctx || !counts) return BH_ERR_INVALID_ARG;
     if (!ctx->walked) return BH_ERR_NOT_BUILT;
     BH_CUDA(cudaSetDevice(ctx->device));
+    { int rc = ensure_counts(ctx); if (rc != BH_OK) return rc; }
     const i64 ng = (ctx->n + ctx->walk_group - 1) / ctx->walk_group;
     group_counts_export_kernel<<<blocks_for(ng, 256), 256, 0, ctx->stream>>>(ctx->gcount.as<uint4>(), ng,
                                                                              reinterpret_cast<i64*>(counts));
@@ -497,6 +538,7 @@ int bh_last_interactions(bh_ctx* ctx, uint32_t* per_target)
     if (!ctx || !per_target) return BH_ERR_INVALID_ARG;
     if (!ctx->walked) return BH_ERR_NOT_BUILT;
     BH_CUDA(cudaSetDevice(ctx->device));
+    { int rc = ensure_counts(ctx); if (rc != BH_OK) return rc; }
     per_target_counts_kernel<<<blocks_for(ctx->n, 256), 256, 0, ctx->stream>>>(ctx->gcount.as<uint4>(), ctx->idx,
                                                                                ctx->n, ctx->walk_group, per_target);
     BH_CUDA(cudaGetLastError());
@@ -512,6 +554,7 @@ int bh_get_stats(bh_ctx* ctx, bh_stats* out)
     cudaStream_t st = ctx->stream;
     DeviceScalars* ds = ctx->scalars.as<DeviceScalars>();
     if (ctx->walked) {
+        { int rc = ensure_counts(ctx); if (rc != BH_OK) return rc; }
         const i64 ng = (ctx->n + ctx->walk_group - 1) / ctx->walk_group;
         BH_CUDA(cudaMemsetAsync(ds->totals, 0, sizeof(ds->totals), st));
         group_counts_total_kernel<<<persistent_grid(ctx, 2), 256, 0, st>>>(ctx->gcount.as<uint4>(), ng, ctx->n,

@@ -59,7 +59,7 @@ struct WalkParams {
 
 __host__ __device__ inline size_t walk_smem_per_warp(int stack_cap)
 {
-    return (size_t)kU2Cap * 16 + 2 * (size_t)kU1Cap * 16 + (size_t)kCCap * 16 + (size_t)kCCap * 4 +
+    return (size_t)kU2Cap * 16 + 2 * (size_t)kU1Cap * 16 + (size_t)kCCap * 16 + (size_t)kCCap * 4 + 32 * 16 +
            (size_t)stack_cap * sizeof(uint2);
 }
 
@@ -192,22 +192,31 @@ __device__ __forceinline__ float warp_max(float v)
     return v;
 }
 
-// fp32 d^2 at the nearest / farthest point of the box [lo, hi] from q, with the rounding sequence
-// of W8 (monotone in every |component|, so they bound every member's fp32 d^2).
-__device__ __forceinline__ void box_d2(const float qx, const float qy, const float qz, const float xl, const float xh,
-                                       const float yl, const float yh, const float zl, const float zh,
-                                       float& d2min, float& d2max)
+// fp32 d^2 at the nearest / farthest point of the boxes of groups A (.x) and B (.y) from q, with the
+// rounding sequence of W8 (monotone in every |component|, so they bound every member's fp32 d^2).
+struct Box2 { float2 xl, xh, yl, yh, zl, zh; };
+
+__device__ __forceinline__ void box_d2(const float4 q, const Box2& b, float2& d2min, float2& d2max)
 {
-    const float ax = __fsub_rn(xl, qx), bx = __fsub_rn(xh, qx);
-    const float ay = __fsub_rn(yl, qy), by = __fsub_rn(yh, qy);
-    const float az = __fsub_rn(zl, qz), bz = __fsub_rn(zh, qz);
-    const float nx = fmaxf(0.f, fmaxf(ax, -bx)), fx = fmaxf(-ax, bx);
-    const float ny = fmaxf(0.f, fmaxf(ay, -by)), fy = fmaxf(-ay, by);
-    const float nz = fmaxf(0.f, fmaxf(az, -bz)), fz = fmaxf(-az, bz);
-    d2min = __fmaf_rn(nz, nz, __fmaf_rn(ny, ny, __fmul_rn(nx, nx)));
-    d2max = __fmaf_rn(fz, fz, __fmaf_rn(fy, fy, __fmul_rn(fx, fx)));
+    const float2 nqx = splat2(-q.x), nqy = splat2(-q.y), nqz = splat2(-q.z);
+    const float2 ax = __fadd2_rn(b.xl, nqx), bx = __fadd2_rn(b.xh, nqx);
+    const float2 ay = __fadd2_rn(b.yl, nqy), by = __fadd2_rn(b.yh, nqy);
+    const float2 az = __fadd2_rn(b.zl, nqz), bz = __fadd2_rn(b.zh, nqz);
+    const float2 nx = make_float2(fmaxf(0.f, fmaxf(ax.x, -bx.x)), fmaxf(0.f, fmaxf(ax.y, -bx.y)));
+    const float2 ny = make_float2(fmaxf(0.f, fmaxf(ay.x, -by.x)), fmaxf(0.f, fmaxf(ay.y, -by.y)));
+    const float2 nz = make_float2(fmaxf(0.f, fmaxf(az.x, -bz.x)), fmaxf(0.f, fmaxf(az.y, -bz.y)));
+    const float2 fx = make_float2(fmaxf(-ax.x, bx.x), fmaxf(-ax.y, bx.y));
+    const float2 fy = make_float2(fmaxf(-ay.x, by.x), fmaxf(-ay.y, by.y));
+    const float2 fz = make_float2(fmaxf(-az.x, bz.x), fmaxf(-az.y, bz.y));
+    d2min = __ffma2_rn(nz, nz, __ffma2_rn(ny, ny, __fmul2_rn(nx, nx)));
+    d2max = __ffma2_rn(fz, fz, __ffma2_rn(fy, fy, __fmul2_rn(fx, fx)));
 }
 
+// COUNT = false: the hot kernel -- builds the lists, evaluates them, writes Phi.
+// COUNT = true : the same traversal and the same decisions, but it only counts (W6): per group
+//                {internal nodes accepted, leaf cells summed, internal nodes opened, nodes that
+//                needed the per-member test}; no lists, no arithmetic on masses, no Phi.
+template <bool COUNT>
 __global__ void __launch_bounds__(kWalkWarps * 32, 3)
 walk_pair_kernel(const WalkParams P)
 {
@@ -224,7 +233,8 @@ walk_pair_kernel(const WalkParams P)
     float* UB = UA + 4 * kU1Cap;                                        // group B only (SoA)
     float4* C = reinterpret_cast<float4*>(UB + 4 * kU1Cap);             // checked leaf cells
     u32* Cm = reinterpret_cast<u32*>(C + kCCap);                        //   and the groups they serve
-    uint2* stack = reinterpret_cast<uint2*>(Cm + kCCap);                // (first child slot, count | groups << 30)
+    float4* amb = reinterpret_cast<float4*>(Cm + kCCap);                // nodes awaiting the member vote
+    uint2* stack = reinterpret_cast<uint2*>(amb + 32);                  // (first child slot, count | groups << 30)
 
     // ---- the targets (W-rule 1): group g = sorted slots [32g, 32g+32) ----
     const bool hasB = gB < P.ngroups;
@@ -234,18 +244,15 @@ walk_pair_kernel(const WalkParams P)
     const i64 sA = gA * 32 + lane, sB = gB * 32 + lane;
     const float4 tA = __ldg(P.leafrec + (liveA ? sA : gA * 32));
     const float4 tB = __ldg(P.leafrec + (liveB ? sB : (hasB ? gB * 32 : gA * 32)));
-    // bounding boxes of the live targets of each group
-    const float axl = warp_min(tA.x), axh = warp_max(tA.x);
-    const float ayl = warp_min(tA.y), ayh = warp_max(tA.y);
-    const float azl = warp_min(tA.z), azh = warp_max(tA.z);
-    const float bxl = warp_min(tB.x), bxh = warp_max(tB.x);
-    const float byl = warp_min(tB.y), byh = warp_max(tB.y);
-    const float bzl = warp_min(tB.z), bzh = warp_max(tB.z);
+    Box2 box;                                         // bounding boxes of the live targets of A and B
+    box.xl = make_float2(warp_min(tA.x), warp_min(tB.x)); box.xh = make_float2(warp_max(tA.x), warp_max(tB.x));
+    box.yl = make_float2(warp_min(tA.y), warp_min(tB.y)); box.yh = make_float2(warp_max(tA.y), warp_max(tB.y));
+    box.zl = make_float2(warp_min(tA.z), warp_min(tB.z)); box.zh = make_float2(warp_max(tA.z), warp_max(tB.z));
     const float2 npx = make_float2(-tA.x, -tB.x), npy = make_float2(-tA.y, -tB.y), npz = make_float2(-tA.z, -tB.z);
 
     double accA = 0.0, accB = 0.0;
     int nU2 = 0, nUA = 0, nUB = 0, nC = 0;          // list fill (warp-uniform)
-    u32 cAccA = 0, cLeafA = 0, cOpenA = 0, cExA = 0;  // per-lane partial counters, reduced at the end
+    u32 cAccA = 0, cLeafA = 0, cOpenA = 0, cExA = 0;  // COUNT: per-lane partial counters
     u32 cAccB = 0, cLeafB = 0, cOpenB = 0, cExB = 0;
     int sp = 0;
     if (P.n >= 2) {                             // root is tested like any other node (W-rule 2)
@@ -258,6 +265,8 @@ walk_pair_kernel(const WalkParams P)
     const int sub = lane >> 3, j = lane & 7;
     const float inv_theta = P.inv_theta;
     const bool mac94 = P.mac == 1;
+    const float4* __restrict__ rec = P.rec;
+    const uint4* __restrict__ aux = reinterpret_cast<const uint4*>(P.aux);
     while (sp > 0) {
         // ---- pop up to 4 entries; lane (sub, j) takes child j of entry sub ----
         int npop = sp < 4 ? sp : 4;
@@ -279,101 +288,114 @@ walk_pair_kernel(const WalkParams P)
         }
         sp -= npop;
         __syncwarp();
-        const u32 msk = e.y >> 30;
         const bool have = jj < (e.y & kCountMask);
+        const u32 msk = have ? (e.y >> 30) : 0u;        // groups that want this child
         const u32 slot = e.x + jj;
         float4 r = make_float4(0.f, 0.f, 0.f, 0.f);
-        WalkAux a; a.size = 0.f; a.delta = 0.f; a.first = 0u; a.count = 0u;
-        if (have) {
-            r = __ldg(P.rec + slot);
-            const uint4 t = __ldg(reinterpret_cast<const uint4*>(P.aux + slot));
-            a.size = __uint_as_float(t.x); a.delta = __uint_as_float(t.y); a.first = t.z; a.count = t.w;
-        }
-        const bool internal = have && a.count > 0u;
-        const bool leaf = have && a.count == 0u;
-        const bool wA = (msk & 1u) != 0u, wB = (msk & 2u) != 0u;
+        uint4 t = make_uint4(0u, 0u, 0u, 0u);           // {size, delta, first child, child count}
+        if (have) { r = __ldg(rec + slot); t = __ldg(aux + slot); }
+        const bool internal = t.w > 0u;
+        const bool leaf = have && !internal;
         // ---- opening test (W-rule 2, fp32 decision W8): r_c = l*(1/theta) [+ delta] ----
-        float rc = __fmul_rn(a.size, inv_theta);
-        if (mac94) rc = __fadd_rn(rc, a.delta);
+        float rc = __fmul_rn(__uint_as_float(t.x), inv_theta);
+        if (mac94) rc = __fadd_rn(rc, __uint_as_float(t.y));
         const float rc2 = __fmul_rn(rc, rc);
-        float d2minA, d2maxA, d2minB, d2maxB;
-        box_d2(r.x, r.y, r.z, axl, axh, ayl, ayh, azl, azh, d2minA, d2maxA);
-        box_d2(r.x, r.y, r.z, bxl, bxh, byl, byh, bzl, bzh, d2minB, d2maxB);
-        bool accA_ = internal && wA && d2minA > rc2;                  // every member of A passes
-        bool accB_ = internal && wB && d2minB > rc2;
-        const bool ambA = internal && wA && !accA_ && d2maxA > rc2;   // some member might pass, some not
-        const bool ambB = internal && wB && !accB_ && d2maxB > rc2;
-        cExA += ambA; cExB += ambB;
-        // ---- nodes a box cannot decide: per-member test + vote (PAPER.md:176) ----
-        u32 am = __ballot_sync(0xffffffffu, ambA || ambB);
-        while (am) {
-            const int src = __ffs(am) - 1;
-            am &= am - 1;
-            const float qx = __shfl_sync(0xffffffffu, r.x, src);
-            const float qy = __shfl_sync(0xffffffffu, r.y, src);
-            const float qz = __shfl_sync(0xffffffffu, r.z, src);
-            const float q2 = __shfl_sync(0xffffffffu, rc2, src);
-            const float2 dx = __fadd2_rn(splat2(qx), npx), dy = __fadd2_rn(splat2(qy), npy),
-                         dz = __fadd2_rn(splat2(qz), npz);
-            const float2 d2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
-            const bool okA = __all_sync(0xffffffffu, !liveA || d2.x > q2);
-            const bool okB = __all_sync(0xffffffffu, !liveB || d2.y > q2);
-            if ((int)lane == src) {
-                if (ambA) accA_ = okA;
-                if (ambB) accB_ = okB;
-            }
+        float2 d2min, d2max;
+        box_d2(r, box, d2min, d2max);
+        u32 accm = 0u, ambm = 0u;                       // groups that accept / need the member vote
+        if (internal) {
+            accm = ((d2min.x > rc2 ? 1u : 0u) | (d2min.y > rc2 ? 2u : 0u)) & msk;     // every member passes
+            ambm = ((d2max.x > rc2 ? 1u : 0u) | (d2max.y > rc2 ? 2u : 0u)) & msk & ~accm;
         }
-        const bool opA = internal && wA && !accA_, opB = internal && wB && !accB_;
-        const u32 om = (opA ? 1u : 0u) | (opB ? 2u : 0u);               // groups that open the node
+        // ---- nodes a box cannot decide: per-member test + vote (PAPER.md:176) ----
+        const u32 bAmb = __ballot_sync(0xffffffffu, ambm != 0u);
+        if (bAmb) {
+            const int myr = __popc(bAmb & lt);
+            if (ambm) amb[myr] = make_float4(r.x, r.y, r.z, rc2);
+            __syncwarp();
+            const int na = __popc(bAmb);
+            u32 resA = 0u, resB = 0u;
+            for (int i = 0; i < na; ++i) {
+                const float4 q = amb[i];
+                const float2 dx = __fadd2_rn(splat2(q.x), npx), dy = __fadd2_rn(splat2(q.y), npy),
+                             dz = __fadd2_rn(splat2(q.z), npz);
+                const float2 d2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
+                const u32 okA = __all_sync(0xffffffffu, !liveA || d2.x > q.w) ? 1u : 0u;
+                const u32 okB = __all_sync(0xffffffffu, !liveB || d2.y > q.w) ? 1u : 0u;
+                resA |= okA << i;
+                resB |= okB << i;
+            }
+            accm |= ambm & (((resA >> myr) & 1u) | (((resB >> myr) & 1u) << 1));
+            if (COUNT) { cExA += ambm & 1u; cExB += ambm >> 1; }
+            __syncwarp();
+        }
+        const u32 om = internal ? (msk & ~accm) : 0u;                   // groups that open the node
+        // ---- push opened nodes ----
+        const u32 bOp = __ballot_sync(0xffffffffu, om != 0u);
+        if (om) stack[sp + __popc(bOp & lt)] = make_uint2(t.z, t.w | (om << 30));
+        sp += __popc(bOp);
+        if (COUNT) {
+            const bool bucket = internal && !(__uint_as_float(t.x) < __int_as_float(0x7f800000));
+            cAccA += accm & 1u; cAccB += accm >> 1;
+            if (leaf) { cLeafA += msk & 1u; cLeafB += msk >> 1; }
+            if (!bucket) { cOpenA += om & 1u; cOpenB += om >> 1; }
+            __syncwarp();
+            continue;
+        }
+        // ---- append accepted nodes and leaf cells to the lists ----
         // leaf cells inside a group's box may be a target's own cell or coincide with one
-        const bool danger = leaf && ((wA && !(d2minA > 0.f)) || (wB && !(d2minB > 0.f)));
-        const u32 um = internal ? ((accA_ ? 1u : 0u) | (accB_ ? 2u : 0u)) : ((leaf && !danger) ? msk : 0u);
+        const bool danger = leaf && (((msk & 1u) && !(d2min.x > 0.f)) || ((msk & 2u) && !(d2min.y > 0.f)));
+        const u32 um = internal ? accm : (danger ? 0u : msk);
         const bool toU2 = um == 3u, toUA = um == 1u, toUB = um == 2u;
-        // ---- append to the lists; push opened nodes ----
         const u32 bU2 = __ballot_sync(0xffffffffu, toU2);
         const u32 bUA = __ballot_sync(0xffffffffu, toUA);
         const u32 bUB = __ballot_sync(0xffffffffu, toUB);
         const u32 bC = __ballot_sync(0xffffffffu, danger);
-        const u32 bOp = __ballot_sync(0xffffffffu, om != 0u);
-        if (toU2) U2[nU2 + __popc(bU2 & lt)] = r;
-        if (toUA) u1_store(UA, nUA + __popc(bUA & lt), r);
-        if (toUB) u1_store(UB, nUB + __popc(bUB & lt), r);
-        if (danger) { const int k = nC + __popc(bC & lt); C[k] = r; Cm[k] = msk; }
-        if (om) stack[sp + __popc(bOp & lt)] = make_uint2(a.first, a.count | (om << 30));
-        sp += __popc(bOp);
+        const u32 bsel = toU2 ? bU2 : (toUA ? bUA : (toUB ? bUB : bC));
+        const int rank = __popc(bsel & lt);
+        if (toU2) U2[nU2 + rank] = r;
+        if (toUA) u1_store(UA, nUA + rank, r);
+        if (toUB) u1_store(UB, nUB + rank, r);
+        if (danger) { C[nC + rank] = r; Cm[nC + rank] = msk; }
         nU2 += __popc(bU2); nUA += __popc(bUA); nUB += __popc(bUB); nC += __popc(bC);
-        const bool bucket = internal && !(a.size < __int_as_float(0x7f800000));
-        cAccA += accA_; cAccB += accB_;
-        cLeafA += leaf && wA; cLeafB += leaf && wB;
-        cOpenA += opA && !bucket; cOpenB += opB && !bucket;
         __syncwarp();
         // ---- evaluate a list before the next step could overflow it ----
-        if (nU2 > kU2Cap - kStepMax) {
-            u2_pad(U2, nU2);
-            __syncwarp();
-            eval_u2(U2, nU2, npx, npy, npz, accA, accB);
-            nU2 = 0;
+        if ((((nUA | nUB | nC) >> 5) != 0) || nU2 >= kU2Cap - kStepMax) {
+            if (nU2 >= kU2Cap - kStepMax) {
+                u2_pad(U2, nU2);
+                __syncwarp();
+                eval_u2(U2, nU2, npx, npy, npz, accA, accB);
+                nU2 = 0;
+            }
+            if (nUA >= kU1Cap - kStepMax) {
+                u1_pad(UA, nUA);
+                __syncwarp();
+                accA += eval_u1(UA, nUA, npx.x, npy.x, npz.x);
+                nUA = 0;
+            }
+            if (nUB >= kU1Cap - kStepMax) {
+                u1_pad(UB, nUB);
+                __syncwarp();
+                accB += eval_u1(UB, nUB, npx.y, npy.y, npz.y);
+                nUB = 0;
+            }
+            if (nC >= kCCap - kStepMax) {
+                eval_c(C, Cm, nC, npx, npy, npz, accA, accB);
+                nC = 0;
+            }
             __syncwarp();
         }
-        if (nUA > kU1Cap - kStepMax) {
-            u1_pad(UA, nUA);
-            __syncwarp();
-            accA += eval_u1(UA, nUA, npx.x, npy.x, npz.x);
-            nUA = 0;
-            __syncwarp();
+    }
+    if (COUNT) {
+        cAccA = __reduce_add_sync(0xffffffffu, cAccA); cLeafA = __reduce_add_sync(0xffffffffu, cLeafA);
+        cOpenA = __reduce_add_sync(0xffffffffu, cOpenA); cExA = __reduce_add_sync(0xffffffffu, cExA);
+        cAccB = __reduce_add_sync(0xffffffffu, cAccB); cLeafB = __reduce_add_sync(0xffffffffu, cLeafB);
+        cOpenB = __reduce_add_sync(0xffffffffu, cOpenB); cExB = __reduce_add_sync(0xffffffffu, cExB);
+        if (lane == 0) {
+            P.gcount[gA] = make_uint4(cAccA, cLeafA, cOpenA, cExA);
+            if (hasB) P.gcount[gB] = make_uint4(cAccB, cLeafB, cOpenB, cExB);
         }
-        if (nUB > kU1Cap - kStepMax) {
-            u1_pad(UB, nUB);
-            __syncwarp();
-            accB += eval_u1(UB, nUB, npx.y, npy.y, npz.y);
-            nUB = 0;
-            __syncwarp();
-        }
-        if (nC > kCCap - kStepMax) {
-            eval_c(C, Cm, nC, npx, npy, npz, accA, accB);
-            nC = 0;
-            __syncwarp();
-        }
+        return;
     }
     if (nU2 > 0) {
         u2_pad(U2, nU2);
@@ -394,14 +416,6 @@ walk_pair_kernel(const WalkParams P)
     // ---- a7: Phi_t = -G * sum, written in the original cell order (W-rule 4) ----
     if (liveA) P.phi[__ldg(P.idx + sA)] = P.negG * accA;
     if (liveB) P.phi[__ldg(P.idx + sB)] = P.negG * accB;
-    cAccA = __reduce_add_sync(0xffffffffu, cAccA); cLeafA = __reduce_add_sync(0xffffffffu, cLeafA);
-    cOpenA = __reduce_add_sync(0xffffffffu, cOpenA); cExA = __reduce_add_sync(0xffffffffu, cExA);
-    cAccB = __reduce_add_sync(0xffffffffu, cAccB); cLeafB = __reduce_add_sync(0xffffffffu, cLeafB);
-    cOpenB = __reduce_add_sync(0xffffffffu, cOpenB); cExB = __reduce_add_sync(0xffffffffu, cExB);
-    if (lane == 0) {
-        P.gcount[gA] = make_uint4(cAccA, cLeafA, cOpenA, cExA);
-        if (hasB) P.gcount[gB] = make_uint4(cAccB, cLeafB, cOpenB, cExB);
-    }
 }
 
 // ---- BH_OPT_GROUP = 1 (W5): every target walks alone --------------------------------------------
