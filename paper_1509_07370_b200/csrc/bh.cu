@@ -39,7 +39,8 @@ struct DevBuf {                 // grow-only device buffer
 
 struct DeviceScalars {          // small device-resident results read back by the host
     KeyReduce keyred;
-    u32 level_hist[kNumLevels];
+    u32 topo_rows[kTopoDigits + 1];   // row starts of the scanned level histogram + grand total
+    u32 scan_total;
     u32 max_bucket;
     u32 walk_overflow;
     unsigned long long totals[5];
@@ -67,19 +68,21 @@ struct bh_ctx {
     int depth = 0, maxlevel = 0, sort_passes = 0;
     i64 n_clamped = 0, max_bucket = 1;
     double cube[4] = {0, 0, 0, 1};
-    i64 level_base[kNumLevels + 1] = {0};
+    TopoLevels lv = {};                   // canonical-id and slot bases per level
 
     // per cell
     DevBuf keysA, keysB, idxA, idxB;      // ping-pong (key, index)
     u64* keys = nullptr;                  // sorted keys (one of keysA/keysB)
     u32* idx = nullptr;                   // perm: original index of sorted slot
-    DevBuf leaf64, leafrec, slot_of, clev, pre_base;
+    DevBuf clev, leaf_slot;               // c(s); slot of sorted cell s
+    DevBuf leaf64, slot_of;               // bh_potential_direct's own copies (built on its first call)
+    bool direct_ready = false;
     // sort / scan scratch
     DevBuf hist, scan_scratch;
-    // per node (pre-order, then canonical order)
-    DevBuf nkey, npre, nlo, bkey, bpre, bfs_of, blo, bhi, nchild, cstart, child_base, node_slot, mom, delta64;
+    // per node (canonical order)
+    DevBuf nlo, nfirst, node_slot, delta64;
     // per slot
-    DevBuf rec, aux, slot_src;
+    DevBuf rec64, rec, aux;
     // walk
     DevBuf gcount;
     DevBuf scalars;                       // DeviceScalars
@@ -182,12 +185,10 @@ int bh_destroy(bh_ctx* ctx)
     if (!ctx) return BH_OK;
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
-    DevBuf* all[] = {&ctx->keysA, &ctx->keysB, &ctx->idxA, &ctx->idxB, &ctx->leaf64, &ctx->leafrec, &ctx->slot_of,
-                     &ctx->clev, &ctx->pre_base, &ctx->hist, &ctx->scan_scratch, &ctx->nkey, &ctx->npre, &ctx->nlo,
-                     &ctx->bkey, &ctx->bpre, &ctx->bfs_of, &ctx->blo, &ctx->bhi, &ctx->nchild, &ctx->cstart,
-                     &ctx->child_base, &ctx->node_slot, &ctx->mom, &ctx->delta64, &ctx->rec, &ctx->aux,
-                     &ctx->slot_src, &ctx->gcount, &ctx->scalars, &ctx->stage[0], &ctx->stage[1], &ctx->stage[2],
-                     &ctx->stage[3], &ctx->stage_phi};
+    DevBuf* all[] = {&ctx->keysA, &ctx->keysB, &ctx->idxA, &ctx->idxB, &ctx->clev, &ctx->leaf_slot, &ctx->leaf64,
+                     &ctx->slot_of, &ctx->hist, &ctx->scan_scratch, &ctx->nlo, &ctx->nfirst, &ctx->node_slot,
+                     &ctx->delta64, &ctx->rec64, &ctx->rec, &ctx->aux, &ctx->gcount, &ctx->scalars, &ctx->stage[0],
+                     &ctx->stage[1], &ctx->stage[2], &ctx->stage[3], &ctx->stage_phi};
     for (DevBuf* b : all) b->release();
     if (ctx->h_scalars) cudaFreeHost(ctx->h_scalars);
     for (int i = 0; i < EV_COUNT; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
@@ -224,13 +225,14 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
     BH_CUDA(ctx->keysB.ensure(sizeof(u64) * n));
     BH_CUDA(ctx->idxA.ensure(sizeof(u32) * n));
     BH_CUDA(ctx->idxB.ensure(sizeof(u32) * n));
-    BH_CUDA(ctx->leaf64.ensure(sizeof(double4) * n));
-    BH_CUDA(ctx->leafrec.ensure(sizeof(float4) * n));
-    BH_CUDA(ctx->slot_of.ensure(sizeof(u32) * n));
     BH_CUDA(ctx->clev.ensure((size_t)n + 16));
-    BH_CUDA(ctx->pre_base.ensure(sizeof(u32) * (n + 4)));
-    BH_CUDA(ctx->hist.ensure(sizeof(u32) * (sort_hist_elems(n) + 4)));
-    BH_CUDA(ctx->scan_scratch.ensure(sizeof(u32) * (scan_scratch_elems(n > (i64)sort_hist_elems(n) ? n : (i64)sort_hist_elems(n)) + 4)));
+    BH_CUDA(ctx->leaf_slot.ensure(sizeof(u32) * n));
+    {
+        const size_t he = sort_hist_elems(n) > topo_hist_elems(n) ? sort_hist_elems(n) : topo_hist_elems(n);
+        BH_CUDA(ctx->hist.ensure(sizeof(u32) * (he + 4)));
+        BH_CUDA(ctx->scan_scratch.ensure(sizeof(u32) * (scan_scratch_elems((i64)he) + 4)));
+    }
+    ctx->direct_ready = false;
 
     BH_CUDA(cudaMemsetAsync(ds, 0, sizeof(DeviceScalars), st));
     {   // key_and starts as all ones
@@ -275,92 +277,68 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
     ctx->idx = v0;
     BH_CUDA(cudaEventRecord(ctx->ev[EV_SORT], st));
 
-    // ---- a3: permute ----
-    permute_kernel<<<blocks_for(n, 256), 256, 0, st>>>(ctx->idx, x, y, z, m, n, ctx->leaf64.as<double4>(),
-                                                       ctx->leafrec.as<float4>(), ctx->slot_of.as<u32>());
-    BH_CUDA(cudaGetLastError());
-    ctx->launches_build += 1;
-    BH_CUDA(cudaEventRecord(ctx->ev[EV_PERM], st));
-
-    // ---- a4: topology ----
+    // ---- a4: topology (a3, the permutation of the cell data, is fused into the assigning kernel) ----
     ctx->nn = 0; ctx->nslots = 0; ctx->depth = 0; ctx->maxlevel = 0; ctx->max_bucket = 1;
-    for (int l = 0; l <= kNumLevels; ++l) ctx->level_base[l] = 0;
+    memset(&ctx->lv, 0, sizeof(ctx->lv));
     if (n >= 2) {
-        u32* cnt = ctx->pre_base.as<u32>();
-        node_count_kernel<<<persistent_grid(ctx, 8), 256, 0, st>>>(ctx->keys, n, cnt, ctx->clev.as<signed char>(),
-                                                                    ds->level_hist);
+        const i64 nchunks = topo_chunks(n);
+        const unsigned tgrid = blocks_for(nchunks, kTopoThreads / 32);
+        u32* hist = ctx->hist.as<u32>();
+        topo_count_kernel<<<tgrid, kTopoThreads, 0, st>>>(ctx->keys, n, ctx->clev.as<signed char>(), hist, nchunks);
         BH_CUDA(cudaGetLastError());
-        // read-back 2: nodes per level (sizes every node / slot array)
-        BH_CUDA(cudaMemcpyAsync(ctx->h_scalars->level_hist, ds->level_hist, sizeof(u32) * kNumLevels,
+        BH_CUDA(exclusive_scan_u32(hist, hist, (i64)kTopoDigits * nchunks, ctx->scan_scratch.as<u32>(),
+                                   &ds->scan_total, st));
+        topo_totals_kernel<<<1, 64, 0, st>>>(hist, nchunks, &ds->scan_total, ds->topo_rows);
+        BH_CUDA(cudaGetLastError());
+        // read-back 2: entities and nodes per level (sizes every node / slot array)
+        BH_CUDA(cudaMemcpyAsync(ctx->h_scalars->topo_rows, ds->topo_rows, sizeof(u32) * (kTopoDigits + 1),
                                 cudaMemcpyDeviceToHost, st));
-        BH_CUDA(exclusive_scan_u32(cnt, cnt, n, ctx->scan_scratch.as<u32>(), nullptr, st));
+        BH_CUDA(cudaEventRecord(ctx->ev[EV_PERM], st));
         BH_CUDA(cudaStreamSynchronize(st));
-        i64 nn = 0;
-        for (int l = 0; l < kNumLevels; ++l) {
-            ctx->level_base[l] = nn;
-            const i64 c = ctx->h_scalars->level_hist[l];
-            if (c) { ctx->maxlevel = l; if (l < kMaxLevel) ctx->depth = l; }
-            nn += c;
-        }
-        ctx->level_base[kNumLevels] = nn;
+        const u32* rows = ctx->h_scalars->topo_rows;
+        const i64 nslots = rows[kSlotLevels];                 // entities of all levels = n + n_nodes
+        const i64 nn = (i64)rows[kTopoDigits] - nslots;
+        for (int l = 0; l <= kSlotLevels; ++l) ctx->lv.slot_base[l] = rows[l];
+        for (int l = 0; l <= kNumLevels; ++l) ctx->lv.node_base[l] = (u32)(rows[kSlotLevels + l] - nslots);
+        for (int l = 0; l < kNumLevels; ++l)
+            if (ctx->lv.node_base[l + 1] > ctx->lv.node_base[l]) { ctx->maxlevel = l; if (l < kMaxLevel) ctx->depth = l; }
         ctx->nn = nn;
-        ctx->nslots = n + nn;
-        if (ctx->nslots >= 4294967296LL) return BH_ERR_TOO_LARGE;
+        ctx->nslots = nslots;
+        if (nslots != n + nn) {
+            snprintf(ctx->cuda_msg, sizeof(ctx->cuda_msg), "topology: %lld entities for %lld cells + %lld nodes",
+                     (long long)nslots, (long long)n, (long long)nn);
+            return BH_ERR_CUDA;
+        }
 
-        BH_CUDA(ctx->nkey.ensure(sizeof(u64) * nn));
-        BH_CUDA(ctx->npre.ensure(sizeof(u32) * nn));
         BH_CUDA(ctx->nlo.ensure(sizeof(u32) * nn));
-        BH_CUDA(ctx->bkey.ensure(sizeof(u64) * nn));
-        BH_CUDA(ctx->bpre.ensure(sizeof(u32) * nn));
-        BH_CUDA(ctx->bfs_of.ensure(sizeof(u32) * nn));
-        BH_CUDA(ctx->blo.ensure(sizeof(u32) * nn));
-        BH_CUDA(ctx->bhi.ensure(sizeof(u32) * nn));
-        BH_CUDA(ctx->nchild.ensure(sizeof(u32) * (nn + 4)));
-        BH_CUDA(ctx->cstart.ensure(sizeof(u32) * 8 * nn));
-        BH_CUDA(ctx->child_base.ensure(sizeof(u32) * (nn + 4)));
+        BH_CUDA(ctx->nfirst.ensure(sizeof(u32) * (nn + 4)));
         BH_CUDA(ctx->node_slot.ensure(sizeof(u32) * nn));
-        BH_CUDA(ctx->mom.ensure(sizeof(double4) * nn));
         BH_CUDA(ctx->delta64.ensure(sizeof(double) * nn));
-        BH_CUDA(ctx->rec.ensure(sizeof(float4) * ctx->nslots));
-        BH_CUDA(ctx->aux.ensure(sizeof(WalkAux) * ctx->nslots));
-        BH_CUDA(ctx->slot_src.ensure(sizeof(int) * ctx->nslots));
-        BH_CUDA(ctx->hist.ensure(sizeof(u32) * (sort_hist_elems(nn) + 4)));
-        BH_CUDA(ctx->scan_scratch.ensure(sizeof(u32) * (scan_scratch_elems(nn > (i64)sort_hist_elems(nn) ? nn : (i64)sort_hist_elems(nn)) + 4)));
+        BH_CUDA(ctx->rec64.ensure(sizeof(double4) * nslots));
+        BH_CUDA(ctx->rec.ensure(sizeof(float4) * nslots));
+        BH_CUDA(ctx->aux.ensure(sizeof(WalkAux) * nslots));
 
-        node_emit_kernel<<<blocks_for(n, 256), 256, 0, st>>>(ctx->clev.as<signed char>(), cnt, n, ctx->nkey.as<u64>(),
-                                                             ctx->npre.as<u32>(), ctx->nlo.as<u32>());
+        topo_assign_kernel<<<tgrid, kTopoThreads, 0, st>>>(
+            ctx->clev.as<signed char>(), n, ctx->idx, x, y, z, m, hist, nchunks, (u32)nslots,
+            ctx->leaf_slot.as<u32>(), ctx->node_slot.as<u32>(), ctx->nfirst.as<u32>(), ctx->nlo.as<u32>(),
+            ctx->rec64.as<double4>(), ctx->rec.as<float4>(), ctx->aux.as<WalkAux>());
         BH_CUDA(cudaGetLastError());
-        // pre-order -> canonical (level, prefix) order: one stable counting pass on the level
-        BH_CUDA(radix_pass(ctx->nkey.as<u64>(), ctx->npre.as<u32>(), ctx->bkey.as<u64>(), ctx->bpre.as<u32>(), nn, 0,
-                           0xffu, ctx->hist.as<u32>(), ctx->scan_scratch.as<u32>(), st));
-        node_children_kernel<<<blocks_for(nn, 256), 256, 0, st>>>(
-            ctx->keys, n, ctx->bkey.as<u64>(), ctx->bpre.as<u32>(), ctx->nlo.as<u32>(), nn, ctx->bfs_of.as<u32>(),
-            ctx->blo.as<u32>(), ctx->bhi.as<u32>(), ctx->nchild.as<u32>(), ctx->cstart.as<u32>(), &ds->max_bucket);
-        BH_CUDA(cudaGetLastError());
-        BH_CUDA(exclusive_scan_u32(ctx->nchild.as<u32>(), ctx->child_base.as<u32>(), nn, ctx->scan_scratch.as<u32>(),
-                                   nullptr, st));
-        slot_fill_kernel<<<blocks_for(nn * 8, 256), 256, 0, st>>>(
-            ctx->bkey.as<u64>(), ctx->bpre.as<u32>(), ctx->blo.as<u32>(), ctx->bhi.as<u32>(), ctx->nchild.as<u32>(),
-            ctx->cstart.as<u32>(), ctx->child_base.as<u32>(), cnt, ctx->bfs_of.as<u32>(), nn,
-            ctx->leafrec.as<float4>(), ctx->slot_src.as<int>(), ctx->node_slot.as<u32>(), ctx->rec.as<float4>(),
-            ctx->aux.as<WalkAux>());
-        BH_CUDA(cudaGetLastError());
-        ctx->launches_build += 1 + 3 + 1 + 5 + 1 + 3 + 1;   // count, scan, emit, level pass, children, scan, fill
+        ctx->launches_build += 1 + 3 + 1 + 1;   // count, scan, totals, assign
         BH_CUDA(cudaEventRecord(ctx->ev[EV_TOPO], st));
 
         // ---- a5: moments, deepest level first ----
         for (int l = ctx->maxlevel; l >= 0; --l) {
-            const i64 b0 = ctx->level_base[l], b1 = ctx->level_base[l + 1];
+            const i64 b0 = ctx->lv.node_base[l], b1 = ctx->lv.node_base[l + 1];
             if (b1 == b0) continue;
             moments_kernel<<<blocks_for(b1 - b0, 128), 128, 0, st>>>(
-                b0, b1, l, ctx->keys, ctx->blo.as<u32>(), ctx->nchild.as<u32>(), ctx->child_base.as<u32>(),
-                ctx->slot_src.as<int>(), ctx->node_slot.as<u32>(), ctx->leaf64.as<double4>(), ctx->mom.as<double4>(),
-                ctx->delta64.as<double>(), ctx->rec.as<float4>(), ctx->aux.as<WalkAux>(), cube[0], cube[1], cube[2],
-                cube[3]);
+                b0, b1, l, ctx->lv.slot_base[l + 2], ctx->keys, ctx->nlo.as<u32>(), ctx->nfirst.as<u32>(),
+                ctx->node_slot.as<u32>(), ctx->rec64.as<double4>(), ctx->delta64.as<double>(),
+                ctx->rec.as<float4>(), ctx->aux.as<WalkAux>(), &ds->max_bucket, cube[0], cube[1], cube[2], cube[3]);
             BH_CUDA(cudaGetLastError());
             ctx->launches_build += 1;
         }
     } else {
+        BH_CUDA(cudaEventRecord(ctx->ev[EV_PERM], st));
         BH_CUDA(cudaEventRecord(ctx->ev[EV_TOPO], st));
     }
     BH_CUDA(cudaEventRecord(ctx->ev[EV_MOM], st));
@@ -389,7 +367,7 @@ int launch_walk(bh_ctx* ctx, double theta, double G, double* phi, int group, int
     WalkParams P;
     P.rec = ctx->rec.as<float4>();
     P.aux = ctx->aux.as<WalkAux>();
-    P.leafrec = ctx->leafrec.as<float4>();
+    P.leaf_slot = ctx->leaf_slot.as<u32>();
     P.idx = ctx->idx;
     P.phi = phi;
     P.gcount = ctx->gcount.as<uint4>();
@@ -464,6 +442,20 @@ int bh_potential_direct(bh_ctx* ctx, double G, const int64_t* targets, int64_t n
     } else if (nt < 0) return BH_ERR_INVALID_ARG;
     if (nt == 0) return BH_OK;
     BH_CUDA(cudaSetDevice(ctx->device));
+    if (!ctx->direct_ready) {     // sorted fp64 copy of the cells + inverse permutation, once per build
+        BH_CUDA(ctx->leaf64.ensure(sizeof(double4) * ctx->n));
+        BH_CUDA(ctx->slot_of.ensure(sizeof(u32) * ctx->n));
+        if (ctx->n == 1) {
+            BH_CUDA(cudaMemsetAsync(ctx->leaf64.p, 0, sizeof(double4), ctx->stream));
+            BH_CUDA(cudaMemsetAsync(ctx->slot_of.p, 0, sizeof(u32), ctx->stream));
+        } else {
+            direct_prepare_kernel<<<blocks_for(ctx->n, 256), 256, 0, ctx->stream>>>(
+                ctx->idx, ctx->leaf_slot.as<u32>(), ctx->rec64.as<double4>(), ctx->n, ctx->leaf64.as<double4>(),
+                ctx->slot_of.as<u32>());
+            BH_CUDA(cudaGetLastError());
+        }
+        ctx->direct_ready = true;
+    }
     direct_kernel<<<blocks_for(nt, kDirectThreads), kDirectThreads, 0, ctx->stream>>>(
         ctx->leaf64.as<double4>(), ctx->n, ctx->slot_of.as<u32>(), reinterpret_cast<const i64*>(targets), nt, -G, phi);
     BH_CUDA(cudaGetLastError());
@@ -512,8 +504,8 @@ int bh_export_tree(bh_ctx* ctx, uint64_t* keys, uint32_t* perm, int32_t* level, 
     if (perm) BH_CUDA(cudaMemcpyAsync(perm, ctx->idx, sizeof(u32) * ctx->n, cudaMemcpyDeviceToDevice, st));
     if (ctx->nn > 0) {
         export_nodes_kernel<<<blocks_for(ctx->nn, 256), 256, 0, st>>>(
-            ctx->nn, ctx->keys, ctx->bkey.as<u64>(), ctx->blo.as<u32>(), ctx->bhi.as<u32>(), ctx->nchild.as<u32>(),
-            ctx->mom.as<double4>(), ctx->delta64.as<double>(), level, reinterpret_cast<u64*>(prefix),
+            ctx->nn, ctx->n, ctx->lv, ctx->keys, ctx->nlo.as<u32>(), ctx->nfirst.as<u32>(), ctx->node_slot.as<u32>(),
+            ctx->rec64.as<double4>(), ctx->delta64.as<double>(), level, reinterpret_cast<u64*>(prefix),
             reinterpret_cast<i64*>(lo), reinterpret_cast<i64*>(hi), nchild, M, Rx, Ry, Rz, delta);
         BH_CUDA(cudaGetLastError());
     }

@@ -6,14 +6,20 @@
 // share the prefix; ranges of >= 2 cells are internal nodes (single-child chains kept), one cell is
 // a leaf cell, >= 2 cells with identical keys form a level-21 bucket.
 //
-// Construction (no locks, no spinning, unlike the paper's insertion kernel PAPER.md:146-150):
-//   c(s) = number of octree levels keys s and s+1 share.  A node of level l starts at sorted slot
-//   s iff c(s-1) < l <= c(s); so slot s starts max(0, c(s) - c(s-1)) nodes, and an exclusive scan
-//   numbers all nodes in depth-first pre-order.  A stable counting sort by level (one radix pass)
-//   turns that into breadth-first = canonical (level, prefix) order.  Per node, the end of its
-//   range and its <= 8 child ranges are found by galloping searches in the sorted keys.  Children
-//   of consecutive nodes get consecutive "slots" in the walk arrays (root = slot 0), so the <= 8
-//   children of a node are one contiguous run of records.
+// Construction (no locks, no spinning, no searches; the paper inserts cells top-down under locks,
+// PAPER.md:146-150):
+//   c(s) = number of octree levels the keys of sorted cells s and s+1 share (c(-1) = c(n-1) = -1).
+//   Cell s starts an internal node at every level l with c(s-1) < l <= c(s), and it is a leaf
+//   child ("leaf entity") at level max(c(s-1), c(s)) + 1 (level 22 = member of a level-21 bucket).
+//   A node's children are exactly the level-(l+1) entities inside its range, so:
+//     * slot order   = all entities sorted by (level, s): the children of one node are contiguous
+//       and in octant order, children of consecutive canonical nodes are consecutive, root = slot 0;
+//     * canonical id = internal entities sorted by (level, s) = (level, prefix) order (T5);
+//     * the first child of node (l, s) is the entity (l+1, s) of the SAME cell, and the child count
+//       is the distance to the first child of the next canonical node.
+//   Both orders are stable counting sorts by level with variable fan-out per cell: one counting
+//   kernel (per-warp-chunk level histograms), one device scan, one assigning kernel that also
+//   gathers the cell data into its slot (a3 is fused into it).
 // Moments (Eq. 5; delta PAPER.md:54, 158) are reduced level by level from the
 // deepest level up, each node from its children in ascending octant order in fp64 (M-rules).
 #pragma once
@@ -21,7 +27,12 @@
 
 namespace bh {
 
-constexpr int kNumLevels = kMaxLevel + 1;   // levels 0..21
+constexpr int kNumLevels = kMaxLevel + 1;        // node levels 0..21
+constexpr int kSlotLevels = kMaxLevel + 2;       // entity levels 0..22
+constexpr int kTopoDigits = kSlotLevels + kNumLevels;   // histogram rows: entities per level, nodes per level
+constexpr int kTopoThreads = 256;
+constexpr int kTopoItems = 16;
+constexpr int kTopoChunk = 32 * kTopoItems;      // cells per warp chunk
 
 struct __align__(16) WalkAux {   // per slot, beside the float4 record (x, y, z, m)
     float size;      // node edge l (fp32 of L/2^level); +inf for a level-21 bucket; 0 for a leaf cell
@@ -30,66 +41,155 @@ struct __align__(16) WalkAux {   // per slot, beside the float4 record (x, y, z,
     u32 count;       // number of children (0: this slot is a leaf cell)
 };
 
-// ---- a3: permute the cells into sorted order ---------------------------------------------------
-// leaf64[s] = (x, y, z, m) fp64 of the cell in sorted slot s; leafrec[s] the same rounded to fp32;
-// slot_of[i] = sorted slot of original cell i.   84 B algorithmic per cell (+4 B slot_of).
-__global__ void __launch_bounds__(256)
-permute_kernel(const u32* __restrict__ idx, const double* __restrict__ x, const double* __restrict__ y,
-               const double* __restrict__ z, const double* __restrict__ m, i64 n,
-               double4* __restrict__ leaf64, float4* __restrict__ leafrec, u32* __restrict__ slot_of)
+inline i64 topo_chunks(i64 n) { return (n + kTopoChunk - 1) / kTopoChunk; }
+inline size_t topo_hist_elems(i64 n) { return (size_t)kTopoDigits * (size_t)topo_chunks(n); }
+
+// entity / internal-node level masks of a cell from c(s-1) = cp and c(s) = cs
+__device__ __forceinline__ void entity_masks(int cp, int cs, u32& imask, u32& emask)
 {
-    const i64 s = (i64)blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= n) return;
-    const u32 i = ld_stream(idx + s);
-    const double px = __ldg(x + i), py = __ldg(y + i), pz = __ldg(z + i), pm = __ldg(m + i);
-    double2* o = reinterpret_cast<double2*>(leaf64 + s);
-    st_stream(o, make_double2(px, py));
-    st_stream(o + 1, make_double2(pz, pm));
-    leafrec[s] = make_float4((float)px, (float)py, (float)pz, (float)pm);
-    slot_of[i] = (u32)s;
+    imask = cs > cp ? (((1u << (cs + 1)) - 1u) & ~((1u << (cp + 1)) - 1u)) : 0u;
+    emask = imask | (1u << ((cp > cs ? cp : cs) + 1));
 }
 
-// ---- a4.1: nodes starting at each sorted slot + per-level histogram ----------------------------
-__global__ void __launch_bounds__(256)
-node_count_kernel(const u64* __restrict__ keys, i64 n, u32* __restrict__ cnt, signed char* __restrict__ clev,
-                  u32* __restrict__ level_hist /* [kNumLevels] */)
+// ---- a4.1: c(s) per cell and the level histograms of every warp chunk -----------------------------
+// hist[d * nchunks + chunk]: d < kSlotLevels: entities of level d starting in the chunk;
+//                            d >= kSlotLevels: internal nodes of level d - kSlotLevels.
+// 8 B read + 1 B written per cell.
+__global__ void __launch_bounds__(kTopoThreads)
+topo_count_kernel(const u64* __restrict__ keys, i64 n, signed char* __restrict__ clev, u32* __restrict__ hist,
+                  i64 nchunks)
 {
-    __shared__ u32 h[kNumLevels];
-    if (threadIdx.x < kNumLevels) h[threadIdx.x] = 0;
-    __syncthreads();
-    const i64 stride = (i64)gridDim.x * blockDim.x;
-    for (i64 s = (i64)blockIdx.x * blockDim.x + threadIdx.x; s < n; s += stride) {
-        const u64 k = keys[s];
-        const int cprev = s > 0 ? common_levels(keys[s - 1], k) : -1;
-        const int cs = s + 1 < n ? common_levels(k, keys[s + 1]) : -1;
-        clev[s] = (signed char)cs;
-        const int c = cs > cprev ? cs - cprev : 0;
-        cnt[s] = (u32)c;
-        for (int l = cprev + 1; l <= cs; ++l) atomicAdd(&h[l], 1u);
+    const u32 lane = lane_id();
+    const i64 chunk = (i64)blockIdx.x * (kTopoThreads / 32) + (threadIdx.x >> 5);
+    if (chunk >= nchunks) return;
+    const i64 wbase = chunk * kTopoChunk;
+    u64 k[kTopoItems];
+    #pragma unroll
+    for (int i = 0; i < kTopoItems; ++i) {
+        const i64 s = wbase + 32 * i + lane;
+        k[i] = s < n ? ld_stream(keys + s) : 0ULL;
     }
-    __syncthreads();
-    if (threadIdx.x < kNumLevels && h[threadIdx.x]) atomicAdd(&level_hist[threadIdx.x], h[threadIdx.x]);
+    int carry = wbase > 0 ? common_levels(__ldg(keys + wbase - 1), __ldg(keys + wbase)) : -1;   // c(wbase - 1)
+    u32 cntT = 0, cntI = 0;                    // lane l: entities / internal nodes of level l in this chunk
+    #pragma unroll
+    for (int i = 0; i < kTopoItems; ++i) {
+        const i64 s = wbase + 32 * i + lane;
+        const bool valid = s < n;
+        u64 kn = __shfl_down_sync(0xffffffffu, k[i], 1);
+        if (i + 1 < kTopoItems) {                          // lane 31's successor: lane 0 of the next row
+            const u64 nx = __shfl_sync(0xffffffffu, k[i + 1], 0);
+            if (lane == 31) kn = nx;
+        } else if (lane == 31) {
+            kn = s + 1 < n ? __ldg(keys + s + 1) : 0ULL;
+        }
+        const int cs = (valid && s + 1 < n) ? common_levels(k[i], kn) : -1;
+        int cp = __shfl_up_sync(0xffffffffu, cs, 1);
+        if (lane == 0) cp = carry;
+        carry = __shfl_sync(0xffffffffu, cs, 31);
+        u32 imask = 0u, emask = 0u;
+        if (valid) {
+            clev[s] = (signed char)cs;
+            entity_masks(cp, cs, imask, emask);
+        }
+        u32 U = __reduce_or_sync(0xffffffffu, emask);
+        while (U) {
+            const int l = __ffs(U) - 1;
+            U &= U - 1u;
+            const u32 bal = __ballot_sync(0xffffffffu, (emask >> l) & 1u);
+            const u32 balI = __ballot_sync(0xffffffffu, (imask >> l) & 1u);
+            if ((int)lane == l) { cntT += __popc(bal); cntI += __popc(balI); }
+        }
+    }
+    if (lane < (u32)kSlotLevels) hist[(i64)lane * nchunks + chunk] = cntT;
+    if (lane < (u32)kNumLevels) hist[(i64)(kSlotLevels + lane) * nchunks + chunk] = cntI;
 }
 
-// ---- a4.2: emit the nodes in pre-order: (level as sort key, pre-order id as payload, lo) ---------
-__global__ void __launch_bounds__(256)
-node_emit_kernel(const signed char* __restrict__ clev, const u32* __restrict__ pre_base, i64 n,
-                 u64* __restrict__ nkey, u32* __restrict__ npre, u32* __restrict__ nlo)
+// row starts of the scanned histogram (+ the grand total) for the host: out[d] = scanned[d * nchunks]
+__global__ void topo_totals_kernel(const u32* __restrict__ scanned, i64 nchunks, const u32* __restrict__ total,
+                                   u32* __restrict__ out /* [kTopoDigits + 1] */)
 {
-    const i64 s = (i64)blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= n) return;
-    const int cs = clev[s];
-    const int cprev = s > 0 ? (int)clev[s - 1] : -1;
-    if (cs <= cprev) return;
-    u32 p = pre_base[s];
-    for (int l = cprev + 1; l <= cs; ++l, ++p) {
-        nkey[p] = (u64)l;
-        npre[p] = p;
-        nlo[p] = (u32)s;
+    const int d = threadIdx.x;
+    if (d < kTopoDigits) out[d] = scanned[(i64)d * nchunks];
+    else if (d == kTopoDigits) out[d] = *total;
+}
+
+// ---- a4.2 + a3: number every entity, link the nodes, move every cell into its slot ------------------
+// `scanned` = exclusive scan of the count kernel's histogram (row-major over [digit][chunk]), so
+// scanned[l][chunk] is the slot of the chunk's first level-l entity and scanned[23 + l][chunk] - nslots
+// the canonical id of its first level-l node.  Per cell: 4 B idx + 1 B c + 32 B gathered; written
+// 4 B slot + 32 B fp64 record + 16 B fp32 record + 16 B aux; per node 12 B.
+__global__ void __launch_bounds__(kTopoThreads)
+topo_assign_kernel(const signed char* __restrict__ clev, i64 n, const u32* __restrict__ idx,
+                   const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
+                   const double* __restrict__ m, const u32* __restrict__ scanned, i64 nchunks, u32 nslots,
+                   u32* __restrict__ leaf_slot, u32* __restrict__ node_slot, u32* __restrict__ nfirst,
+                   u32* __restrict__ nlo, double4* __restrict__ rec64, float4* __restrict__ rec,
+                   WalkAux* __restrict__ aux)
+{
+    const u32 lane = lane_id();
+    const u32 lt = lanemask_lt();
+    const i64 chunk = (i64)blockIdx.x * (kTopoThreads / 32) + (threadIdx.x >> 5);
+    if (chunk >= nchunks) return;
+    const i64 wbase = chunk * kTopoChunk;
+    // lane l: slot of the next level-l entity / canonical id of the next level-l node
+    u32 cntT = lane < (u32)kSlotLevels ? scanned[(i64)lane * nchunks + chunk] : 0u;
+    u32 cntI = lane < (u32)kNumLevels ? scanned[(i64)(kSlotLevels + lane) * nchunks + chunk] - nslots : 0u;
+    int carry = wbase > 0 ? (int)clev[wbase - 1] : -1;
+    const uint4 leaf_aux = make_uint4(0u, 0u, 0u, 0u);
+    #pragma unroll 2
+    for (int i = 0; i < kTopoItems; ++i) {
+        if (wbase + 32 * i >= n) break;
+        const i64 s = wbase + 32 * i + lane;
+        const bool valid = s < n;
+        double px = 0.0, py = 0.0, pz = 0.0, pm = 0.0;
+        int cs = -1;
+        if (valid) {
+            const u32 o = ld_stream(idx + s);
+            px = __ldg(x + o); py = __ldg(y + o); pz = __ldg(z + o); pm = __ldg(m + o);
+            cs = (int)clev[s];
+        }
+        int cp = __shfl_up_sync(0xffffffffu, cs, 1);
+        if (lane == 0) cp = carry;
+        carry = __shfl_sync(0xffffffffu, cs, 31);
+        u32 imask = 0u, emask = 0u;
+        if (valid) entity_masks(cp, cs, imask, emask);
+        u32 U = __reduce_or_sync(0xffffffffu, emask);
+        u32 pend = 0xffffffffu, myslot = 0u;
+        while (U) {                                   // ascending levels
+            const int l = __ffs(U) - 1;
+            U &= U - 1u;
+            const bool has = (emask >> l) & 1u, isint = (imask >> l) & 1u;
+            const u32 bal = __ballot_sync(0xffffffffu, has);
+            const u32 balI = __ballot_sync(0xffffffffu, isint);
+            const u32 baseT = __shfl_sync(0xffffffffu, cntT, l);
+            const u32 baseI = __shfl_sync(0xffffffffu, cntI, l);
+            if ((int)lane == l) { cntT += __popc(bal); cntI += __popc(balI); }
+            if (has) {
+                const u32 slot = baseT + __popc(bal & lt);
+                if (pend != 0xffffffffu) nfirst[pend] = slot;       // entity (l, s) is the first child of (l-1, s)
+                if (isint) {
+                    const u32 b = baseI + __popc(balI & lt);
+                    node_slot[b] = slot;
+                    nlo[b] = (u32)s;
+                    pend = b;
+                } else {
+                    myslot = slot;
+                    pend = 0xffffffffu;
+                }
+            }
+        }
+        if (valid) {
+            leaf_slot[s] = myslot;
+            double2* o64 = reinterpret_cast<double2*>(rec64 + myslot);
+            o64[0] = make_double2(px, py);
+            o64[1] = make_double2(pz, pm);
+            rec[myslot] = make_float4((float)px, (float)py, (float)pz, (float)pm);
+            reinterpret_cast<uint4*>(aux)[myslot] = leaf_aux;
+        }
     }
 }
 
-// first index in [a, hi) whose key is >= limit (hi if none); gallops from a (ranges are short on average)
+// first index in [a, hi) whose key is >= limit (hi if none); gallops from a
 __device__ __forceinline__ i64 gallop_lower_bound(const u64* __restrict__ keys, i64 a, i64 hi, u64 limit)
 {
     if (a >= hi || keys[a] >= limit) return a;
@@ -104,93 +204,6 @@ __device__ __forceinline__ i64 gallop_lower_bound(const u64* __restrict__ keys, 
     return up;
 }
 
-// ---- a4.3: per node (canonical order b): range end, child boundaries, child count ---------------
-__global__ void __launch_bounds__(256)
-node_children_kernel(const u64* __restrict__ keys, i64 n, const u64* __restrict__ bkey,
-                     const u32* __restrict__ bpre, const u32* __restrict__ nlo, i64 nn,
-                     u32* __restrict__ bfs_of, u32* __restrict__ blo, u32* __restrict__ bhi,
-                     u32* __restrict__ nchild, u32* __restrict__ cstart /* [8*nn] */,
-                     u32* __restrict__ max_bucket)
-{
-    const i64 b = (i64)blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= nn) return;
-    const int level = (int)bkey[b];
-    const u32 p = bpre[b];
-    const i64 lo = nlo[p];
-    bfs_of[p] = (u32)b;
-    i64 hi;
-    if (level == 0) hi = n;
-    else {
-        const int sh = 3 * (kMaxLevel - level);
-        const u64 limit = ((keys[lo] >> sh) + 1ULL) << sh;
-        hi = gallop_lower_bound(keys, lo + 1, n, limit);
-    }
-    blo[b] = (u32)lo;
-    bhi[b] = (u32)hi;
-    if (level == kMaxLevel) {             // bucket: its cells are its children
-        nchild[b] = (u32)(hi - lo);
-        atomicMax(max_bucket, (u32)(hi - lo));
-        return;
-    }
-    const int sh1 = 3 * (kMaxLevel - level - 1);
-    int j = 0;
-    i64 a = lo;
-    while (a < hi) {
-        cstart[8 * b + j] = (u32)a;
-        ++j;
-        const u64 limit = ((keys[a] >> sh1) + 1ULL) << sh1;
-        a = gallop_lower_bound(keys, a + 1, hi, limit);
-    }
-    nchild[b] = (u32)j;
-}
-
-// ---- a4.4: fill the slots: leaf-cell records, links to internal children --------------------------
-// 8 threads per node.  slot_src[slot] >= 0: sorted cell index;  < 0: ~(canonical id of the internal child)
-__global__ void __launch_bounds__(256)
-slot_fill_kernel(const u64* __restrict__ bkey, const u32* __restrict__ bpre, const u32* __restrict__ blo,
-                 const u32* __restrict__ bhi, const u32* __restrict__ nchild, const u32* __restrict__ cstart,
-                 const u32* __restrict__ child_base, const u32* __restrict__ pre_base,
-                 const u32* __restrict__ bfs_of, i64 nn, const float4* __restrict__ leafrec,
-                 int* __restrict__ slot_src, u32* __restrict__ node_slot, float4* __restrict__ rec,
-                 WalkAux* __restrict__ aux)
-{
-    const i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x;
-    const i64 b = t >> 3;
-    const int j0 = (int)(t & 7);
-    if (b >= nn) return;
-    const int level = (int)bkey[b];
-    const u32 cnt = nchild[b];
-    const u32 first = 1u + child_base[b];
-    const u32 lo = blo[b], hi = bhi[b];
-    if (b == 0 && j0 == 0) node_slot[0] = 0u;          // root record lives in slot 0
-    WalkAux leaf_aux; leaf_aux.size = 0.f; leaf_aux.delta = 0.f; leaf_aux.first = 0u; leaf_aux.count = 0u;
-    if (level == kMaxLevel) {
-        for (u32 j = j0; j < cnt; j += 8) {
-            const u32 a = lo + j, slot = first + j;
-            slot_src[slot] = (int)a;
-            rec[slot] = leafrec[a];
-            aux[slot] = leaf_aux;
-        }
-        return;
-    }
-    if ((u32)j0 >= cnt) return;
-    const u32 a = cstart[8 * b + j0];
-    const u32 e = (u32)j0 + 1 < cnt ? cstart[8 * b + j0 + 1] : hi;
-    const u32 slot = first + j0;
-    if (e - a == 1) {
-        slot_src[slot] = (int)a;
-        rec[slot] = leafrec[a];
-        aux[slot] = leaf_aux;
-    } else {
-        // pre-order id of the child node (level+1, a): this node's id + 1 if it starts at lo, else
-        // the first node starting at a (there c(a-1) == level exactly)
-        const u32 pre = (a == lo) ? bpre[b] + 1u : pre_base[a];
-        const u32 cb = bfs_of[pre];
-        slot_src[slot] = ~(int)cb;
-        node_slot[cb] = slot;
-    }
-}
-
 // ---- a5: moments of the nodes [b0, b1) of one level from their children ---------------------------
 __device__ __forceinline__ u32 compact3(u64 v)   // inverse of the key bit-spread: every third bit
 {
@@ -203,21 +216,21 @@ __device__ __forceinline__ u32 compact3(u64 v)   // inverse of the key bit-sprea
     return (u32)v;
 }
 
+// Node b of level `level`: children = slots [nfirst[b], nfirst[b+1]) (the last node of the level ends at
+// slot_end, the end of the level-(level+1) slots).  Reads 32 B per child, writes 80 B per node.
 __global__ void __launch_bounds__(128)
-moments_kernel(i64 b0, i64 b1, int level, const u64* __restrict__ keys, const u32* __restrict__ blo,
-               const u32* __restrict__ nchild, const u32* __restrict__ child_base,
-               const int* __restrict__ slot_src, const u32* __restrict__ node_slot,
-               const double4* __restrict__ leaf64, double4* __restrict__ mom, double* __restrict__ delta64,
-               float4* __restrict__ rec, WalkAux* __restrict__ aux, double x0, double y0, double z0, double L)
+moments_kernel(i64 b0, i64 b1, int level, u32 slot_end, const u64* __restrict__ keys,
+               const u32* __restrict__ nlo, const u32* __restrict__ nfirst, const u32* __restrict__ node_slot,
+               double4* __restrict__ rec64, double* __restrict__ delta64, float4* __restrict__ rec,
+               WalkAux* __restrict__ aux, u32* __restrict__ max_bucket, double x0, double y0, double z0, double L)
 {
     const i64 b = b0 + (i64)blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= b1) return;
-    const u32 cnt = nchild[b];
-    const u32 first = 1u + child_base[b];
+    const u32 first = nfirst[b];
+    const u32 cnt = (b + 1 < b1 ? nfirst[b + 1] : slot_end) - first;
     double M = 0.0, Sx = 0.0, Sy = 0.0, Sz = 0.0;
     for (u32 j = 0; j < cnt; ++j) {       // ascending octant order (M-rule 1); no fma contraction
-        const int src = slot_src[first + j];
-        const double2* p = reinterpret_cast<const double2*>(src >= 0 ? leaf64 + src : mom + (~src));
+        const double2* p = reinterpret_cast<const double2*>(rec64 + first + j);
         const double2 xy = p[0], zm = p[1];
         M = __dadd_rn(M, zm.y);
         Sx = __dadd_rn(Sx, __dmul_rn(zm.y, xy.x));
@@ -225,7 +238,7 @@ moments_kernel(i64 b0, i64 b1, int level, const u64* __restrict__ keys, const u3
         Sz = __dadd_rn(Sz, __dmul_rn(zm.y, zm.x));
     }
     const double size = ldexp(L, -level);
-    const u64 prefix = level == 0 ? 0ULL : keys[blo[b]] >> (3 * (kMaxLevel - level));
+    const u64 prefix = level == 0 ? 0ULL : keys[nlo[b]] >> (3 * (kMaxLevel - level));
     const double cx = __dadd_rn(x0, __dmul_rn((double)compact3(prefix) + 0.5, size));
     const double cy = __dadd_rn(y0, __dmul_rn((double)compact3(prefix >> 1) + 0.5, size));
     const double cz = __dadd_rn(z0, __dmul_rn((double)compact3(prefix >> 2) + 0.5, size));
@@ -237,11 +250,11 @@ moments_kernel(i64 b0, i64 b1, int level, const u64* __restrict__ keys, const u3
     } else {                               // M-rule 2: zero-mass node sits at its geometric centre
         Rx = cx; Ry = cy; Rz = cz; del = 0.0;
     }
-    double2* o = reinterpret_cast<double2*>(mom + b);
+    const u32 slot = node_slot[b];
+    double2* o = reinterpret_cast<double2*>(rec64 + slot);
     o[0] = make_double2(Rx, Ry);
     o[1] = make_double2(Rz, M);
     delta64[b] = del;
-    const u32 slot = node_slot[b];
     rec[slot] = make_float4((float)Rx, (float)Ry, (float)Rz, (float)M);
     WalkAux a;
     a.size = level == kMaxLevel ? __int_as_float(0x7f800000) : (float)size;
@@ -249,30 +262,56 @@ moments_kernel(i64 b0, i64 b1, int level, const u64* __restrict__ keys, const u3
     a.first = first;
     a.count = cnt;
     aux[slot] = a;
+    if (level == kMaxLevel) atomicMax(max_bucket, cnt);
 }
 
-// ---- export (parity only): prefix of each node in canonical order --------------------------------
+struct TopoLevels {               // host-computed from the scanned histogram
+    u32 node_base[kNumLevels + 1];    // canonical id of the first node of each level; [22] = n_nodes
+    u32 slot_base[kSlotLevels + 1];   // first slot of each entity level; [23] = n_slots
+};
+
+// ---- export (parity only): the nodes in canonical order ------------------------------------------
 __global__ void __launch_bounds__(256)
-export_nodes_kernel(i64 nn, const u64* __restrict__ keys, const u64* __restrict__ bkey,
-                    const u32* __restrict__ blo, const u32* __restrict__ bhi, const u32* __restrict__ nchild,
-                    const double4* __restrict__ mom, const double* __restrict__ delta64,
+export_nodes_kernel(i64 nn, i64 n, const TopoLevels lv, const u64* __restrict__ keys, const u32* __restrict__ nlo,
+                    const u32* __restrict__ nfirst, const u32* __restrict__ node_slot,
+                    const double4* __restrict__ rec64, const double* __restrict__ delta64,
                     int* level, u64* prefix, i64* lo, i64* hi, int* nch, double* M, double* Rx, double* Ry,
                     double* Rz, double* delta)
 {
     const i64 b = (i64)blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= nn) return;
-    const int l = (int)bkey[b];
+    int l = 0;
+    while (l + 1 < kNumLevels && (i64)lv.node_base[l + 1] <= b) ++l;
+    const i64 s = nlo[b];
     if (level) level[b] = l;
-    if (prefix) prefix[b] = l == 0 ? 0ULL : keys[blo[b]] >> (3 * (kMaxLevel - l));
-    if (lo) lo[b] = blo[b];
-    if (hi) hi[b] = bhi[b];
-    if (nch) nch[b] = (int)nchild[b];
-    const double4 q = mom[b];
+    if (prefix) prefix[b] = l == 0 ? 0ULL : keys[s] >> (3 * (kMaxLevel - l));
+    if (lo) lo[b] = s;
+    if (hi) {
+        if (l == 0) hi[b] = n;
+        else {
+            const int sh = 3 * (kMaxLevel - l);
+            hi[b] = gallop_lower_bound(keys, s + 1, n, ((keys[s] >> sh) + 1ULL) << sh);
+        }
+    }
+    if (nch) nch[b] = (int)((b + 1 < (i64)lv.node_base[l + 1] ? nfirst[b + 1] : lv.slot_base[l + 2]) - nfirst[b]);
+    const double4 q = rec64[node_slot[b]];
     if (Rx) Rx[b] = q.x;
     if (Ry) Ry[b] = q.y;
     if (Rz) Rz[b] = q.z;
     if (M) M[b] = q.w;
     if (delta) delta[b] = delta64[b];
+}
+
+// ---- bh_potential_direct's own copies (built on its first call after a build, not on the hot path) --
+__global__ void __launch_bounds__(256)
+direct_prepare_kernel(const u32* __restrict__ idx, const u32* __restrict__ leaf_slot,
+                      const double4* __restrict__ rec64, i64 n, double4* __restrict__ leaf64,
+                      u32* __restrict__ slot_of)
+{
+    const i64 s = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    leaf64[s] = rec64[leaf_slot[s]];
+    slot_of[idx[s]] = (u32)s;
 }
 
 }  // namespace bh

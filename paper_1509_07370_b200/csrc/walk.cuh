@@ -45,7 +45,7 @@ constexpr float kTinyD2 = 1.0e-36f;           // keeps d^2 of the unchecked list
 struct WalkParams {
     const float4* rec;        // [n_slots] (x, y, z, m) of every node / leaf-cell slot
     const WalkAux* aux;       // [n_slots]
-    const float4* leafrec;    // [n] sorted cells (targets)
+    const u32* leaf_slot;     // [n] slot of sorted cell s (the targets are read from rec)
     const u32* idx;           // [n] original index of sorted slot
     double* phi;              // [n] original order
     uint4* gcount;            // [ngroups] {accepted, leaf, opened, exact-tested}
@@ -242,8 +242,8 @@ walk_pair_kernel(const WalkParams P)
     const int ntB = hasB ? (int)min((i64)32, P.n - gB * 32) : 0;
     const bool liveA = (int)lane < ntA, liveB = (int)lane < ntB;
     const i64 sA = gA * 32 + lane, sB = gB * 32 + lane;
-    const float4 tA = __ldg(P.leafrec + (liveA ? sA : gA * 32));
-    const float4 tB = __ldg(P.leafrec + (liveB ? sB : (hasB ? gB * 32 : gA * 32)));
+    const float4 tA = __ldg(P.rec + __ldg(P.leaf_slot + (liveA ? sA : gA * 32)));
+    const float4 tB = __ldg(P.rec + __ldg(P.leaf_slot + (liveB ? sB : (hasB ? gB * 32 : gA * 32))));
     Box2 box;                                         // bounding boxes of the live targets of A and B
     box.xl = make_float2(warp_min(tA.x), warp_min(tB.x)); box.xh = make_float2(warp_max(tA.x), warp_max(tB.x));
     box.yl = make_float2(warp_min(tA.y), warp_min(tB.y)); box.yh = make_float2(warp_max(tA.y), warp_max(tB.y));
@@ -429,7 +429,7 @@ walk_single_kernel(const WalkParams P)
 {
     const i64 s = (i64)blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= P.n) return;
-    const float4 tp = __ldg(P.leafrec + s);
+    const float4 tp = __ldg(P.rec + __ldg(P.leaf_slot + s));
     u32 st_first[kSingleStack], st_count[kSingleStack];
     int sp = 0;
     if (P.n >= 2) { st_first[0] = 0u; st_count[0] = 1u; sp = 1; }
