@@ -98,7 +98,7 @@ class ClockSampler:
 def build_bytes_per_cell(n, n_nodes, sort_passes):
     """Algorithmic HBM bytes of bh_build per cell."""
     keys = 36.0
-    sort = sort_passes * (8.0 + 24.0)                # classic pass: histogram read + read/write of 12 B
+    sort = (8.0 + 24.0 * sort_passes) if sort_passes else 0.0   # one histogram read + read/write of 12 B per pass
     permute = 84.0 + 4.0
     topo = 8.0 + 5.0 + (n_nodes / n) * 24.0
     mom = 32.0 + (n_nodes / n) * 72.0
@@ -274,11 +274,11 @@ def run_ours(args):
         "walk_interactions_per_s": world * inter / t_walk,
         "interactions_per_target": inter / n,
         "ms_build": t_build * 1e3, "ms_walk": t_walk * 1e3,
-        "build_passes_ms": {"keys": st.ms_keys, "sort": st.ms_sort, "permute": st.ms_permute,
-                            "topology": st.ms_topology, "moments": st.ms_moments},
+        "build_passes_ms": {"keys": st.ms_keys, "sort": st.ms_sort, "count": st.ms_count,
+                            "assign_permute": st.ms_assign, "moments": st.ms_moments},
         "tree": {"n_nodes": st.n_nodes, "depth": st.depth, "sort_passes": st.sort_passes,
                  "exact_tests_per_group": st.n_exact_tests / ((n + 31) // 32)},
-        "roofline": {"bound": "alu", "kernel": "walk_group32_kernel", "achieved": walk_tflops, "peak": fp32_peak_tflops,
+        "roofline": {"bound": "alu", "kernel": "walk_pair_kernel<false>", "achieved": walk_tflops, "peak": fp32_peak_tflops,
                      "unit": "TFLOP/s", "frac": walk_tflops / fp32_peak_tflops, "traffic": None,
                      "peak_source": "nominal FP32: %d SMs x 128 lanes x 2 x %.0f MHz (sm_max_mhz, MEASURED_PEAKS.json %s); "
                                     "13 flops/interaction" % (st_sms(local), sm_max_mhz, peak_src),

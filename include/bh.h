@@ -40,7 +40,7 @@ typedef struct bh_ctx bh_ctx;
 #define BH_ERR_NOT_BUILT   -2   /* bh_potential / export / direct before a successful bh_build */
 #define BH_ERR_CUDA        -3   /* a CUDA runtime call failed; see bh_last_cuda_error() */
 #define BH_ERR_OOM         -4   /* device or host allocation failed */
-#define BH_ERR_TOO_LARGE   -5   /* bh_potential_direct over all n with n above BH_DIRECT_ALL_MAX; or n + nodes >= 2^32 */
+#define BH_ERR_TOO_LARGE   -5   /* bh_potential_direct over all n with n above BH_DIRECT_ALL_MAX; n + nodes >= 2^32; n >= 2^30 */
 
 /* ---- options (bh_set_option) ---------------------------------------------------------------- */
 #define BH_OPT_MAC    1   /* opening criterion */
@@ -67,7 +67,9 @@ typedef struct bh_stats {
     int64_t n_exact_tests;     /* last walk: nodes whose vote needed the per-target test (diagnostic)  */
     double  interactions;      /* last walk: sum over TARGETS of (accepted + leaf) of their group     */
     /* device time in ms of the passes of the last bh_build / bh_potential (CUDA events) */
-    float ms_keys, ms_sort, ms_permute, ms_topology, ms_moments, ms_build_total;
+    /* device ms of the last build: keys (a1), sort (a2), count = c(s) + level histograms + scan (a4),
+     * assign = entity numbering + cells moved into their slots (a4 + a3), moments (a5), whole build */
+    float ms_keys, ms_sort, ms_count, ms_assign, ms_moments, ms_build_total;
     float ms_walk;
     int32_t launches_build;    /* kernels the last bh_build launched                                   */
     int32_t launches_walk;     /* kernels the last bh_potential launched                               */

@@ -24,8 +24,8 @@ class Stats(C.Structure):
                 ("sort_passes", C.c_int32), ("n_clamped", C.c_int64), ("max_bucket", C.c_int64),
                 ("n_accepted", C.c_int64), ("n_leaf", C.c_int64), ("n_opened", C.c_int64),
                 ("n_exact_tests", C.c_int64), ("interactions", C.c_double),
-                ("ms_keys", C.c_float), ("ms_sort", C.c_float), ("ms_permute", C.c_float),
-                ("ms_topology", C.c_float), ("ms_moments", C.c_float), ("ms_build_total", C.c_float),
+                ("ms_keys", C.c_float), ("ms_sort", C.c_float), ("ms_count", C.c_float),
+                ("ms_assign", C.c_float), ("ms_moments", C.c_float), ("ms_build_total", C.c_float),
                 ("ms_walk", C.c_float), ("launches_build", C.c_int32), ("launches_walk", C.c_int32)]
 
     def as_dict(self):

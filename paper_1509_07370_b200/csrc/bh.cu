@@ -168,7 +168,7 @@ int bh_create(bh_ctx** out, int device, void* cuda_stream)
         if (rc) break;
         if ((e = ctx->scalars.ensure(sizeof(DeviceScalars))) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaMalloc"); break; }
         if ((e = cudaMallocHost(&ctx->h_scalars, sizeof(DeviceScalars))) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaMallocHost"); break; }
-        if ((e = cudaFuncSetAttribute(radix_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        if ((e = cudaFuncSetAttribute(radix_onesweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       (int)sizeof(SortSmem))) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(sort)"); break; }
         if ((e = cudaFuncSetAttribute(walk_pair_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       227 * 1024)) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(walk)"); break; }
@@ -208,6 +208,7 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
              const double cube[4])
 {
     if (!ctx || !x || !y || !z || !m || !cube) return BH_ERR_INVALID_ARG;
+    if (n >= (1LL << 30) && n < 2147483648LL) return BH_ERR_TOO_LARGE;   // 30-bit tile counters of the sort
     if (n <= 0 || n >= 2147483648LL || !(cube[3] > 0.0) || !isfinite(cube[0]) || !isfinite(cube[1]) ||
         !isfinite(cube[2]) || !isfinite(cube[3]))
         return BH_ERR_INVALID_ARG;
@@ -264,17 +265,12 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
     ctx->sort_passes = plan.npasses;
 
     // ---- a2: radix sort of (key, index) ----
-    u64* k0 = ctx->keysA.as<u64>(); u64* k1 = ctx->keysB.as<u64>();
-    u32* v0 = ctx->idxA.as<u32>();  u32* v1 = ctx->idxB.as<u32>();
-    for (int p = 0; p < plan.npasses; ++p) {
-        BH_CUDA(radix_pass(k0, v0, k1, v1, n, plan.shift[p], plan.mask[p], ctx->hist.as<u32>(),
-                           ctx->scan_scratch.as<u32>(), st));
-        ctx->launches_build += 5;   // histogram + 3 scan kernels + scatter
-        u64* tk = k0; k0 = k1; k1 = tk;
-        u32* tv = v0; v0 = v1; v1 = tv;
-    }
-    ctx->keys = k0;
-    ctx->idx = v0;
+    BH_CUDA(radix_sort_pairs(ctx->keysA.as<u64>(), ctx->idxA.as<u32>(), ctx->keysB.as<u64>(), ctx->idxB.as<u32>(), n,
+                             plan, ctx->hist.as<u32>(), persistent_grid(ctx, 8), st));
+    ctx->launches_build += plan.npasses ? 1 + plan.npasses : 0;   // histogram + one kernel per pass
+    const bool odd = plan.npasses & 1;
+    ctx->keys = odd ? ctx->keysB.as<u64>() : ctx->keysA.as<u64>();
+    ctx->idx = odd ? ctx->idxB.as<u32>() : ctx->idxA.as<u32>();
     BH_CUDA(cudaEventRecord(ctx->ev[EV_SORT], st));
 
     // ---- a4: topology (a3, the permutation of the cell data, is fused into the assigning kernel) ----
@@ -326,16 +322,33 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
         ctx->launches_build += 1 + 3 + 1 + 1;   // count, scan, totals, assign
         BH_CUDA(cudaEventRecord(ctx->ev[EV_TOPO], st));
 
-        // ---- a5: moments, deepest level first ----
-        for (int l = ctx->maxlevel; l >= 0; --l) {
-            const i64 b0 = ctx->lv.node_base[l], b1 = ctx->lv.node_base[l + 1];
-            if (b1 == b0) continue;
-            moments_kernel<<<blocks_for(b1 - b0, 128), 128, 0, st>>>(
-                b0, b1, l, ctx->lv.slot_base[l + 2], ctx->keys, ctx->nlo.as<u32>(), ctx->nfirst.as<u32>(),
-                ctx->node_slot.as<u32>(), ctx->rec64.as<double4>(), ctx->delta64.as<double>(),
-                ctx->rec.as<float4>(), ctx->aux.as<WalkAux>(), &ds->max_bucket, cube[0], cube[1], cube[2], cube[3]);
-            BH_CUDA(cudaGetLastError());
-            ctx->launches_build += 1;
+        // ---- a5: moments, deepest level first; runs of small levels share one single-block launch ----
+        MomentArgs MA;
+        MA.keys = ctx->keys; MA.nlo = ctx->nlo.as<u32>(); MA.nfirst = ctx->nfirst.as<u32>();
+        MA.node_slot = ctx->node_slot.as<u32>(); MA.rec64 = ctx->rec64.as<double4>();
+        MA.delta64 = ctx->delta64.as<double>(); MA.rec = ctx->rec.as<float4>(); MA.aux = ctx->aux.as<WalkAux>();
+        MA.max_bucket = &ds->max_bucket; MA.x0 = cube[0]; MA.y0 = cube[1]; MA.z0 = cube[2]; MA.L = cube[3];
+        SmallLevels sl;
+        sl.nlev = 0;
+        for (int l = ctx->maxlevel; l >= -1; --l) {
+            const i64 b0 = l >= 0 ? ctx->lv.node_base[l] : 0, b1 = l >= 0 ? ctx->lv.node_base[l + 1] : 0;
+            const bool small = l >= 0 && b1 - b0 <= kSmallLevelNodes;
+            if ((!small || l < 0) && sl.nlev > 0) {          // flush the pending run of small levels
+                moments_small_kernel<<<1, kMomSmallThreads, 0, st>>>(sl, MA);
+                BH_CUDA(cudaGetLastError());
+                ctx->launches_build += 1;
+                sl.nlev = 0;
+            }
+            if (l < 0 || b1 == b0) continue;
+            if (small) {
+                sl.level[sl.nlev] = l; sl.b0[sl.nlev] = (u32)b0; sl.b1[sl.nlev] = (u32)b1;
+                sl.slot_end[sl.nlev] = ctx->lv.slot_base[l + 2];
+                ++sl.nlev;
+            } else {
+                moments_kernel<<<blocks_for(b1 - b0, 128), 128, 0, st>>>(b0, b1, l, ctx->lv.slot_base[l + 2], MA);
+                BH_CUDA(cudaGetLastError());
+                ctx->launches_build += 1;
+            }
         }
     } else {
         BH_CUDA(cudaEventRecord(ctx->ev[EV_PERM], st));
@@ -574,8 +587,8 @@ int bh_get_stats(bh_ctx* ctx, bh_stats* out)
     if (ctx->ev_build) {
         cudaEventElapsedTime(&out->ms_keys, ctx->ev[EV_B0], ctx->ev[EV_KEYS]);
         cudaEventElapsedTime(&out->ms_sort, ctx->ev[EV_KEYS], ctx->ev[EV_SORT]);
-        cudaEventElapsedTime(&out->ms_permute, ctx->ev[EV_SORT], ctx->ev[EV_PERM]);
-        cudaEventElapsedTime(&out->ms_topology, ctx->ev[EV_PERM], ctx->ev[EV_TOPO]);
+        cudaEventElapsedTime(&out->ms_count, ctx->ev[EV_SORT], ctx->ev[EV_PERM]);
+        cudaEventElapsedTime(&out->ms_assign, ctx->ev[EV_PERM], ctx->ev[EV_TOPO]);
         cudaEventElapsedTime(&out->ms_moments, ctx->ev[EV_TOPO], ctx->ev[EV_MOM]);
         cudaEventElapsedTime(&out->ms_build_total, ctx->ev[EV_B0], ctx->ev[EV_MOM]);
     }

@@ -1,8 +1,11 @@
 // sort.cuh -- step a2: stable least-significant-digit radix sort of (u64 key, u32 value) pairs,
-// 8-bit digits, one pass = tile histograms -> device scan -> ranked scatter.
-// Stable, so ties keep ascending original index (DESIGN.md S-rule: ascending (key, index)).
+// 8-bit digits.  Stable, so ties keep ascending original index (DESIGN.md S-rule: ascending (key, index)).
 // Only digits that cover varying key bits are sorted (the host picks the passes from the OR/AND of
-// all keys).  HBM-bound: per pass 8 B (histogram read) + 12 B read + 12 B written per pair.
+// all keys).  One histogram kernel counts every pass's digits in a single read of the keys; each pass
+// is then ONE kernel: a tile ranks its pairs, publishes its digit counts and obtains its global
+// offsets by decoupled look-back over the preceding tiles (tiles are handed out by a ticket counter,
+// so a tile only ever waits for tiles that are already running).  HBM-bound: 8 B for the
+// histograms + 24 B (12 B read, 12 B written) per pass and pair.
 #pragma once
 #include "common.cuh"
 #include "scan.cuh"
@@ -13,46 +16,92 @@ constexpr int kSortThreads = 256;
 constexpr int kSortItems = 16;
 constexpr int kSortTile = kSortThreads * kSortItems;   // 4096 pairs per CTA
 constexpr int kRadix = 256;
+constexpr int kMaxPasses = 8;
+constexpr u32 kFlagAgg = 1u << 30, kFlagPrefix = 2u << 30, kValMask = (1u << 30) - 1u;   // tile status words
 
-// per-tile digit histogram, written digit-major: hist[d * ntiles + tile]
-__global__ void __launch_bounds__(kSortThreads)
-radix_hist_kernel(const u64* __restrict__ keys, i64 n, int shift, u32 mask, u32* __restrict__ hist, int ntiles)
+// lanes of the warp whose 8-bit digit equals this lane's: eight ballots, independent of how many
+// distinct digits the warp holds (match.any slows down with every distinct value)
+__device__ __forceinline__ u32 digit_peers(u32 d)
 {
-    __shared__ u32 h[kRadix];
-    h[threadIdx.x] = 0;
+    u32 peers = 0xffffffffu;
+    #pragma unroll
+    for (int b = 0; b < 8; ++b) {
+        const bool bit = (d >> b) & 1u;
+        const u32 bal = __ballot_sync(0xffffffffu, bit);
+        peers &= bit ? bal : ~bal;
+    }
+    return peers;
+}
+
+struct SortPlan {
+    int npasses;
+    int shift[kMaxPasses];
+    u32 mask[kMaxPasses];
+};
+
+// ghist[p * pass_stride + d] = number of keys whose digit of pass p is d
+__global__ void __launch_bounds__(kSortThreads)
+radix_hist_strided_kernel(const u64* __restrict__ keys, i64 n, const SortPlan plan, u32* __restrict__ ghist,
+                          u32 pass_stride)
+{
+    __shared__ u32 h[kMaxPasses * kRadix];
+    for (int i = threadIdx.x; i < plan.npasses * kRadix; i += kSortThreads) h[i] = 0;
     __syncthreads();
-    const i64 base = (i64)blockIdx.x * kSortTile;
-    #pragma unroll 4
-    for (int i = 0; i < kSortItems; ++i) {
-        const i64 e = base + (i64)i * kSortThreads + threadIdx.x;
-        if (e < n) atomicAdd(&h[(u32)(ld_stream(keys + e) >> shift) & mask], 1u);
+    constexpr int kRows = 4;                              // rows of 32 keys a warp keeps in flight
+    const i64 stride = (i64)gridDim.x * kSortThreads * kRows;
+    const u32 lane = threadIdx.x & 31;
+    for (i64 wb = ((i64)blockIdx.x * kSortThreads + (threadIdx.x & ~31)) * kRows; wb < n; wb += stride) {   // warp-uniform
+        u64 k[kRows];
+        #pragma unroll
+        for (int r = 0; r < kRows; ++r) k[r] = wb + 32 * r + lane < n ? ld_stream(keys + wb + 32 * r + lane) : 0ULL;
+        #pragma unroll
+        for (int r = 0; r < kRows; ++r) {
+            const bool valid = wb + 32 * r + lane < n;
+            const u32 vmask = __ballot_sync(0xffffffffu, valid);
+            #pragma unroll
+            for (int p = 0; p < kMaxPasses; ++p) {      // static indices keep the plan in constant memory
+                if (p >= plan.npasses) break;
+                const u32 d = (u32)(k[r] >> plan.shift[p]) & plan.mask[p];
+                const u32 d0 = __shfl_sync(0xffffffffu, d, 0);
+                // neighbouring cells mostly share their upper digits: one atomic for the whole row then
+                if (vmask == 0xffffffffu && __all_sync(0xffffffffu, d == d0)) {
+                    if (lane == 0) atomicAdd(&h[p * kRadix + d0], 32u);
+                } else if (valid) {
+                    atomicAdd(&h[p * kRadix + d], 1u);
+                }
+            }
+        }
     }
     __syncthreads();
-    hist[(size_t)threadIdx.x * ntiles + blockIdx.x] = h[threadIdx.x];
+    for (int i = threadIdx.x; i < plan.npasses * kRadix; i += kSortThreads)
+        if (h[i]) atomicAdd(&ghist[(size_t)(i >> 8) * pass_stride + (i & 255)], h[i]);
 }
 
 struct SortSmem {
-    u64 keys[kSortTile];             // 32 KB
+    u32 klo[kSortTile];              // 16 KB  } the tile in digit order; slot q lives at swz(q), which
+    u32 khi[kSortTile];              // 16 KB  } keeps power-of-two strides (digit starts) off one bank
     u32 vals[kSortTile];             // 16 KB
     u32 wcnt[kSortThreads / 32][kRadix];   // 8 KB: per-warp digit counts, then per-warp digit offsets
     u32 dstart[kRadix];              // tile-local start of each digit
     u32 gbase[kRadix];               // global position of local slot q of digit d is gbase[d] + q
     u32 s_warp[9];
+    u32 s_tile;
 };
 
-__global__ void __launch_bounds__(kSortThreads)
-radix_scatter_kernel(const u64* __restrict__ kin, const u32* __restrict__ vin, u64* __restrict__ kout,
-                     u32* __restrict__ vout, const u32* __restrict__ tile_offs, i64 n, int ntiles,
-                     int shift, u32 mask)
+// One pass.  status[tile * 256 + d]: flag (bits 31..30) | count (30 bits); ticket: next tile to hand out.
+__global__ void __launch_bounds__(kSortThreads, 3)
+radix_onesweep_kernel(const u64* __restrict__ kin, const u32* __restrict__ vin, u64* __restrict__ kout,
+                      u32* __restrict__ vout, const u32* __restrict__ ghist /* this pass: [256] */,
+                      u32* __restrict__ status, u32* __restrict__ ticket, i64 n, int shift, u32 mask)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     SortSmem& S = *reinterpret_cast<SortSmem*>(smem_raw);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int tile = blockIdx.x;
-    const i64 base = (i64)tile * kSortTile;
-
+    if (tid == 0) S.s_tile = atomicAdd(ticket, 1u);
     for (int i = tid; i < (kSortThreads / 32) * kRadix; i += kSortThreads) (&S.wcnt[0][0])[i] = 0;
     __syncthreads();
+    const int tile = (int)S.s_tile;
+    const i64 base = (i64)tile * kSortTile;
 
     // warp-striped load: warp w owns the contiguous chunk [w*512, w*512+512) of the tile
     u64 key[kSortItems];
@@ -64,14 +113,13 @@ radix_scatter_kernel(const u64* __restrict__ kin, const u32* __restrict__ vin, u
         const i64 e = wbase + i * 32 + lane;
         const bool ok = e < n;
         key[i] = ok ? ld_stream(kin + e) : ~0ULL;
-        val[i] = ok ? ld_stream(vin + e) : 0u;
     }
     // stable rank inside the warp chunk: items are visited in memory order
     const u32 lt = lanemask_lt();
     #pragma unroll
     for (int i = 0; i < kSortItems; ++i) {
         const u32 d = (u32)(key[i] >> shift) & mask;     // padding keys (~0) take the top digit, last
-        const u32 peers = __match_any_sync(0xffffffffu, d);
+        const u32 peers = digit_peers(d);
         const u32 cnt = S.wcnt[warp][d];
         __syncwarp();
         const u32 r = __popc(peers & lt);
@@ -79,43 +127,60 @@ radix_scatter_kernel(const u64* __restrict__ kin, const u32* __restrict__ vin, u
         __syncwarp();
         rank[i] = cnt + r;
     }
+    #pragma unroll
+    for (int i = 0; i < kSortItems; ++i) {       // the values arrive while the digit offsets are worked out
+        const i64 e = wbase + i * 32 + lane;
+        val[i] = e < n ? ld_stream(vin + e) : 0u;
+    }
     __syncthreads();
     {   // thread d: exclusive scan of digit d over the warps, then over the digits
         const int d = tid;
         u32 run = 0;
         #pragma unroll
         for (int w = 0; w < kSortThreads / 32; ++w) { u32 c = S.wcnt[w][d]; S.wcnt[w][d] = run; run += c; }
+        // publish this tile's count of digit d, then look back for the pairs of digit d in earlier tiles
+        volatile u32* st = status + (size_t)tile * kRadix + d;
+        if (tile == 0) *st = kFlagPrefix | run; else *st = kFlagAgg | run;
         u32 total;
-        const u32 ex = block_excl_scan_256(run, total, S.s_warp);
+        const u32 ex = block_excl_scan_256(run, total, S.s_warp);          // tile-local start of digit d
+        const u32 gstart = block_excl_scan_256(ghist[d], total, S.s_warp);  // global start of digit d
+        u32 before = 0;
+        if (tile > 0) {
+            for (int t = tile - 1;; --t) {
+                volatile const u32* pt = status + (size_t)t * kRadix + d;
+                u32 v;
+                do { v = *pt; } while ((v >> 30) == 0u);
+                before += v & kValMask;
+                if (v & kFlagPrefix) break;
+            }
+            *st = kFlagPrefix | (before + run);
+        }
         S.dstart[d] = ex;
-        S.gbase[d] = tile_offs[(size_t)d * ntiles + tile] - ex;
+        S.gbase[d] = gstart + before - ex;
     }
     __syncthreads();
     #pragma unroll
     for (int i = 0; i < kSortItems; ++i) {
         const u32 d = (u32)(key[i] >> shift) & mask;
         const u32 q = S.dstart[d] + S.wcnt[warp][d] + rank[i];
-        S.keys[q] = key[i];
-        S.vals[q] = val[i];
+        const u32 qs = q ^ ((q >> 5) & 31u);
+        S.klo[qs] = (u32)key[i];
+        S.khi[qs] = (u32)(key[i] >> 32);
+        S.vals[qs] = val[i];
     }
     __syncthreads();
     const i64 left = n - base;
     const int nvalid = left < kSortTile ? (int)left : kSortTile;
     #pragma unroll 4
     for (int q = tid; q < nvalid; q += kSortThreads) {
-        const u64 k = S.keys[q];
+        const u32 qs = (u32)q ^ (((u32)q >> 5) & 31u);
+        const u64 k = ((u64)S.khi[qs] << 32) | S.klo[qs];
         const u32 d = (u32)(k >> shift) & mask;
         const u32 g = S.gbase[d] + (u32)q;
         kout[g] = k;
-        vout[g] = S.vals[q];
+        vout[g] = S.vals[qs];
     }
 }
-
-struct SortPlan {
-    int npasses;
-    int shift[8];
-    u32 mask[8];
-};
 
 // passes covering exactly the varying bits [lo_bit, hi_bit] in 8-bit digits
 inline SortPlan make_sort_plan(u64 varying)
@@ -133,18 +198,31 @@ inline SortPlan make_sort_plan(u64 varying)
     return p;
 }
 
-inline size_t sort_hist_elems(i64 n) { return (size_t)kRadix * (size_t)((n + kSortTile - 1) / kSortTile); }
+inline i64 sort_tiles(i64 n) { return (n + kSortTile - 1) / kSortTile; }
+// u32 words of sort scratch: per pass [256 histogram][ntiles * 256 status][1 ticket]
+inline size_t sort_pass_words(i64 n) { return (size_t)kRadix + (size_t)sort_tiles(n) * kRadix + 1; }
+inline size_t sort_hist_elems(i64 n) { return (size_t)kMaxPasses * sort_pass_words(n); }
 
-// one pass (k0,v0) -> (k1,v1); hist holds sort_hist_elems(n) u32, scratch scan_scratch_elems(that)
-inline cudaError_t radix_pass(const u64* k0, const u32* v0, u64* k1, u32* v1, i64 n, int shift, u32 mask,
-                              u32* hist, u32* scan_scratch, cudaStream_t st)
+// Sorts (k0, v0) in plan.npasses passes, ping-ponging with (k1, v1); the result is in (k0, v0) for an even
+// number of passes, else in (k1, v1).  scratch holds plan.npasses * sort_pass_words(n) u32.
+inline cudaError_t radix_sort_pairs(u64* k0, u32* v0, u64* k1, u32* v1, i64 n, const SortPlan& plan, u32* scratch,
+                                    int hist_grid, cudaStream_t st)
 {
-    const int ntiles = (int)((n + kSortTile - 1) / kSortTile);
-    radix_hist_kernel<<<ntiles, kSortThreads, 0, st>>>(k0, n, shift, mask, hist, ntiles);
-    cudaError_t e = exclusive_scan_u32(hist, hist, (i64)kRadix * ntiles, scan_scratch, nullptr, st);
+    if (plan.npasses == 0) return cudaSuccess;
+    const size_t pw = sort_pass_words(n);
+    const int ntiles = (int)sort_tiles(n);
+    cudaError_t e = cudaMemsetAsync(scratch, 0, sizeof(u32) * pw * plan.npasses, st);
     if (e != cudaSuccess) return e;
-    radix_scatter_kernel<<<ntiles, kSortThreads, sizeof(SortSmem), st>>>(k0, v0, k1, v1, hist, n, ntiles,
-                                                                         shift, mask);
+    // all histograms in one read; each pass's 256 counters sit at the head of its scratch block
+    SortPlan hp = plan;
+    radix_hist_strided_kernel<<<hist_grid, kSortThreads, 0, st>>>(k0, n, hp, scratch, (u32)pw);
+    for (int p = 0; p < plan.npasses; ++p) {
+        u32* blk = scratch + pw * p;
+        radix_onesweep_kernel<<<ntiles, kSortThreads, sizeof(SortSmem), st>>>(
+            k0, v0, k1, v1, blk, blk + kRadix, blk + kRadix + (size_t)ntiles * kRadix, n, plan.shift[p], plan.mask[p]);
+        u64* tk = k0; k0 = k1; k1 = tk;
+        u32* tv = v0; v0 = v1; v1 = tv;
+    }
     return cudaGetLastError();
 }
 

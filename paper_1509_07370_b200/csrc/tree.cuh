@@ -31,7 +31,7 @@ constexpr int kNumLevels = kMaxLevel + 1;        // node levels 0..21
 constexpr int kSlotLevels = kMaxLevel + 2;       // entity levels 0..22
 constexpr int kTopoDigits = kSlotLevels + kNumLevels;   // histogram rows: entities per level, nodes per level
 constexpr int kTopoThreads = 256;
-constexpr int kTopoItems = 16;
+constexpr int kTopoItems = 8;
 constexpr int kTopoChunk = 32 * kTopoItems;      // cells per warp chunk
 
 struct __align__(16) WalkAux {   // per slot, beside the float4 record (x, y, z, m)
@@ -59,49 +59,59 @@ __global__ void __launch_bounds__(kTopoThreads)
 topo_count_kernel(const u64* __restrict__ keys, i64 n, signed char* __restrict__ clev, u32* __restrict__ hist,
                   i64 nchunks)
 {
+    __shared__ u32 h[kTopoThreads / 32][kTopoDigits + 3];
     const u32 lane = lane_id();
-    const i64 chunk = (i64)blockIdx.x * (kTopoThreads / 32) + (threadIdx.x >> 5);
-    if (chunk >= nchunks) return;
+    const int warp = threadIdx.x >> 5;
+    const i64 chunk = (i64)blockIdx.x * (kTopoThreads / 32) + warp;
+    if (chunk >= nchunks) return;                      // whole warp leaves; only warp-level sync below
+    u32* hw = h[warp];
+    for (int d = lane; d < kTopoDigits; d += 32) hw[d] = 0u;
+    __syncwarp();
     const i64 wbase = chunk * kTopoChunk;
-    u64 k[kTopoItems];
-    #pragma unroll
-    for (int i = 0; i < kTopoItems; ++i) {
-        const i64 s = wbase + 32 * i + lane;
-        k[i] = s < n ? ld_stream(keys + s) : 0ULL;
-    }
     int carry = wbase > 0 ? common_levels(__ldg(keys + wbase - 1), __ldg(keys + wbase)) : -1;   // c(wbase - 1)
-    u32 cntT = 0, cntI = 0;                    // lane l: entities / internal nodes of level l in this chunk
-    #pragma unroll
-    for (int i = 0; i < kTopoItems; ++i) {
-        const i64 s = wbase + 32 * i + lane;
-        const bool valid = s < n;
-        u64 kn = __shfl_down_sync(0xffffffffu, k[i], 1);
-        if (i + 1 < kTopoItems) {                          // lane 31's successor: lane 0 of the next row
-            const u64 nx = __shfl_sync(0xffffffffu, k[i + 1], 0);
-            if (lane == 31) kn = nx;
-        } else if (lane == 31) {
-            kn = s + 1 < n ? __ldg(keys + s + 1) : 0ULL;
+    constexpr int kBatch = 4;                           // rows whose loads are in flight together
+    static_assert(kTopoItems % kBatch == 0, "rows per chunk");
+    for (int i0 = 0; i0 < kTopoItems; i0 += kBatch) {
+        if (wbase + 32 * i0 >= n) break;
+        u64 k[kBatch], kn[kBatch];
+        #pragma unroll
+        for (int r = 0; r < kBatch; ++r) {
+            const i64 s = wbase + 32 * (i0 + r) + lane;
+            k[r] = s < n ? ld_stream(keys + s) : 0ULL;
+            kn[r] = (lane == 31 && s + 1 < n) ? __ldg(keys + s + 1) : 0ULL;   // lane 31's successor
         }
-        const int cs = (valid && s + 1 < n) ? common_levels(k[i], kn) : -1;
-        int cp = __shfl_up_sync(0xffffffffu, cs, 1);
-        if (lane == 0) cp = carry;
-        carry = __shfl_sync(0xffffffffu, cs, 31);
-        u32 imask = 0u, emask = 0u;
-        if (valid) {
-            clev[s] = (signed char)cs;
-            entity_masks(cp, cs, imask, emask);
-        }
-        u32 U = __reduce_or_sync(0xffffffffu, emask);
-        while (U) {
-            const int l = __ffs(U) - 1;
-            U &= U - 1u;
-            const u32 bal = __ballot_sync(0xffffffffu, (emask >> l) & 1u);
-            const u32 balI = __ballot_sync(0xffffffffu, (imask >> l) & 1u);
-            if ((int)lane == l) { cntT += __popc(bal); cntI += __popc(balI); }
+        #pragma unroll
+        for (int r = 0; r < kBatch; ++r) {
+            const i64 s = wbase + 32 * (i0 + r) + lane;
+            const bool valid = s < n;
+            const u64 nx = __shfl_down_sync(0xffffffffu, k[r], 1);
+            if (lane != 31) kn[r] = nx;
+            const int cs = (valid && s + 1 < n) ? common_levels(k[r], kn[r]) : -1;
+            int cp = __shfl_up_sync(0xffffffffu, cs, 1);
+            if (lane == 0) cp = carry;
+            carry = __shfl_sync(0xffffffffu, cs, 31);
+            if (valid) clev[s] = (signed char)cs;
+            // leaf entity: usually the same level for the whole row -> one shared atomic
+            const int leafL = valid ? (cp > cs ? cp : cs) + 1 : -1;
+            const int l0 = __shfl_sync(0xffffffffu, leafL, 0);
+            const u32 vmask = __ballot_sync(0xffffffffu, valid);
+            const u32 same = __ballot_sync(0xffffffffu, leafL == l0);
+            if ((same & vmask) == vmask) {
+                if (lane == 0 && vmask) atomicAdd(&hw[l0], (u32)__popc(vmask));
+            } else if (valid) {
+                atomicAdd(&hw[leafL], 1u);
+            }
+            // internal nodes started by this cell: levels cp+1 .. cs (few lanes, few levels)
+            if (valid) {
+                for (int l = cp + 1; l <= cs; ++l) {
+                    atomicAdd(&hw[l], 1u);
+                    atomicAdd(&hw[kSlotLevels + l], 1u);
+                }
+            }
         }
     }
-    if (lane < (u32)kSlotLevels) hist[(i64)lane * nchunks + chunk] = cntT;
-    if (lane < (u32)kNumLevels) hist[(i64)(kSlotLevels + lane) * nchunks + chunk] = cntI;
+    __syncwarp();
+    for (int d = lane; d < kTopoDigits; d += 32) hist[(i64)d * nchunks + chunk] = hw[d];
 }
 
 // row starts of the scanned histogram (+ the grand total) for the host: out[d] = scanned[d * nchunks]
@@ -136,17 +146,24 @@ topo_assign_kernel(const signed char* __restrict__ clev, i64 n, const u32* __res
     u32 cntI = lane < (u32)kNumLevels ? scanned[(i64)(kSlotLevels + lane) * nchunks + chunk] - nslots : 0u;
     int carry = wbase > 0 ? (int)clev[wbase - 1] : -1;
     const uint4 leaf_aux = make_uint4(0u, 0u, 0u, 0u);
-    #pragma unroll 2
+    u32 oi[kTopoItems];                        // the chunk's permutation entries and c(s), fetched up front so
+    int ci[kTopoItems];                        // that a row's gathers do not wait behind them
+    #pragma unroll
+    for (int i = 0; i < kTopoItems; ++i) {
+        const i64 s = wbase + 32 * i + lane;
+        oi[i] = s < n ? ld_stream(idx + s) : 0u;
+        ci[i] = s < n ? (int)clev[s] : -1;
+    }
+    #pragma unroll
     for (int i = 0; i < kTopoItems; ++i) {
         if (wbase + 32 * i >= n) break;
         const i64 s = wbase + 32 * i + lane;
         const bool valid = s < n;
         double px = 0.0, py = 0.0, pz = 0.0, pm = 0.0;
-        int cs = -1;
+        const int cs = ci[i];
         if (valid) {
-            const u32 o = ld_stream(idx + s);
+            const u32 o = oi[i];
             px = __ldg(x + o); py = __ldg(y + o); pz = __ldg(z + o); pm = __ldg(m + o);
-            cs = (int)clev[s];
         }
         int cp = __shfl_up_sync(0xffffffffu, cs, 1);
         if (lane == 0) cp = carry;
@@ -179,12 +196,12 @@ topo_assign_kernel(const signed char* __restrict__ clev, i64 n, const u32* __res
             }
         }
         if (valid) {
-            leaf_slot[s] = myslot;
+            st_stream(leaf_slot + s, myslot);          // written once, read much later: keep L2 for the gathers
             double2* o64 = reinterpret_cast<double2*>(rec64 + myslot);
-            o64[0] = make_double2(px, py);
-            o64[1] = make_double2(pz, pm);
-            rec[myslot] = make_float4((float)px, (float)py, (float)pz, (float)pm);
-            reinterpret_cast<uint4*>(aux)[myslot] = leaf_aux;
+            st_stream(o64, make_double2(px, py));
+            st_stream(o64 + 1, make_double2(pz, pm));
+            st_stream(rec + myslot, make_float4((float)px, (float)py, (float)pz, (float)pm));
+            st_stream(reinterpret_cast<uint4*>(aux) + myslot, leaf_aux);
         }
     }
 }
@@ -218,14 +235,18 @@ __device__ __forceinline__ u32 compact3(u64 v)   // inverse of the key bit-sprea
 
 // Node b of level `level`: children = slots [nfirst[b], nfirst[b+1]) (the last node of the level ends at
 // slot_end, the end of the level-(level+1) slots).  Reads 32 B per child, writes 80 B per node.
-__global__ void __launch_bounds__(128)
-moments_kernel(i64 b0, i64 b1, int level, u32 slot_end, const u64* __restrict__ keys,
-               const u32* __restrict__ nlo, const u32* __restrict__ nfirst, const u32* __restrict__ node_slot,
-               double4* __restrict__ rec64, double* __restrict__ delta64, float4* __restrict__ rec,
-               WalkAux* __restrict__ aux, u32* __restrict__ max_bucket, double x0, double y0, double z0, double L)
+struct MomentArgs {
+    const u64* keys; const u32* nlo; const u32* nfirst; const u32* node_slot;
+    double4* rec64; double* delta64; float4* rec; WalkAux* aux; u32* max_bucket;
+    double x0, y0, z0, L;
+};
+
+__device__ __forceinline__ void moments_node(i64 b, i64 b1, int level, u32 slot_end, const MomentArgs& A)
 {
-    const i64 b = b0 + (i64)blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= b1) return;
+    const u64* keys = A.keys; const u32* nlo = A.nlo; const u32* nfirst = A.nfirst; const u32* node_slot = A.node_slot;
+    double4* rec64 = A.rec64; double* delta64 = A.delta64; float4* rec = A.rec; WalkAux* aux = A.aux;
+    u32* max_bucket = A.max_bucket;
+    const double x0 = A.x0, y0 = A.y0, z0 = A.z0, L = A.L;
     const u32 first = nfirst[b];
     const u32 cnt = (b + 1 < b1 ? nfirst[b + 1] : slot_end) - first;
     double M = 0.0, Sx = 0.0, Sy = 0.0, Sz = 0.0;
@@ -263,6 +284,33 @@ moments_kernel(i64 b0, i64 b1, int level, u32 slot_end, const u64* __restrict__ 
     a.count = cnt;
     aux[slot] = a;
     if (level == kMaxLevel) atomicMax(max_bucket, cnt);
+}
+
+__global__ void __launch_bounds__(128)
+moments_kernel(i64 b0, i64 b1, int level, u32 slot_end, const MomentArgs A)
+{
+    const i64 b = b0 + (i64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b < b1) moments_node(b, b1, level, slot_end, A);
+}
+
+// a run of small levels (deepest first) in ONE block: a level's nodes are complete before the next starts
+constexpr int kSmallLevelNodes = 512;
+constexpr int kMomSmallThreads = 512;
+struct SmallLevels {
+    int nlev;
+    int level[kNumLevels];
+    u32 b0[kNumLevels], b1[kNumLevels], slot_end[kNumLevels];
+};
+
+__global__ void __launch_bounds__(kMomSmallThreads)
+moments_small_kernel(const SmallLevels sl, const MomentArgs A)
+{
+    for (int k = 0; k < sl.nlev; ++k) {
+        for (i64 b = (i64)sl.b0[k] + threadIdx.x; b < (i64)sl.b1[k]; b += kMomSmallThreads)
+            moments_node(b, sl.b1[k], sl.level[k], sl.slot_end[k], A);
+        __threadfence_block();
+        __syncthreads();
+    }
 }
 
 struct TopoLevels {               // host-computed from the scanned histogram

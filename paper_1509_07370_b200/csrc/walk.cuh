@@ -261,7 +261,7 @@ walk_pair_kernel(const WalkParams P)
     }
     __syncwarp();
 
-    const u32 lt = lanemask_lt();
+    const u32 lt = (1u << lane) - 1u;
     const int sub = lane >> 3, j = lane & 7;
     const float inv_theta = P.inv_theta;
     const bool mac94 = P.mac == 1;
