@@ -72,70 +72,64 @@ __device__ __forceinline__ float rsqrt_approx(float v)
 
 __device__ __forceinline__ float2 splat2(float v) { return make_float2(v, v); }
 
-// ---- U2: entries both groups take; packed across the lane's two targets -------------------------
-// np* = (-p_A, -p_B).  The list is padded to a multiple of 4 entries by the caller.
-__device__ __forceinline__ void u2_body(const float4 v, const float2 npx, const float2 npy, const float2 npz,
-                                        float2& s)
+// ---- unchecked lists: SoA (x[CAP] y[CAP] z[CAP] m[CAP]), evaluated four entries per iteration ------
+// The packed fp32x2 operands are two ENTRIES (adjacent registers of one 16-byte shared load), the
+// target's coordinates are loop-invariant splatted pairs: no per-entry register shuffling.
+// Lists are padded to a multiple of 4 entries by the caller.
+struct Tgt2 { float2 x, y, z; };           // (-p, -p) per coordinate of one target
+
+__device__ __forceinline__ void quad_body(const float4 x, const float4 y, const float4 z, const float4 m,
+                                          const Tgt2& t, float2& s0, float2& s1)
 {
-    const float2 dx = __fadd2_rn(splat2(v.x), npx);
-    const float2 dy = __fadd2_rn(splat2(v.y), npy);
-    const float2 dz = __fadd2_rn(splat2(v.z), npz);
-    float2 d2 = __ffma2_rn(dx, dx, splat2(kTinyD2));
-    d2 = __ffma2_rn(dy, dy, d2);
-    d2 = __ffma2_rn(dz, dz, d2);
-    const float2 r = make_float2(rsqrt_approx(d2.x), rsqrt_approx(d2.y));
-    s = __ffma2_rn(splat2(v.w), r, s);
+    const float2 dx0 = __fadd2_rn(make_float2(x.x, x.y), t.x), dx1 = __fadd2_rn(make_float2(x.z, x.w), t.x);
+    const float2 dy0 = __fadd2_rn(make_float2(y.x, y.y), t.y), dy1 = __fadd2_rn(make_float2(y.z, y.w), t.y);
+    const float2 dz0 = __fadd2_rn(make_float2(z.x, z.y), t.z), dz1 = __fadd2_rn(make_float2(z.z, z.w), t.z);
+    float2 d0 = __ffma2_rn(dx0, dx0, splat2(kTinyD2));
+    float2 d1 = __ffma2_rn(dx1, dx1, splat2(kTinyD2));
+    d0 = __ffma2_rn(dy0, dy0, d0);
+    d1 = __ffma2_rn(dy1, dy1, d1);
+    d0 = __ffma2_rn(dz0, dz0, d0);
+    d1 = __ffma2_rn(dz1, dz1, d1);
+    const float2 r0 = make_float2(rsqrt_approx(d0.x), rsqrt_approx(d0.y));
+    const float2 r1 = make_float2(rsqrt_approx(d1.x), rsqrt_approx(d1.y));
+    s0 = __ffma2_rn(make_float2(m.x, m.y), r0, s0);
+    s1 = __ffma2_rn(make_float2(m.z, m.w), r1, s1);
 }
 
-__device__ __forceinline__ void eval_u2(const float4* __restrict__ L, int cnt, const float2 npx, const float2 npy,
-                                        const float2 npz, double& accA, double& accB)
-{
-    float2 s0 = splat2(0.f), s1 = splat2(0.f), s2 = splat2(0.f), s3 = splat2(0.f);
-    const int nq = (cnt + 3) >> 2;
-    #pragma unroll 2
-    for (int q = 0; q < nq; ++q) {
-        const float4 v0 = L[4 * q + 0], v1 = L[4 * q + 1], v2 = L[4 * q + 2], v3 = L[4 * q + 3];
-        u2_body(v0, npx, npy, npz, s0);
-        u2_body(v1, npx, npy, npz, s1);
-        u2_body(v2, npx, npy, npz, s2);
-        u2_body(v3, npx, npy, npz, s3);
-    }
-    accA += ((double)s0.x + (double)s1.x) + ((double)s2.x + (double)s3.x);
-    accB += ((double)s0.y + (double)s1.y) + ((double)s2.y + (double)s3.y);
-}
-
-// ---- UA / UB: entries one group takes; SoA lists, packed across two entries --------------------
-// np = (-p, -p, -p) of the one target.  Padded to a multiple of 4 entries by the caller.
-__device__ __forceinline__ double eval_u1(const float* __restrict__ L, int cnt, const float npx, const float npy,
-                                          const float npz)
+// one target
+template <int CAP>
+__device__ __forceinline__ double eval_soa(const float* __restrict__ L, int cnt, const Tgt2& t)
 {
     const float4* X = reinterpret_cast<const float4*>(L);
-    const float4* Y = reinterpret_cast<const float4*>(L + kU1Cap);
-    const float4* Z = reinterpret_cast<const float4*>(L + 2 * kU1Cap);
-    const float4* M = reinterpret_cast<const float4*>(L + 3 * kU1Cap);
+    const float4* Y = reinterpret_cast<const float4*>(L + CAP);
+    const float4* Z = reinterpret_cast<const float4*>(L + 2 * CAP);
+    const float4* M = reinterpret_cast<const float4*>(L + 3 * CAP);
     float2 s0 = splat2(0.f), s1 = splat2(0.f);
+    const int nq = (cnt + 3) >> 2;
+    #pragma unroll 2
+    for (int q = 0; q < nq; ++q) quad_body(X[q], Y[q], Z[q], M[q], t, s0, s1);
+    return ((double)s0.x + (double)s0.y) + ((double)s1.x + (double)s1.y);
+}
+
+// two targets (the lane's member of group A and of group B) from the same loads
+template <int CAP>
+__device__ __forceinline__ void eval_soa2(const float* __restrict__ L, int cnt, const Tgt2& tA, const Tgt2& tB,
+                                          double& accA, double& accB)
+{
+    const float4* X = reinterpret_cast<const float4*>(L);
+    const float4* Y = reinterpret_cast<const float4*>(L + CAP);
+    const float4* Z = reinterpret_cast<const float4*>(L + 2 * CAP);
+    const float4* M = reinterpret_cast<const float4*>(L + 3 * CAP);
+    float2 a0 = splat2(0.f), a1 = splat2(0.f), b0 = splat2(0.f), b1 = splat2(0.f);
     const int nq = (cnt + 3) >> 2;
     #pragma unroll 2
     for (int q = 0; q < nq; ++q) {
         const float4 x = X[q], y = Y[q], z = Z[q], m = M[q];
-        const float2 dx0 = __fadd2_rn(make_float2(x.x, x.y), splat2(npx));
-        const float2 dx1 = __fadd2_rn(make_float2(x.z, x.w), splat2(npx));
-        const float2 dy0 = __fadd2_rn(make_float2(y.x, y.y), splat2(npy));
-        const float2 dy1 = __fadd2_rn(make_float2(y.z, y.w), splat2(npy));
-        const float2 dz0 = __fadd2_rn(make_float2(z.x, z.y), splat2(npz));
-        const float2 dz1 = __fadd2_rn(make_float2(z.z, z.w), splat2(npz));
-        float2 d0 = __ffma2_rn(dx0, dx0, splat2(kTinyD2));
-        float2 d1 = __ffma2_rn(dx1, dx1, splat2(kTinyD2));
-        d0 = __ffma2_rn(dy0, dy0, d0);
-        d1 = __ffma2_rn(dy1, dy1, d1);
-        d0 = __ffma2_rn(dz0, dz0, d0);
-        d1 = __ffma2_rn(dz1, dz1, d1);
-        const float2 r0 = make_float2(rsqrt_approx(d0.x), rsqrt_approx(d0.y));
-        const float2 r1 = make_float2(rsqrt_approx(d1.x), rsqrt_approx(d1.y));
-        s0 = __ffma2_rn(make_float2(m.x, m.y), r0, s0);
-        s1 = __ffma2_rn(make_float2(m.z, m.w), r1, s1);
+        quad_body(x, y, z, m, tA, a0, a1);
+        quad_body(x, y, z, m, tB, b0, b1);
     }
-    return ((double)s0.x + (double)s0.y) + ((double)s1.x + (double)s1.y);
+    accA += ((double)a0.x + (double)a0.y) + ((double)a1.x + (double)a1.y);
+    accB += ((double)b0.x + (double)b0.y) + ((double)b1.x + (double)b1.y);
 }
 
 // ---- C: leaf cells inside a group's bounding box; zero-distance pairs are skipped (W3) ----------
@@ -162,21 +156,18 @@ __device__ __forceinline__ void eval_c(const float4* __restrict__ L, const u32* 
     accB += (double)s.y;
 }
 
-__device__ __forceinline__ void u1_store(float* L, int e, float4 r)
+template <int CAP>
+__device__ __forceinline__ void soa_store(float* L, int e, float4 r)
 {
-    L[e] = r.x; L[kU1Cap + e] = r.y; L[2 * kU1Cap + e] = r.z; L[3 * kU1Cap + e] = r.w;
+    L[e] = r.x; L[CAP + e] = r.y; L[2 * CAP + e] = r.z; L[3 * CAP + e] = r.w;
 }
 
 // zero-mass entries far away (finite d^2, no NaN) up to the next multiple of 4
-__device__ __forceinline__ void u2_pad(float4* L, int cnt)
+template <int CAP>
+__device__ __forceinline__ void soa_pad(float* L, int cnt)
 {
     const int e = cnt + (int)lane_id();
-    if (e < ((cnt + 3) & ~3)) L[e] = make_float4(3.0e18f, 3.0e18f, 3.0e18f, 0.f);
-}
-__device__ __forceinline__ void u1_pad(float* L, int cnt)
-{
-    const int e = cnt + (int)lane_id();
-    if (e < ((cnt + 3) & ~3)) u1_store(L, e, make_float4(3.0e18f, 3.0e18f, 3.0e18f, 0.f));
+    if (e < ((cnt + 3) & ~3)) soa_store<CAP>(L, e, make_float4(3.0e18f, 3.0e18f, 3.0e18f, 0.f));
 }
 
 __device__ __forceinline__ float warp_min(float v)
@@ -228,8 +219,8 @@ walk_pair_kernel(const WalkParams P)
     if (gA >= P.ngroups) return;                      // whole warp leaves; no block-level sync below
 
     unsigned char* my = smem_raw + (size_t)warp * walk_smem_per_warp(P.stack_cap);
-    float4* U2 = reinterpret_cast<float4*>(my);                         // both groups
-    float* UA = reinterpret_cast<float*>(U2 + kU2Cap);                  // group A only (SoA)
+    float* U2 = reinterpret_cast<float*>(my);                           // both groups (SoA)
+    float* UA = U2 + 4 * kU2Cap;                                        // group A only (SoA)
     float* UB = UA + 4 * kU1Cap;                                        // group B only (SoA)
     float4* C = reinterpret_cast<float4*>(UB + 4 * kU1Cap);             // checked leaf cells
     u32* Cm = reinterpret_cast<u32*>(C + kCCap);                        //   and the groups they serve
@@ -249,6 +240,9 @@ walk_pair_kernel(const WalkParams P)
     box.yl = make_float2(warp_min(tA.y), warp_min(tB.y)); box.yh = make_float2(warp_max(tA.y), warp_max(tB.y));
     box.zl = make_float2(warp_min(tA.z), warp_min(tB.z)); box.zh = make_float2(warp_max(tA.z), warp_max(tB.z));
     const float2 npx = make_float2(-tA.x, -tB.x), npy = make_float2(-tA.y, -tB.y), npz = make_float2(-tA.z, -tB.z);
+    Tgt2 TA, TB;                                      // splatted per target, for the entry-packed lists
+    TA.x = splat2(-tA.x); TA.y = splat2(-tA.y); TA.z = splat2(-tA.z);
+    TB.x = splat2(-tB.x); TB.y = splat2(-tB.y); TB.z = splat2(-tB.z);
 
     double accA = 0.0, accB = 0.0;
     int nU2 = 0, nUA = 0, nUB = 0, nC = 0;          // list fill (warp-uniform)
@@ -353,30 +347,30 @@ walk_pair_kernel(const WalkParams P)
         const u32 bC = __ballot_sync(0xffffffffu, danger);
         const u32 bsel = toU2 ? bU2 : (toUA ? bUA : (toUB ? bUB : bC));
         const int rank = __popc(bsel & lt);
-        if (toU2) U2[nU2 + rank] = r;
-        if (toUA) u1_store(UA, nUA + rank, r);
-        if (toUB) u1_store(UB, nUB + rank, r);
+        if (toU2) soa_store<kU2Cap>(U2, nU2 + rank, r);
+        if (toUA) soa_store<kU1Cap>(UA, nUA + rank, r);
+        if (toUB) soa_store<kU1Cap>(UB, nUB + rank, r);
         if (danger) { C[nC + rank] = r; Cm[nC + rank] = msk; }
         nU2 += __popc(bU2); nUA += __popc(bUA); nUB += __popc(bUB); nC += __popc(bC);
         __syncwarp();
         // ---- evaluate a list before the next step could overflow it ----
         if ((((nUA | nUB | nC) >> 5) != 0) || nU2 >= kU2Cap - kStepMax) {
             if (nU2 >= kU2Cap - kStepMax) {
-                u2_pad(U2, nU2);
+                soa_pad<kU2Cap>(U2, nU2);
                 __syncwarp();
-                eval_u2(U2, nU2, npx, npy, npz, accA, accB);
+                eval_soa2<kU2Cap>(U2, nU2, TA, TB, accA, accB);
                 nU2 = 0;
             }
             if (nUA >= kU1Cap - kStepMax) {
-                u1_pad(UA, nUA);
+                soa_pad<kU1Cap>(UA, nUA);
                 __syncwarp();
-                accA += eval_u1(UA, nUA, npx.x, npy.x, npz.x);
+                accA += eval_soa<kU1Cap>(UA, nUA, TA);
                 nUA = 0;
             }
             if (nUB >= kU1Cap - kStepMax) {
-                u1_pad(UB, nUB);
+                soa_pad<kU1Cap>(UB, nUB);
                 __syncwarp();
-                accB += eval_u1(UB, nUB, npx.y, npy.y, npz.y);
+                accB += eval_soa<kU1Cap>(UB, nUB, TB);
                 nUB = 0;
             }
             if (nC >= kCCap - kStepMax) {
@@ -398,19 +392,19 @@ walk_pair_kernel(const WalkParams P)
         return;
     }
     if (nU2 > 0) {
-        u2_pad(U2, nU2);
+        soa_pad<kU2Cap>(U2, nU2);
         __syncwarp();
-        eval_u2(U2, nU2, npx, npy, npz, accA, accB);
+        eval_soa2<kU2Cap>(U2, nU2, TA, TB, accA, accB);
     }
     if (nUA > 0) {
-        u1_pad(UA, nUA);
+        soa_pad<kU1Cap>(UA, nUA);
         __syncwarp();
-        accA += eval_u1(UA, nUA, npx.x, npy.x, npz.x);
+        accA += eval_soa<kU1Cap>(UA, nUA, TA);
     }
     if (nUB > 0) {
-        u1_pad(UB, nUB);
+        soa_pad<kU1Cap>(UB, nUB);
         __syncwarp();
-        accB += eval_u1(UB, nUB, npx.y, npy.y, npz.y);
+        accB += eval_soa<kU1Cap>(UB, nUB, TB);
     }
     if (nC > 0) eval_c(C, Cm, nC, npx, npy, npz, accA, accB);
     // ---- a7: Phi_t = -G * sum, written in the original cell order (W-rule 4) ----
