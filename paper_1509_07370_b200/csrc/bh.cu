@@ -72,8 +72,7 @@ struct bh_ctx {
 
     // per cell
     DevBuf keysA, keysB, idxA, idxB;      // ping-pong (key, index)
-    u64* keys = nullptr;                  // sorted keys (one of keysA/keysB)
-    u32* idx = nullptr;                   // perm: original index of sorted slot
+    SortedView sv = {};                   // the sorted cells as the sort left them (packed / generic / identity)
     DevBuf clev, leaf_slot;               // c(s); slot of sorted cell s
     DevBuf leaf64, slot_of;               // bh_potential_direct's own copies (built on its first call)
     bool direct_ready = false;
@@ -168,8 +167,14 @@ int bh_create(bh_ctx** out, int device, void* cuda_stream)
         if (rc) break;
         if ((e = ctx->scalars.ensure(sizeof(DeviceScalars))) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaMalloc"); break; }
         if ((e = cudaMallocHost(&ctx->h_scalars, sizeof(DeviceScalars))) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaMallocHost"); break; }
-        if ((e = cudaFuncSetAttribute(radix_onesweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)sizeof(SortSmem))) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(sort)"); break; }
+        if ((e = cudaFuncSetAttribute(radix_onesweep_kernel<kGeneric>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)sort_smem_bytes(false))) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(sort)"); break; }
+        if ((e = cudaFuncSetAttribute(radix_onesweep_kernel<kGenericFirst>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)sort_smem_bytes(false))) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(sort)"); break; }
+        if ((e = cudaFuncSetAttribute(radix_onesweep_kernel<kPacked>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)sort_smem_bytes(true))) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(sort)"); break; }
+        if ((e = cudaFuncSetAttribute(radix_onesweep_kernel<kPackedFirst>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)sort_smem_bytes(true))) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(sort)"); break; }
         if ((e = cudaFuncSetAttribute(walk_pair_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       227 * 1024)) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(walk)"); break; }
         if ((e = cudaFuncSetAttribute(walk_pair_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -224,8 +229,6 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
     // ---- buffers that depend on n only ----
     BH_CUDA(ctx->keysA.ensure(sizeof(u64) * n));
     BH_CUDA(ctx->keysB.ensure(sizeof(u64) * n));
-    BH_CUDA(ctx->idxA.ensure(sizeof(u32) * n));
-    BH_CUDA(ctx->idxB.ensure(sizeof(u32) * n));
     BH_CUDA(ctx->clev.ensure((size_t)n + 16));
     BH_CUDA(ctx->leaf_slot.ensure(sizeof(u32) * n));
     {
@@ -248,10 +251,10 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
         const int grid = persistent_grid(ctx, 8);
         if (aligned16(x) && aligned16(y) && aligned16(z))
             morton_keys_kernel<2><<<grid, 256, 0, st>>>(x, y, z, n, cube[0], cube[1], cube[2], s,
-                                                        ctx->keysA.as<u64>(), ctx->idxA.as<u32>(), &ds->keyred);
+                                                        ctx->keysA.as<u64>(), &ds->keyred);
         else
             morton_keys_kernel<1><<<grid, 256, 0, st>>>(x, y, z, n, cube[0], cube[1], cube[2], s,
-                                                        ctx->keysA.as<u64>(), ctx->idxA.as<u32>(), &ds->keyred);
+                                                        ctx->keysA.as<u64>(), &ds->keyred);
         BH_CUDA(cudaGetLastError());
     }
     ctx->launches_build += 1;
@@ -265,12 +268,28 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
     ctx->sort_passes = plan.npasses;
 
     // ---- a2: radix sort of (key, index) ----
+    if (plan.npasses > 0 && !plan.packed) {      // the permutation is stored only when a key window of 32 bits is too narrow
+        BH_CUDA(ctx->idxA.ensure(sizeof(u32) * n));
+        BH_CUDA(ctx->idxB.ensure(sizeof(u32) * n));
+    }
     BH_CUDA(radix_sort_pairs(ctx->keysA.as<u64>(), ctx->idxA.as<u32>(), ctx->keysB.as<u64>(), ctx->idxB.as<u32>(), n,
                              plan, ctx->hist.as<u32>(), persistent_grid(ctx, 8), st));
     ctx->launches_build += plan.npasses ? 1 + plan.npasses : 0;   // histogram + one kernel per pass
-    const bool odd = plan.npasses & 1;
-    ctx->keys = odd ? ctx->keysB.as<u64>() : ctx->keysA.as<u64>();
-    ctx->idx = odd ? ctx->idxB.as<u32>() : ctx->idxA.as<u32>();
+    {
+        const bool odd = plan.npasses & 1;
+        const u64* kres = odd ? ctx->keysB.as<u64>() : ctx->keysA.as<u64>();
+        SortedView& sv = ctx->sv;
+        sv.packed = nullptr; sv.keys = nullptr; sv.idx = nullptr; sv.cbits = 0; sv.lo = 0;
+        if (plan.npasses == 0) sv.keys = kres;                      // identity: all keys equal
+        else if (plan.packed) {
+            sv.packed = kres;
+            sv.lo = plan.lo;
+            sv.cbits = ctx->h_scalars->keyred.key_and & ~(0xffffffffULL << plan.lo);
+        } else {
+            sv.keys = kres;
+            sv.idx = odd ? ctx->idxB.as<u32>() : ctx->idxA.as<u32>();
+        }
+    }
     BH_CUDA(cudaEventRecord(ctx->ev[EV_SORT], st));
 
     // ---- a4: topology (a3, the permutation of the cell data, is fused into the assigning kernel) ----
@@ -280,7 +299,7 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
         const i64 nchunks = topo_chunks(n);
         const unsigned tgrid = blocks_for(nchunks, kTopoThreads / 32);
         u32* hist = ctx->hist.as<u32>();
-        topo_count_kernel<<<tgrid, kTopoThreads, 0, st>>>(ctx->keys, n, ctx->clev.as<signed char>(), hist, nchunks);
+        topo_count_kernel<<<tgrid, kTopoThreads, 0, st>>>(ctx->sv, n, ctx->clev.as<signed char>(), hist, nchunks);
         BH_CUDA(cudaGetLastError());
         BH_CUDA(exclusive_scan_u32(hist, hist, (i64)kTopoDigits * nchunks, ctx->scan_scratch.as<u32>(),
                                    &ds->scan_total, st));
@@ -315,7 +334,7 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
         BH_CUDA(ctx->aux.ensure(sizeof(WalkAux) * nslots));
 
         topo_assign_kernel<<<tgrid, kTopoThreads, 0, st>>>(
-            ctx->clev.as<signed char>(), n, ctx->idx, x, y, z, m, hist, nchunks, (u32)nslots,
+            ctx->clev.as<signed char>(), n, ctx->sv, x, y, z, m, hist, nchunks, (u32)nslots,
             ctx->leaf_slot.as<u32>(), ctx->node_slot.as<u32>(), ctx->nfirst.as<u32>(), ctx->nlo.as<u32>(),
             ctx->rec64.as<double4>(), ctx->rec.as<float4>(), ctx->aux.as<WalkAux>());
         BH_CUDA(cudaGetLastError());
@@ -324,7 +343,7 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
 
         // ---- a5: moments, deepest level first; runs of small levels share one single-block launch ----
         MomentArgs MA;
-        MA.keys = ctx->keys; MA.nlo = ctx->nlo.as<u32>(); MA.nfirst = ctx->nfirst.as<u32>();
+        MA.sv = ctx->sv; MA.nlo = ctx->nlo.as<u32>(); MA.nfirst = ctx->nfirst.as<u32>();
         MA.node_slot = ctx->node_slot.as<u32>(); MA.rec64 = ctx->rec64.as<double4>();
         MA.delta64 = ctx->delta64.as<double>(); MA.rec = ctx->rec.as<float4>(); MA.aux = ctx->aux.as<WalkAux>();
         MA.max_bucket = &ds->max_bucket; MA.x0 = cube[0]; MA.y0 = cube[1]; MA.z0 = cube[2]; MA.L = cube[3];
@@ -381,7 +400,7 @@ int launch_walk(bh_ctx* ctx, double theta, double G, double* phi, int group, int
     P.rec = ctx->rec.as<float4>();
     P.aux = ctx->aux.as<WalkAux>();
     P.leaf_slot = ctx->leaf_slot.as<u32>();
-    P.idx = ctx->idx;
+    P.sv = ctx->sv;
     P.phi = phi;
     P.gcount = ctx->gcount.as<uint4>();
     P.n = n;
@@ -463,7 +482,7 @@ int bh_potential_direct(bh_ctx* ctx, double G, const int64_t* targets, int64_t n
             BH_CUDA(cudaMemsetAsync(ctx->slot_of.p, 0, sizeof(u32), ctx->stream));
         } else {
             direct_prepare_kernel<<<blocks_for(ctx->n, 256), 256, 0, ctx->stream>>>(
-                ctx->idx, ctx->leaf_slot.as<u32>(), ctx->rec64.as<double4>(), ctx->n, ctx->leaf64.as<double4>(),
+                ctx->sv, ctx->leaf_slot.as<u32>(), ctx->rec64.as<double4>(), ctx->n, ctx->leaf64.as<double4>(),
                 ctx->slot_of.as<u32>());
             BH_CUDA(cudaGetLastError());
         }
@@ -513,11 +532,13 @@ int bh_export_tree(bh_ctx* ctx, uint64_t* keys, uint32_t* perm, int32_t* level, 
     if (!ctx->built) return BH_ERR_NOT_BUILT;
     BH_CUDA(cudaSetDevice(ctx->device));
     cudaStream_t st = ctx->stream;
-    if (keys) BH_CUDA(cudaMemcpyAsync(keys, ctx->keys, sizeof(u64) * ctx->n, cudaMemcpyDeviceToDevice, st));
-    if (perm) BH_CUDA(cudaMemcpyAsync(perm, ctx->idx, sizeof(u32) * ctx->n, cudaMemcpyDeviceToDevice, st));
+    if (keys || perm) {
+        export_sorted_kernel<<<blocks_for(ctx->n, 256), 256, 0, st>>>(ctx->sv, ctx->n, reinterpret_cast<u64*>(keys), perm);
+        BH_CUDA(cudaGetLastError());
+    }
     if (ctx->nn > 0) {
         export_nodes_kernel<<<blocks_for(ctx->nn, 256), 256, 0, st>>>(
-            ctx->nn, ctx->n, ctx->lv, ctx->keys, ctx->nlo.as<u32>(), ctx->nfirst.as<u32>(), ctx->node_slot.as<u32>(),
+            ctx->nn, ctx->n, ctx->lv, ctx->sv, ctx->nlo.as<u32>(), ctx->nfirst.as<u32>(), ctx->node_slot.as<u32>(),
             ctx->rec64.as<double4>(), ctx->delta64.as<double>(), level, reinterpret_cast<u64*>(prefix),
             reinterpret_cast<i64*>(lo), reinterpret_cast<i64*>(hi), nchild, M, Rx, Ry, Rz, delta);
         BH_CUDA(cudaGetLastError());
@@ -544,7 +565,7 @@ int bh_last_interactions(bh_ctx* ctx, uint32_t* per_target)
     if (!ctx->walked) return BH_ERR_NOT_BUILT;
     BH_CUDA(cudaSetDevice(ctx->device));
     { int rc = ensure_counts(ctx); if (rc != BH_OK) return rc; }
-    per_target_counts_kernel<<<blocks_for(ctx->n, 256), 256, 0, ctx->stream>>>(ctx->gcount.as<uint4>(), ctx->idx,
+    per_target_counts_kernel<<<blocks_for(ctx->n, 256), 256, 0, ctx->stream>>>(ctx->gcount.as<uint4>(), ctx->sv,
                                                                                ctx->n, ctx->walk_group, per_target);
     BH_CUDA(cudaGetLastError());
     return BH_OK;

@@ -36,4 +36,26 @@ __device__ __forceinline__ int common_levels(u64 a, u64 b)
 template <typename T> __device__ __forceinline__ T ld_stream(const T* p) { return __ldcs(p); }
 template <typename T> __device__ __forceinline__ void st_stream(T* p, T v) { __stcs(p, v); }
 
+// The cells in sorted order (ascending (key, original index)) as the sort leaves them:
+//   packed   : one u64 per cell = (key bits [lo, lo+32) << 32) | original index -- used whenever all
+//              varying key bits fit in 32 (every grid up to 1024^3 and the AMR workloads); cbits holds
+//              the key bits outside that window, which are the same for all cells;
+//   generic  : keys[] + idx[];
+//   identity : all keys equal, nothing was sorted: keys[] as generated, idx(s) = s.
+struct SortedView {
+    const u64* packed;
+    const u64* keys;
+    const u32* idx;
+    u64 cbits;
+    int lo;
+};
+__device__ __forceinline__ u64 sv_key(const SortedView& v, i64 s)
+{
+    return v.packed ? (((v.packed[s] >> 32) << v.lo) | v.cbits) : v.keys[s];
+}
+__device__ __forceinline__ u32 sv_idx(const SortedView& v, i64 s)
+{
+    return v.packed ? (u32)v.packed[s] : (v.idx ? v.idx[s] : (u32)s);
+}
+
 }  // namespace bh

@@ -3,7 +3,8 @@
 //   s = 2^21 / L (fp64, computed once on the host);  t = (v - v0) * s as one fp64 subtract and one
 //   fp64 multiply (round-to-nearest, NO fma contraction);  q = floor(t) clamped to [0, 2^21-1]
 //   (NaN -> 0);  key bit 3k+0/1/2 = bit k of qx/qy/qz.
-// HBM-bound stream: 24 B read + 12 B written per cell.
+// The permutation starts as the identity and is never stored: the first sort pass uses the element index.
+// HBM-bound stream: 24 B read + 8 B written per cell.
 #pragma once
 #include "common.cuh"
 
@@ -49,7 +50,7 @@ template <int VEC>
 __global__ void __launch_bounds__(256)
 morton_keys_kernel(const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
                    i64 n, double x0, double y0, double z0, double s,
-                   u64* __restrict__ keys, u32* __restrict__ idx, KeyReduce* __restrict__ red)
+                   u64* __restrict__ keys, KeyReduce* __restrict__ red)
 {
     u64 k_or = 0, k_and = ~0ULL;
     u32 n_cl = 0;
@@ -64,7 +65,6 @@ morton_keys_kernel(const double* __restrict__ x, const double* __restrict__ y, c
             u64 ka = morton_key(xx.x, yy.x, zz.x, x0, y0, z0, s, c0);
             u64 kb = morton_key(xx.y, yy.y, zz.y, x0, y0, z0, s, c1);
             reinterpret_cast<ulonglong2*>(keys)[v] = make_ulonglong2(ka, kb);
-            reinterpret_cast<uint2*>(idx)[v] = make_uint2((u32)(2 * v), (u32)(2 * v + 1));
             k_or |= ka | kb;
             k_and &= ka & kb;
             n_cl += c0 + c1;
@@ -73,7 +73,6 @@ morton_keys_kernel(const double* __restrict__ x, const double* __restrict__ y, c
             u32 c0 = 0;
             u64 ka = morton_key(x[n - 1], y[n - 1], z[n - 1], x0, y0, z0, s, c0);
             keys[n - 1] = ka;
-            idx[n - 1] = (u32)(n - 1);
             k_or |= ka; k_and &= ka; n_cl += c0;
         }
     } else {
@@ -81,7 +80,6 @@ morton_keys_kernel(const double* __restrict__ x, const double* __restrict__ y, c
             u32 c0 = 0;
             u64 ka = morton_key(x[i], y[i], z[i], x0, y0, z0, s, c0);
             keys[i] = ka;
-            idx[i] = (u32)i;
             k_or |= ka; k_and &= ka; n_cl += c0;
         }
     }

@@ -33,10 +33,14 @@ __device__ __forceinline__ u32 digit_peers(u32 d)
     return peers;
 }
 
+
+
 struct SortPlan {
     int npasses;
-    int shift[kMaxPasses];
+    int shift[kMaxPasses];           // bit position of each pass's digit in the 63-bit key
     u32 mask[kMaxPasses];
+    int lo;                          // lowest varying key bit
+    bool packed;                     // all varying bits inside [lo, lo + 32)
 };
 
 // ghist[p * pass_stride + d] = number of keys whose digit of pass p is d
@@ -80,22 +84,34 @@ radix_hist_strided_kernel(const u64* __restrict__ keys, i64 n, const SortPlan pl
 struct SortSmem {
     u32 klo[kSortTile];              // 16 KB  } the tile in digit order; slot q lives at swz(q), which
     u32 khi[kSortTile];              // 16 KB  } keeps power-of-two strides (digit starts) off one bank
-    u32 vals[kSortTile];             // 16 KB
     u32 wcnt[kSortThreads / 32][kRadix];   // 8 KB: per-warp digit counts, then per-warp digit offsets
     u32 dstart[kRadix];              // tile-local start of each digit
     u32 gbase[kRadix];               // global position of local slot q of digit d is gbase[d] + q
     u32 s_warp[9];
     u32 s_tile;
 };
+struct SortSmemVals { u32 vals[kSortTile]; };    // generic mode only: the values, behind SortSmem
+
+// What one pass reads and writes.
+//   kGenericFirst: reads keys, value = element index;  writes (key, value)
+//   kGeneric     : reads (key, value);                 writes (key, value)
+//   kPackedFirst : reads keys;  writes words (key bits [lo, lo+32) << 32 | element index)
+//   kPacked      : reads words; writes words
+enum SortMode { kGenericFirst = 0, kGeneric = 1, kPackedFirst = 2, kPacked = 3 };
 
 // One pass.  status[tile * 256 + d]: flag (bits 31..30) | count (30 bits); ticket: next tile to hand out.
-__global__ void __launch_bounds__(kSortThreads, 3)
+// `shift` addresses the digit inside the element this pass ranks on: the u64 key (generic modes and
+// kPackedFirst, which ranks on the raw key) or the packed word (kPacked).
+template <int MODE>
+__global__ void __launch_bounds__(kSortThreads, (MODE >= kPackedFirst ? 4 : 3))
 radix_onesweep_kernel(const u64* __restrict__ kin, const u32* __restrict__ vin, u64* __restrict__ kout,
                       u32* __restrict__ vout, const u32* __restrict__ ghist /* this pass: [256] */,
-                      u32* __restrict__ status, u32* __restrict__ ticket, i64 n, int shift, u32 mask)
+                      u32* __restrict__ status, u32* __restrict__ ticket, i64 n, int shift, u32 mask, int lo)
 {
+    constexpr bool kVals = MODE == kGenericFirst || MODE == kGeneric;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     SortSmem& S = *reinterpret_cast<SortSmem*>(smem_raw);
+    u32* svals = reinterpret_cast<SortSmemVals*>(smem_raw + sizeof(SortSmem))->vals;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     if (tid == 0) S.s_tile = atomicAdd(ticket, 1u);
     for (int i = tid; i < (kSortThreads / 32) * kRadix; i += kSortThreads) (&S.wcnt[0][0])[i] = 0;
@@ -105,20 +121,18 @@ radix_onesweep_kernel(const u64* __restrict__ kin, const u32* __restrict__ vin, 
 
     // warp-striped load: warp w owns the contiguous chunk [w*512, w*512+512) of the tile
     u64 key[kSortItems];
-    u32 val[kSortItems];
     u32 rank[kSortItems];
     const i64 wbase = base + (i64)warp * (32 * kSortItems);
     #pragma unroll
     for (int i = 0; i < kSortItems; ++i) {
         const i64 e = wbase + i * 32 + lane;
-        const bool ok = e < n;
-        key[i] = ok ? ld_stream(kin + e) : ~0ULL;
+        key[i] = e < n ? ld_stream(kin + e) : ~0ULL;       // padding takes the top digit, last in the tile
     }
     // stable rank inside the warp chunk: items are visited in memory order
-    const u32 lt = lanemask_lt();
+    const u32 lt = (1u << lane) - 1u;
     #pragma unroll
     for (int i = 0; i < kSortItems; ++i) {
-        const u32 d = (u32)(key[i] >> shift) & mask;     // padding keys (~0) take the top digit, last
+        const u32 d = (u32)(key[i] >> shift) & mask;
         const u32 peers = digit_peers(d);
         const u32 cnt = S.wcnt[warp][d];
         __syncwarp();
@@ -127,10 +141,13 @@ radix_onesweep_kernel(const u64* __restrict__ kin, const u32* __restrict__ vin, 
         __syncwarp();
         rank[i] = cnt + r;
     }
-    #pragma unroll
-    for (int i = 0; i < kSortItems; ++i) {       // the values arrive while the digit offsets are worked out
-        const i64 e = wbase + i * 32 + lane;
-        val[i] = e < n ? ld_stream(vin + e) : 0u;
+    u32 val[kVals ? kSortItems : 1];
+    if (MODE == kGeneric) {
+        #pragma unroll
+        for (int i = 0; i < kSortItems; ++i) {   // the values arrive while the digit offsets are worked out
+            const i64 e = wbase + i * 32 + lane;
+            val[i] = e < n ? ld_stream(vin + e) : 0u;
+        }
     }
     __syncthreads();
     {   // thread d: exclusive scan of digit d over the warps, then over the digits
@@ -164,21 +181,29 @@ radix_onesweep_kernel(const u64* __restrict__ kin, const u32* __restrict__ vin, 
         const u32 d = (u32)(key[i] >> shift) & mask;
         const u32 q = S.dstart[d] + S.wcnt[warp][d] + rank[i];
         const u32 qs = q ^ ((q >> 5) & 31u);
-        S.klo[qs] = (u32)key[i];
-        S.khi[qs] = (u32)(key[i] >> 32);
-        S.vals[qs] = val[i];
+        const u32 e32 = (u32)(wbase + i * 32 + lane);
+        if (MODE == kPackedFirst) {                         // word = key window | element index
+            S.klo[qs] = e32;
+            S.khi[qs] = (u32)(key[i] >> lo);
+        } else {
+            S.klo[qs] = (u32)key[i];
+            S.khi[qs] = (u32)(key[i] >> 32);
+        }
+        if (MODE == kGenericFirst) svals[qs] = e32;
+        if (MODE == kGeneric) svals[qs] = val[i];
     }
     __syncthreads();
     const i64 left = n - base;
     const int nvalid = left < kSortTile ? (int)left : kSortTile;
+    const int dshift = MODE == kPackedFirst ? shift - lo + 32 : shift;   // the digit inside what was stored
     #pragma unroll 4
     for (int q = tid; q < nvalid; q += kSortThreads) {
         const u32 qs = (u32)q ^ (((u32)q >> 5) & 31u);
         const u64 k = ((u64)S.khi[qs] << 32) | S.klo[qs];
-        const u32 d = (u32)(k >> shift) & mask;
+        const u32 d = (u32)(k >> dshift) & mask;
         const u32 g = S.gbase[d] + (u32)q;
         kout[g] = k;
-        vout[g] = S.vals[qs];
+        if (kVals) vout[g] = svals[qs];
     }
 }
 
@@ -187,8 +212,12 @@ inline SortPlan make_sort_plan(u64 varying)
 {
     SortPlan p;
     p.npasses = 0;
+    p.lo = 0;
+    p.packed = false;
     if (varying == 0) return p;
     int lo = __builtin_ctzll(varying), hi = 63 - __builtin_clzll(varying);
+    p.lo = lo;
+    p.packed = hi - lo + 1 <= 32;
     for (int b = lo; b <= hi; b += 8) {
         int w = hi - b + 1 < 8 ? hi - b + 1 : 8;
         p.shift[p.npasses] = b;
@@ -202,9 +231,12 @@ inline i64 sort_tiles(i64 n) { return (n + kSortTile - 1) / kSortTile; }
 // u32 words of sort scratch: per pass [256 histogram][ntiles * 256 status][1 ticket]
 inline size_t sort_pass_words(i64 n) { return (size_t)kRadix + (size_t)sort_tiles(n) * kRadix + 1; }
 inline size_t sort_hist_elems(i64 n) { return (size_t)kMaxPasses * sort_pass_words(n); }
+inline size_t sort_smem_bytes(bool packed) { return sizeof(SortSmem) + (packed ? 0 : sizeof(SortSmemVals)); }
 
-// Sorts (k0, v0) in plan.npasses passes, ping-ponging with (k1, v1); the result is in (k0, v0) for an even
-// number of passes, else in (k1, v1).  scratch holds plan.npasses * sort_pass_words(n) u32.
+// Sorts the n keys in k0 (values = their indices 0..n-1, implicit) in plan.npasses >= 1 passes, ping-ponging
+// between (k0, v0) and (k1, v1); pass p writes to buffer 1 if p is even, else to buffer 0, so the result
+// is in buffer (npasses & 1).  Packed plans never touch v0 / v1 (may be null).
+// scratch holds plan.npasses * sort_pass_words(n) u32.
 inline cudaError_t radix_sort_pairs(u64* k0, u32* v0, u64* k1, u32* v1, i64 n, const SortPlan& plan, u32* scratch,
                                     int hist_grid, cudaStream_t st)
 {
@@ -214,12 +246,27 @@ inline cudaError_t radix_sort_pairs(u64* k0, u32* v0, u64* k1, u32* v1, i64 n, c
     cudaError_t e = cudaMemsetAsync(scratch, 0, sizeof(u32) * pw * plan.npasses, st);
     if (e != cudaSuccess) return e;
     // all histograms in one read; each pass's 256 counters sit at the head of its scratch block
-    SortPlan hp = plan;
-    radix_hist_strided_kernel<<<hist_grid, kSortThreads, 0, st>>>(k0, n, hp, scratch, (u32)pw);
+    radix_hist_strided_kernel<<<hist_grid, kSortThreads, 0, st>>>(k0, n, plan, scratch, (u32)pw);
+    const size_t smem = sort_smem_bytes(plan.packed);
     for (int p = 0; p < plan.npasses; ++p) {
         u32* blk = scratch + pw * p;
-        radix_onesweep_kernel<<<ntiles, kSortThreads, sizeof(SortSmem), st>>>(
-            k0, v0, k1, v1, blk, blk + kRadix, blk + kRadix + (size_t)ntiles * kRadix, n, plan.shift[p], plan.mask[p]);
+        u32* status = blk + kRadix;
+        u32* ticket = status + (size_t)ntiles * kRadix;
+        if (plan.packed) {
+            if (p == 0)
+                radix_onesweep_kernel<kPackedFirst><<<ntiles, kSortThreads, smem, st>>>(
+                    k0, nullptr, k1, nullptr, blk, status, ticket, n, plan.shift[p], plan.mask[p], plan.lo);
+            else   // the key window sits in the upper half of the word
+                radix_onesweep_kernel<kPacked><<<ntiles, kSortThreads, smem, st>>>(
+                    k0, nullptr, k1, nullptr, blk, status, ticket, n, plan.shift[p] - plan.lo + 32, plan.mask[p], plan.lo);
+        } else {
+            if (p == 0)
+                radix_onesweep_kernel<kGenericFirst><<<ntiles, kSortThreads, smem, st>>>(
+                    k0, nullptr, k1, v1, blk, status, ticket, n, plan.shift[p], plan.mask[p], plan.lo);
+            else
+                radix_onesweep_kernel<kGeneric><<<ntiles, kSortThreads, smem, st>>>(
+                    k0, v0, k1, v1, blk, status, ticket, n, plan.shift[p], plan.mask[p], plan.lo);
+        }
         u64* tk = k0; k0 = k1; k1 = tk;
         u32* tv = v0; v0 = v1; v1 = tv;
     }

@@ -56,7 +56,7 @@ __device__ __forceinline__ void entity_masks(int cp, int cs, u32& imask, u32& em
 //                            d >= kSlotLevels: internal nodes of level d - kSlotLevels.
 // 8 B read + 1 B written per cell.
 __global__ void __launch_bounds__(kTopoThreads)
-topo_count_kernel(const u64* __restrict__ keys, i64 n, signed char* __restrict__ clev, u32* __restrict__ hist,
+topo_count_kernel(const SortedView sv, i64 n, signed char* __restrict__ clev, u32* __restrict__ hist,
                   i64 nchunks)
 {
     __shared__ u32 h[kTopoThreads / 32][kTopoDigits + 3];
@@ -68,7 +68,7 @@ topo_count_kernel(const u64* __restrict__ keys, i64 n, signed char* __restrict__
     for (int d = lane; d < kTopoDigits; d += 32) hw[d] = 0u;
     __syncwarp();
     const i64 wbase = chunk * kTopoChunk;
-    int carry = wbase > 0 ? common_levels(__ldg(keys + wbase - 1), __ldg(keys + wbase)) : -1;   // c(wbase - 1)
+    int carry = wbase > 0 ? common_levels(sv_key(sv, wbase - 1), sv_key(sv, wbase)) : -1;   // c(wbase - 1)
     constexpr int kBatch = 4;                           // rows whose loads are in flight together
     static_assert(kTopoItems % kBatch == 0, "rows per chunk");
     for (int i0 = 0; i0 < kTopoItems; i0 += kBatch) {
@@ -77,8 +77,8 @@ topo_count_kernel(const u64* __restrict__ keys, i64 n, signed char* __restrict__
         #pragma unroll
         for (int r = 0; r < kBatch; ++r) {
             const i64 s = wbase + 32 * (i0 + r) + lane;
-            k[r] = s < n ? ld_stream(keys + s) : 0ULL;
-            kn[r] = (lane == 31 && s + 1 < n) ? __ldg(keys + s + 1) : 0ULL;   // lane 31's successor
+            k[r] = s < n ? sv_key(sv, s) : 0ULL;
+            kn[r] = (lane == 31 && s + 1 < n) ? sv_key(sv, s + 1) : 0ULL;   // lane 31's successor
         }
         #pragma unroll
         for (int r = 0; r < kBatch; ++r) {
@@ -129,7 +129,7 @@ __global__ void topo_totals_kernel(const u32* __restrict__ scanned, i64 nchunks,
 // the canonical id of its first level-l node.  Per cell: 4 B idx + 1 B c + 32 B gathered; written
 // 4 B slot + 32 B fp64 record + 16 B fp32 record + 16 B aux; per node 12 B.
 __global__ void __launch_bounds__(kTopoThreads)
-topo_assign_kernel(const signed char* __restrict__ clev, i64 n, const u32* __restrict__ idx,
+topo_assign_kernel(const signed char* __restrict__ clev, i64 n, const SortedView sv,
                    const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
                    const double* __restrict__ m, const u32* __restrict__ scanned, i64 nchunks, u32 nslots,
                    u32* __restrict__ leaf_slot, u32* __restrict__ node_slot, u32* __restrict__ nfirst,
@@ -151,7 +151,7 @@ topo_assign_kernel(const signed char* __restrict__ clev, i64 n, const u32* __res
     #pragma unroll
     for (int i = 0; i < kTopoItems; ++i) {
         const i64 s = wbase + 32 * i + lane;
-        oi[i] = s < n ? ld_stream(idx + s) : 0u;
+        oi[i] = s < n ? sv_idx(sv, s) : 0u;
         ci[i] = s < n ? (int)clev[s] : -1;
     }
     #pragma unroll
@@ -207,16 +207,16 @@ topo_assign_kernel(const signed char* __restrict__ clev, i64 n, const u32* __res
 }
 
 // first index in [a, hi) whose key is >= limit (hi if none); gallops from a
-__device__ __forceinline__ i64 gallop_lower_bound(const u64* __restrict__ keys, i64 a, i64 hi, u64 limit)
+__device__ __forceinline__ i64 gallop_lower_bound(const SortedView& sv, i64 a, i64 hi, u64 limit)
 {
-    if (a >= hi || keys[a] >= limit) return a;
+    if (a >= hi || sv_key(sv, a) >= limit) return a;
     i64 lo = a;                 // keys[lo] < limit
     i64 step = 1;
-    while (lo + step < hi && keys[lo + step] < limit) { lo += step; step <<= 1; }
+    while (lo + step < hi && sv_key(sv, lo + step) < limit) { lo += step; step <<= 1; }
     i64 up = lo + step < hi ? lo + step : hi;   // keys[up] >= limit or up == hi
     while (up - lo > 1) {
         const i64 mid = lo + ((up - lo) >> 1);
-        if (keys[mid] < limit) lo = mid; else up = mid;
+        if (sv_key(sv, mid) < limit) lo = mid; else up = mid;
     }
     return up;
 }
@@ -236,14 +236,14 @@ __device__ __forceinline__ u32 compact3(u64 v)   // inverse of the key bit-sprea
 // Node b of level `level`: children = slots [nfirst[b], nfirst[b+1]) (the last node of the level ends at
 // slot_end, the end of the level-(level+1) slots).  Reads 32 B per child, writes 80 B per node.
 struct MomentArgs {
-    const u64* keys; const u32* nlo; const u32* nfirst; const u32* node_slot;
+    SortedView sv; const u32* nlo; const u32* nfirst; const u32* node_slot;
     double4* rec64; double* delta64; float4* rec; WalkAux* aux; u32* max_bucket;
     double x0, y0, z0, L;
 };
 
 __device__ __forceinline__ void moments_node(i64 b, i64 b1, int level, u32 slot_end, const MomentArgs& A)
 {
-    const u64* keys = A.keys; const u32* nlo = A.nlo; const u32* nfirst = A.nfirst; const u32* node_slot = A.node_slot;
+    const u32* nlo = A.nlo; const u32* nfirst = A.nfirst; const u32* node_slot = A.node_slot;
     double4* rec64 = A.rec64; double* delta64 = A.delta64; float4* rec = A.rec; WalkAux* aux = A.aux;
     u32* max_bucket = A.max_bucket;
     const double x0 = A.x0, y0 = A.y0, z0 = A.z0, L = A.L;
@@ -259,7 +259,7 @@ __device__ __forceinline__ void moments_node(i64 b, i64 b1, int level, u32 slot_
         Sz = __dadd_rn(Sz, __dmul_rn(zm.y, zm.x));
     }
     const double size = ldexp(L, -level);
-    const u64 prefix = level == 0 ? 0ULL : keys[nlo[b]] >> (3 * (kMaxLevel - level));
+    const u64 prefix = level == 0 ? 0ULL : sv_key(A.sv, nlo[b]) >> (3 * (kMaxLevel - level));
     const double cx = __dadd_rn(x0, __dmul_rn((double)compact3(prefix) + 0.5, size));
     const double cy = __dadd_rn(y0, __dmul_rn((double)compact3(prefix >> 1) + 0.5, size));
     const double cz = __dadd_rn(z0, __dmul_rn((double)compact3(prefix >> 2) + 0.5, size));
@@ -320,7 +320,7 @@ struct TopoLevels {               // host-computed from the scanned histogram
 
 // ---- export (parity only): the nodes in canonical order ------------------------------------------
 __global__ void __launch_bounds__(256)
-export_nodes_kernel(i64 nn, i64 n, const TopoLevels lv, const u64* __restrict__ keys, const u32* __restrict__ nlo,
+export_nodes_kernel(i64 nn, i64 n, const TopoLevels lv, const SortedView sv, const u32* __restrict__ nlo,
                     const u32* __restrict__ nfirst, const u32* __restrict__ node_slot,
                     const double4* __restrict__ rec64, const double* __restrict__ delta64,
                     int* level, u64* prefix, i64* lo, i64* hi, int* nch, double* M, double* Rx, double* Ry,
@@ -332,13 +332,13 @@ export_nodes_kernel(i64 nn, i64 n, const TopoLevels lv, const u64* __restrict__ 
     while (l + 1 < kNumLevels && (i64)lv.node_base[l + 1] <= b) ++l;
     const i64 s = nlo[b];
     if (level) level[b] = l;
-    if (prefix) prefix[b] = l == 0 ? 0ULL : keys[s] >> (3 * (kMaxLevel - l));
+    if (prefix) prefix[b] = l == 0 ? 0ULL : sv_key(sv, s) >> (3 * (kMaxLevel - l));
     if (lo) lo[b] = s;
     if (hi) {
         if (l == 0) hi[b] = n;
         else {
             const int sh = 3 * (kMaxLevel - l);
-            hi[b] = gallop_lower_bound(keys, s + 1, n, ((keys[s] >> sh) + 1ULL) << sh);
+            hi[b] = gallop_lower_bound(sv, s + 1, n, ((sv_key(sv, s) >> sh) + 1ULL) << sh);
         }
     }
     if (nch) nch[b] = (int)((b + 1 < (i64)lv.node_base[l + 1] ? nfirst[b + 1] : lv.slot_base[l + 2]) - nfirst[b]);
@@ -352,14 +352,24 @@ export_nodes_kernel(i64 nn, i64 n, const TopoLevels lv, const u64* __restrict__ 
 
 // ---- bh_potential_direct's own copies (built on its first call after a build, not on the hot path) --
 __global__ void __launch_bounds__(256)
-direct_prepare_kernel(const u32* __restrict__ idx, const u32* __restrict__ leaf_slot,
+direct_prepare_kernel(const SortedView sv, const u32* __restrict__ leaf_slot,
                       const double4* __restrict__ rec64, i64 n, double4* __restrict__ leaf64,
                       u32* __restrict__ slot_of)
 {
     const i64 s = (i64)blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n) return;
     leaf64[s] = rec64[leaf_slot[s]];
-    slot_of[idx[s]] = (u32)s;
+    slot_of[sv_idx(sv, s)] = (u32)s;
+}
+
+// sorted keys and permutation as plain arrays (bh_export_tree)
+__global__ void __launch_bounds__(256)
+export_sorted_kernel(const SortedView sv, i64 n, u64* __restrict__ keys, u32* __restrict__ perm)
+{
+    const i64 s = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    if (keys) keys[s] = sv_key(sv, s);
+    if (perm) perm[s] = sv_idx(sv, s);
 }
 
 }  // namespace bh

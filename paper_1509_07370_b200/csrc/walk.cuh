@@ -46,7 +46,7 @@ struct WalkParams {
     const float4* rec;        // [n_slots] (x, y, z, m) of every node / leaf-cell slot
     const WalkAux* aux;       // [n_slots]
     const u32* leaf_slot;     // [n] slot of sorted cell s (the targets are read from rec)
-    const u32* idx;           // [n] original index of sorted slot
+    SortedView sv;            // sorted cells: original index of sorted slot s
     double* phi;              // [n] original order
     uint4* gcount;            // [ngroups] {accepted, leaf, opened, exact-tested}
     i64 n;
@@ -408,8 +408,8 @@ walk_pair_kernel(const WalkParams P)
     }
     if (nC > 0) eval_c(C, Cm, nC, npx, npy, npz, accA, accB);
     // ---- a7: Phi_t = -G * sum, written in the original cell order (W-rule 4) ----
-    if (liveA) P.phi[__ldg(P.idx + sA)] = P.negG * accA;
-    if (liveB) P.phi[__ldg(P.idx + sB)] = P.negG * accB;
+    if (liveA) P.phi[sv_idx(P.sv, sA)] = P.negG * accA;
+    if (liveB) P.phi[sv_idx(P.sv, sB)] = P.negG * accB;
 }
 
 // ---- BH_OPT_GROUP = 1 (W5): every target walks alone --------------------------------------------
@@ -460,7 +460,7 @@ walk_single_kernel(const WalkParams P)
         }
     }
     acc += (double)part;
-    P.phi[__ldg(P.idx + s)] = P.negG * acc;
+    P.phi[sv_idx(P.sv, s)] = P.negG * acc;
     P.gcount[s] = make_uint4(c_acc, c_leaf, c_open, 0u);
 }
 
@@ -475,13 +475,13 @@ group_counts_export_kernel(const uint4* __restrict__ gcount, i64 ngroups, i64* _
 }
 
 __global__ void __launch_bounds__(256)
-per_target_counts_kernel(const uint4* __restrict__ gcount, const u32* __restrict__ idx, i64 n, int group,
+per_target_counts_kernel(const uint4* __restrict__ gcount, const SortedView sv, i64 n, int group,
                          u32* __restrict__ out)
 {
     const i64 s = (i64)blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n) return;
     const uint4 c = gcount[s / group];
-    out[idx[s]] = c.x + c.y;
+    out[sv_idx(sv, s)] = c.x + c.y;
 }
 
 // totals[0..3] = sum of the four group counters; totals[4] = sum over targets of (acc + leaf)
