@@ -58,4 +58,16 @@ __device__ __forceinline__ u32 sv_idx(const SortedView& v, i64 s)
     return v.packed ? (u32)v.packed[s] : (v.idx ? v.idx[s] : (u32)s);
 }
 
+// c(s): octree levels the keys of sorted cells s and s+1 share (s + 1 < n).  In the packed form only the
+// 32-bit key windows differ, so the highest differing key bit is lo + 31 - clz(xor of the windows).
+__device__ __forceinline__ int sv_common_levels(const SortedView& v, i64 s)
+{
+    if (v.packed) {
+        const u32* w = reinterpret_cast<const u32*>(v.packed);
+        const u32 x = w[2 * s + 1] ^ w[2 * s + 3];
+        return x == 0u ? kMaxLevel : (31 + __clz((int)x) - v.lo) / 3;     // (62 - (lo + 31 - clz)) / 3
+    }
+    return common_levels(v.keys[s], v.keys[s + 1]);
+}
+
 }  // namespace bh

@@ -66,10 +66,11 @@ radix_hist_strided_kernel(const u64* __restrict__ keys, i64 n, const SortPlan pl
             for (int p = 0; p < kMaxPasses; ++p) {      // static indices keep the plan in constant memory
                 if (p >= plan.npasses) break;
                 const u32 d = (u32)(k[r] >> plan.shift[p]) & plan.mask[p];
-                const u32 d0 = __shfl_sync(0xffffffffu, d, 0);
                 // neighbouring cells mostly share their upper digits: one atomic for the whole row then
-                if (vmask == 0xffffffffu && __all_sync(0xffffffffu, d == d0)) {
-                    if (lane == 0) atomicAdd(&h[p * kRadix + d0], 32u);
+                int same;
+                __match_all_sync(0xffffffffu, d, &same);
+                if (same && vmask == 0xffffffffu) {
+                    if (lane == 0) atomicAdd(&h[p * kRadix + d], 32u);
                 } else if (valid) {
                     atomicAdd(&h[p * kRadix + d], 1u);
                 }

@@ -68,28 +68,48 @@ topo_count_kernel(const SortedView sv, i64 n, signed char* __restrict__ clev, u3
     for (int d = lane; d < kTopoDigits; d += 32) hw[d] = 0u;
     __syncwarp();
     const i64 wbase = chunk * kTopoChunk;
-    int carry = wbase > 0 ? common_levels(sv_key(sv, wbase - 1), sv_key(sv, wbase)) : -1;   // c(wbase - 1)
-    constexpr int kBatch = 4;                           // rows whose loads are in flight together
-    static_assert(kTopoItems % kBatch == 0, "rows per chunk");
-    for (int i0 = 0; i0 < kTopoItems; i0 += kBatch) {
-        if (wbase + 32 * i0 >= n) break;
-        u64 k[kBatch], kn[kBatch];
+    // c(s) of the chunk's cells: every load is issued before the first use (indices clamped, results
+    // masked), so a warp has its whole chunk in flight at once
+    int c[kTopoItems];
+    int cprev;                                        // c(wbase - 1)
+    const i64 last = n - 1;
+    if (sv.packed) {
+        const u32* w = reinterpret_cast<const u32*>(sv.packed);
+        u32 x[kTopoItems];
         #pragma unroll
-        for (int r = 0; r < kBatch; ++r) {
-            const i64 s = wbase + 32 * (i0 + r) + lane;
-            k[r] = s < n ? sv_key(sv, s) : 0ULL;
-            kn[r] = (lane == 31 && s + 1 < n) ? sv_key(sv, s + 1) : 0ULL;   // lane 31's successor
+        for (int i = 0; i < kTopoItems; ++i) {
+            const i64 s = wbase + 32 * i + lane;
+            const i64 s0 = s < last ? s : last, s1 = s + 1 < last ? s + 1 : last;
+            x[i] = w[2 * s0 + 1] ^ w[2 * s1 + 1];
         }
+        const u32 xp = wbase > 0 ? (w[2 * wbase - 1] ^ w[2 * wbase + 1]) : 0u;
         #pragma unroll
-        for (int r = 0; r < kBatch; ++r) {
-            const i64 s = wbase + 32 * (i0 + r) + lane;
+        for (int i = 0; i < kTopoItems; ++i) c[i] = x[i] == 0u ? kMaxLevel : (31 + __clz((int)x[i]) - sv.lo) / 3;
+        cprev = xp == 0u ? kMaxLevel : (31 + __clz((int)xp) - sv.lo) / 3;
+    } else {
+        u64 x[kTopoItems];
+        #pragma unroll
+        for (int i = 0; i < kTopoItems; ++i) {
+            const i64 s = wbase + 32 * i + lane;
+            const i64 s0 = s < last ? s : last, s1 = s + 1 < last ? s + 1 : last;
+            x[i] = sv.keys[s0] ^ sv.keys[s1];
+        }
+        const u64 xp = wbase > 0 ? (sv.keys[wbase - 1] ^ sv.keys[wbase]) : 0ULL;
+        #pragma unroll
+        for (int i = 0; i < kTopoItems; ++i) c[i] = x[i] == 0ULL ? kMaxLevel : (__clzll((long long)x[i]) - 1) / 3;
+        cprev = xp == 0ULL ? kMaxLevel : (__clzll((long long)xp) - 1) / 3;
+    }
+    if (wbase == 0) cprev = -1;
+    #pragma unroll
+    for (int i = 0; i < kTopoItems; ++i) {
+        if (wbase + 32 * i >= n) break;
+        {
+            const i64 s = wbase + 32 * i + lane;
             const bool valid = s < n;
-            const u64 nx = __shfl_down_sync(0xffffffffu, k[r], 1);
-            if (lane != 31) kn[r] = nx;
-            const int cs = (valid && s + 1 < n) ? common_levels(k[r], kn[r]) : -1;
+            const int cs = (valid && s + 1 < n) ? c[i] : -1;
             int cp = __shfl_up_sync(0xffffffffu, cs, 1);
-            if (lane == 0) cp = carry;
-            carry = __shfl_sync(0xffffffffu, cs, 31);
+            if (lane == 0) cp = cprev;
+            cprev = __shfl_sync(0xffffffffu, cs, 31);
             if (valid) clev[s] = (signed char)cs;
             // leaf entity: usually the same level for the whole row -> one shared atomic
             const int leafL = valid ? (cp > cs ? cp : cs) + 1 : -1;
@@ -137,7 +157,7 @@ topo_assign_kernel(const signed char* __restrict__ clev, i64 n, const SortedView
                    WalkAux* __restrict__ aux)
 {
     const u32 lane = lane_id();
-    const u32 lt = lanemask_lt();
+    const u32 lt = (1u << lane) - 1u;
     const i64 chunk = (i64)blockIdx.x * (kTopoThreads / 32) + (threadIdx.x >> 5);
     if (chunk >= nchunks) return;
     const i64 wbase = chunk * kTopoChunk;
