@@ -177,6 +177,7 @@ def run_ours(args):
     import torch
     import bh_workloads as wl
     import paper_1509_07370_b200 as bh
+    from paper_1509_07370_b200 import ranks
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -230,10 +231,7 @@ def run_ours(args):
     dev_total = ev[0][0].elapsed_time(ev[-1][2]) / 1e3          # device time first event -> last event
     t_build = sum(e[0].elapsed_time(e[1]) for e in ev) / args.steps / 1e3
     t_walk = sum(e[1].elapsed_time(e[2]) for e in ev) / args.steps / 1e3
-    t = torch.tensor([dev_total, elapsed], dtype=torch.float64, device=dev)
-    if dist:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    dev_total, elapsed = float(t[0]), float(t[1])
+    dev_total, elapsed, t_build, t_walk = ranks.max_over_ranks([dev_total, elapsed, t_build, t_walk], dev)
     st = ctx.get_stats()
 
     # ---- e2e: the public host-buffer call, copies inside the timed region ----
@@ -249,10 +247,7 @@ def run_ours(args):
         ctx.solve_host(hx[0], hx[1], hx[2], hx[3], w.cube, w.theta, w.G, out=phi_host.numpy())
     torch.cuda.synchronize()
     e2e_t = time.perf_counter() - t1
-    te = torch.tensor([e2e_t], dtype=torch.float64, device=dev)
-    if dist:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_t = float(te[0])
+    e2e_t = ranks.max_over_ranks([e2e_t], dev)[0]
 
     if rank != 0:
         if dist:
@@ -264,7 +259,7 @@ def run_ours(args):
     walk_tflops = inter * FLOPS_PER_INTERACTION / t_walk / 1e12
     bpc = build_bytes_per_cell(n, st.n_nodes, st.sort_passes)
     line = {
-        "metric": "cells_per_s_build_plus_walk", "value": world * n * args.steps / dev_total, "unit": "cells/s",
+        "metric": "cells_per_s_build_plus_walk", "value": ranks.whole_job_rate(n, args.steps, dev_total, world), "unit": "cells/s",
         "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": dev_total / args.steps * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": w.name, "n_cells": n, "theta": w.theta, "group": 32, "mac": "eq3", "G": w.G,
@@ -279,14 +274,15 @@ def run_ours(args):
         "tree": {"n_nodes": st.n_nodes, "depth": st.depth, "sort_passes": st.sort_passes,
                  "exact_tests_per_group": st.n_exact_tests / ((n + 31) // 32)},
         "roofline": {"bound": "alu", "kernel": "walk_pair_kernel<false>", "achieved": walk_tflops, "peak": fp32_peak_tflops,
-                     "unit": "TFLOP/s", "frac": walk_tflops / fp32_peak_tflops, "traffic": None,
+                     "unit": "TFLOP/s", "frac": walk_tflops / fp32_peak_tflops, "traffic": walk_traffic(w.name, w.theta),
+                     "launch_ms": t_walk * 1e3, "flops_per_launch": inter * FLOPS_PER_INTERACTION,
                      "peak_source": "nominal FP32: %d SMs x 128 lanes x 2 x %.0f MHz (sm_max_mhz, MEASURED_PEAKS.json %s); "
                                     "13 flops/interaction" % (st_sms(local), sm_max_mhz, peak_src),
                      "build_hbm": {"achieved": bpc * n / t_build / 1e9, "peak": hbm_gbs, "unit": "GB/s",
                                    "frac": bpc * n / t_build / 1e9 / hbm_gbs, "bytes_per_cell": bpc,
                                    "peak_source": peak_src}},
         "clocks": clocks,
-        "e2e": {"value": world * n * e2e_steps / e2e_t, "unit": "cells/s", "h2d_bytes_per_step": 4 * 8 * n,
+        "e2e": {"value": ranks.whole_job_rate(n, e2e_steps, e2e_t, world), "unit": "cells/s", "h2d_bytes_per_step": 4 * 8 * n,
                 "d2h_bytes_per_step": 8 * n, "steps": e2e_steps, "api": "bh_solve_host (pinned host buffers)"},
         "gpu_launches": launches_per_step * args.steps,
     }
@@ -305,6 +301,20 @@ def run_ours(args):
     if dist:
         dist.destroy_process_group()
     return 0
+
+
+def walk_traffic(workload, theta):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one walk launch from the committed ncu --set full capture
+    (profiles/walk_traffic.csv), if one was taken on this workload; else None."""
+    import csv
+    try:
+        with open(os.path.join(ROOT, "profiles", "walk_traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == workload and abs(float(row["theta"]) - theta) < 1e-12:
+                    return float(row["dram_bytes_per_launch"])
+    except Exception:
+        pass
+    return None
 
 
 def st_sms(index):

@@ -1,0 +1,156 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times.
+
+The oracle cannot walk 16.8 M targets in seconds, so per workload: Morton keys, permutation and tree
+topology are compared in full (the oracle's build takes seconds), node moments in full, and Phi plus
+the per-group interaction counters on sampled runs of groups the oracle walks one by one (groups are
+independent given the tree, so parity on a sample is exact for that sample).  Configs 0 and 1 are
+also held against the closed forms the paper uses (§4.1), config 4 is the
+opening-angle sweep with the direct-sum-on-subsample error.
+"""
+import numpy as np
+import pytest
+
+import bh_workloads as wl
+from tests import analytic
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def bh():
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import paper_1509_07370_b200 as pkg
+    return pkg
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).cuda()
+
+
+def _build(bh, w):
+    ctx = bh.Context(0)
+    ctx.build(_dev(w.x), _dev(w.y), _dev(w.z), _dev(w.m), w.cube)
+    return ctx
+
+
+def _sample_runs(ngroups, nruns, per):
+    """`nruns` evenly spaced runs of `per` consecutive groups, first and last group included."""
+    per = min(per, ngroups)
+    starts = np.unique(np.linspace(0, ngroups - per, nruns).astype(np.int64))
+    return [(int(s), int(s) + per) for s in starts]
+
+
+def _check_sampled(ctx, ot, w, theta, mac=0, nruns=12, per=24, max_tol=1e-4, med_tol=1e-6):
+    """Phi and the (accepted, leaf, opened) counters of sampled groups against the oracle."""
+    ctx.set_mac(mac)
+    phi = ctx.potential(theta, w.G).cpu().numpy()
+    cnt = ctx.last_group_counts().cpu().numpy()
+    perm = ot.sorted_keys_perm()[1].astype(np.int64)
+    ngroups = (w.n + 31) // 32
+    rels, flips, ngr = [], 0, 0
+    buf = np.full(w.n, np.nan)
+    for g0, g1 in _sample_runs(ngroups, nruns, per):
+        _, ocnt = ot.potential(theta, w.G, mac=mac, group=32, mac_fp32=True, groups=(g0, g1), want_counts=True,
+                               out=buf)
+        flips += int(np.sum(np.any(cnt[g0:g1] != ocnt, axis=1)))
+        ngr += g1 - g0
+        tg = perm[32 * g0:min(32 * g1, w.n)]
+        ref = buf[tg]
+        ok = ref != 0
+        rels.append(np.abs(phi[tg][ok] - ref[ok]) / np.abs(ref[ok]))
+    rel = np.concatenate(rels)
+    assert flips == 0, f"{flips} of {ngr} sampled groups differ in (accepted, leaf, opened)"
+    assert rel.max() <= max_tol, f"max rel {rel.max():.3e}"
+    assert np.median(rel) <= med_tol, f"median rel {np.median(rel):.3e}"
+    return phi, cnt
+
+
+def _check_tree(ctx, ot, w):
+    t = {k: v.cpu().numpy() for k, v in ctx.export_tree().items()}
+    ok, op = ot.sorted_keys_perm()
+    assert np.array_equal(t["keys"].view(np.uint64), ok), "Morton keys differ"
+    assert np.array_equal(t["perm"].view(np.uint32), op), "permutation differs"
+    on = ot.nodes()
+    n, nn, ns = ctx.tree_sizes()
+    assert (n, nn, ns) == (w.n, ot.n_nodes, w.n + ot.n_nodes)
+    for k in ("level", "lo", "hi", "nchild"):
+        assert np.array_equal(t[k].astype(np.int64), on[k].astype(np.int64)), k
+    assert np.array_equal(t["prefix"].view(np.uint64), on["prefix"].astype(np.uint64))
+    scale = np.maximum(np.abs(on["M"]), 1e-300)
+    assert np.max(np.abs(t["M"] - on["M"]) / scale) <= 1e-6
+    for k in ("Rx", "Ry", "Rz", "delta"):
+        assert np.max(np.abs(t[k] - on[k])) / w.cube[3] <= 1e-6, k
+
+
+def test_config0_uniform_sphere(bh, oracle):
+    """32^3 sphere: full oracle parity, full direct sum, closed form 2 pi G rho (R^2 - r^2/3) inside."""
+    w = wl.by_name("sphere32")
+    ctx = _build(bh, w)
+    ot = oracle.OracleTree(w.x, w.y, w.z, w.m, w.cube)
+    _check_tree(ctx, ot, w)
+    phi, _ = _check_sampled(ctx, ot, w, 0.5, nruns=1, per=1 << 20)       # all 1024 groups
+    direct = ctx.potential_direct(w.G).cpu().numpy()
+    ref = oracle.direct(w.x, w.y, w.z, w.m, w.G)
+    assert np.max(np.abs(direct - ref) / np.abs(ref)) <= 1e-12
+    assert np.max(np.abs(phi - direct) / np.abs(direct)) <= 5e-3          # the tree code's own error at theta 0.5
+    r = np.sqrt((w.x - 0.5) ** 2 + (w.y - 0.5) ** 2 + (w.z - 0.5) ** 2)
+    inside = r < 0.3
+    exact = analytic.sphere_potential(r[inside], 0.4, 1.0, w.G)
+    assert np.max(np.abs(phi[inside] - exact) / np.abs(exact)) <= 2e-2    # 32^3 staircase of the sphere's surface
+
+
+def test_config1_maclaurin(bh, oracle):
+    """128^3 MacLaurin spheroid (e = 0.9): sampled oracle parity, analytic interior potential (Eq. 6, R12)."""
+    w = wl.by_name("maclaurin128")
+    ctx = _build(bh, w)
+    ot = oracle.OracleTree(w.x, w.y, w.z, w.m, w.cube)
+    _check_tree(ctx, ot, w)
+    phi, _ = _check_sampled(ctx, ot, w, 0.5)
+    a1, e = 0.4, 0.9
+    a3 = a1 * np.sqrt(1 - e * e)
+    X, Y, Z = w.x - 0.5, w.y - 0.5, w.z - 0.5
+    deep = (X * X + Y * Y) / (0.8 * a1) ** 2 + Z * Z / (0.8 * a3) ** 2 < 1.0
+    exact = analytic.maclaurin_interior(X[deep], Y[deep], Z[deep], a1, e, 1.0, w.G)
+    assert np.max(np.abs(phi[deep] - exact) / np.abs(exact)) <= 1e-2
+
+
+def test_config2_amr_core_and_config4_theta_sweep(bh, oracle):
+    """~3.9 M-cell AMR collapsing core: tree in full, then theta in {0.3, 0.5, 0.7, 1.0}: sampled oracle
+    parity, interactions per target, and the error against the fp64 direct sum on 4096 sampled targets."""
+    w = wl.by_name("amr_core")
+    assert 2_000_000 <= w.n <= 5_000_000
+    ctx = _build(bh, w)
+    ot = oracle.OracleTree(w.x, w.y, w.z, w.m, w.cube)
+    _check_tree(ctx, ot, w)
+    rng = np.random.Generator(np.random.PCG64(4096))
+    tg = np.sort(rng.choice(w.n, 4096, replace=False)).astype(np.int64)
+    direct = ctx.potential_direct(w.G, targets=torch.from_numpy(tg).cuda()).cpu().numpy()
+    sub = rng.choice(4096, 64, replace=False)                              # the oracle's direct sum on a few of them
+    ref = oracle.direct(w.x, w.y, w.z, w.m, w.G, targets=tg[sub])
+    assert np.max(np.abs(direct[sub] - ref) / np.abs(ref)) <= 1e-12
+    errs, inter = [], []
+    for theta in (0.3, 0.5, 0.7, 1.0):
+        phi, cnt = _check_sampled(ctx, ot, w, theta, nruns=6, per=8)
+        errs.append(np.max(np.abs(phi[tg] - direct) / np.abs(direct)))
+        inter.append(ctx.get_stats().interactions / w.n)
+    assert all(a < b for a, b in zip(errs, errs[1:])), errs               # error grows with theta
+    assert all(a > b for a, b in zip(inter, inter[1:])), inter            # work shrinks with theta
+    assert errs[0] <= 2e-3 and errs[1] <= 1e-2
+
+
+def test_config3_turb256_bench_configuration(bh, oracle):
+    """The workload bench.py times (16.8 M cells, theta 0.5): keys / topology / moments in full, Phi sampled."""
+    w = wl.by_name("turb256")
+    ctx = _build(bh, w)
+    ot = oracle.OracleTree(w.x, w.y, w.z, w.m, w.cube)
+    _check_tree(ctx, ot, w)
+    st = ctx.get_stats()
+    assert st.n_nodes == (w.n - 1) // 7 and st.depth == 7 and st.sort_passes == 3
+    _check_sampled(ctx, ot, w, 0.5, nruns=16, per=16)
+    _check_sampled(ctx, ot, w, 0.5, mac=1, nruns=4, per=8)
+    # properties that hold at any size: every potential is finite and negative (all masses are positive)
+    phi = ctx.potential(0.5, w.G).cpu().numpy()
+    assert np.all(np.isfinite(phi)) and np.all(phi < 0)
