@@ -308,17 +308,20 @@ walk_pair_kernel(const WalkParams P)
             if (ambm) amb[myr] = make_float4(r.x, r.y, r.z, rc2);
             __syncwarp();
             const int na = __popc(bAmb);
-            u32 resA = 0u, resB = 0u;
+            // bit i of failA / failB: this lane's member of A / B does NOT pass node i; one OR-reduction
+            // per group then replaces a vote per node
+            u32 failA = 0u, failB = 0u;
+            #pragma unroll 4
             for (int i = 0; i < na; ++i) {
                 const float4 q = amb[i];
                 const float2 dx = __fadd2_rn(splat2(q.x), npx), dy = __fadd2_rn(splat2(q.y), npy),
                              dz = __fadd2_rn(splat2(q.z), npz);
                 const float2 d2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
-                const u32 okA = __all_sync(0xffffffffu, !liveA || d2.x > q.w) ? 1u : 0u;
-                const u32 okB = __all_sync(0xffffffffu, !liveB || d2.y > q.w) ? 1u : 0u;
-                resA |= okA << i;
-                resB |= okB << i;
+                failA |= (d2.x > q.w ? 0u : 1u) << i;
+                failB |= (d2.y > q.w ? 0u : 1u) << i;
             }
+            const u32 resA = ~__reduce_or_sync(0xffffffffu, liveA ? failA : 0u);
+            const u32 resB = ~__reduce_or_sync(0xffffffffu, liveB ? failB : 0u);
             accm |= ambm & (((resA >> myr) & 1u) | (((resB >> myr) & 1u) << 1));
             if (COUNT) { cExA += ambm & 1u; cExB += ambm >> 1; }
             __syncwarp();
