@@ -110,6 +110,14 @@ int bh_set_option(bh_ctx* ctx, int key, int value);
 int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, const double* m,
              int64_t n, const double cube[4]);
 
+/* bh_update_masses: new masses for the SAME cells (positions unchanged since the last bh_build).
+ * An AMR code calls the solver every time step but moves no cell between regrids,
+ * so keys, sort and topology of the last build stay valid: only the mass fields of the leaf records
+ * and the moments (Eq. 5) are recomputed, with the same arithmetic as bh_build -- a following
+ * bh_potential gives bit-identical results to a fresh bh_build with these masses.
+ *   m : DEVICE, const double[n], original cell order; borrowed until the stream has passed the call. */
+int bh_update_masses(bh_ctx* ctx, const double* m);
+
 /* bh_potential: Phi_i = -G sum_j m_j/|r_i - r_j| over the nodes and leaf cells the group walk of
  * PAPER.md:176-178 selects (DESIGN.md W-rules).
  *   theta : >= 0; theta = 0 opens every node (the result is then the direct sum in fp32 terms).

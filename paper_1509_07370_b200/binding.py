@@ -15,7 +15,7 @@ BH_DIRECT_ALL_MAX = 1 << 18
 EXPORTED_SYMBOLS = (
     "bh_create", "bh_destroy", "bh_strerror", "bh_last_cuda_error", "bh_set_option", "bh_build", "bh_potential",
     "bh_potential_direct", "bh_solve_host", "bh_tree_sizes", "bh_export_tree", "bh_last_group_counts",
-    "bh_last_interactions", "bh_get_stats",
+    "bh_last_interactions", "bh_get_stats", "bh_update_masses",
 )
 
 
@@ -60,6 +60,7 @@ def lib():
         L.bh_last_cuda_error.restype = C.c_char_p
         L.bh_set_option.argtypes = [vp, i32, i32]
         L.bh_build.argtypes = [vp, dp, dp, dp, dp, i64, C.POINTER(C.c_double)]
+        L.bh_update_masses.argtypes = [vp, dp]
         L.bh_potential.argtypes = [vp, C.c_double, C.c_double, dp]
         L.bh_potential_direct.argtypes = [vp, C.c_double, dp, i64, dp]
         L.bh_solve_host.argtypes = [vp, dp, dp, dp, dp, i64, C.POINTER(C.c_double), C.c_double, C.c_double, dp]
@@ -140,6 +141,12 @@ class Context:
         self._check(self._L.bh_build(self._h, self._dev(x, f64), self._dev(y, f64), self._dev(z, f64),
                                      self._dev(m, f64), n, _cube(cube)))
         self.n = n
+
+    def update_masses(self, m):
+        """New masses for the cells of the last build (positions unchanged): leaf records and moments only."""
+        if m.numel() != self.n:
+            raise ValueError("m must have the length of the last build")
+        self._check(self._L.bh_update_masses(self._h, self._dev(m, self._torch.float64)))
 
     def potential(self, theta: float, G: float = 1.0, out=None):
         torch = self._torch

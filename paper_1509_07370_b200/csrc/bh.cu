@@ -120,6 +120,43 @@ int persistent_grid(const bh_ctx* ctx, int per_sm)
     return sms * per_sm;
 }
 
+
+// a5: moments of every level, deepest first; runs of small levels share one single-block launch
+int launch_moments(bh_ctx* ctx)
+{
+    cudaStream_t st = ctx->stream;
+    DeviceScalars* ds = ctx->scalars.as<DeviceScalars>();
+    MomentArgs MA;
+    MA.sv = ctx->sv; MA.nlo = ctx->nlo.as<u32>(); MA.nfirst = ctx->nfirst.as<u32>();
+    MA.node_slot = ctx->node_slot.as<u32>(); MA.rec64 = ctx->rec64.as<double4>();
+    MA.delta64 = ctx->delta64.as<double>(); MA.rec = ctx->rec.as<float4>(); MA.aux = ctx->aux.as<WalkAux>();
+    MA.max_bucket = &ds->max_bucket;
+    MA.x0 = ctx->cube[0]; MA.y0 = ctx->cube[1]; MA.z0 = ctx->cube[2]; MA.L = ctx->cube[3];
+    SmallLevels sl;
+    sl.nlev = 0;
+    for (int l = ctx->maxlevel; l >= -1; --l) {
+        const i64 b0 = l >= 0 ? ctx->lv.node_base[l] : 0, b1 = l >= 0 ? ctx->lv.node_base[l + 1] : 0;
+        const bool small = l >= 0 && b1 - b0 <= kSmallLevelNodes;
+        if ((!small || l < 0) && sl.nlev > 0) {          // flush the pending run of small levels
+            moments_small_kernel<<<1, kMomSmallThreads, 0, st>>>(sl, MA);
+            BH_CUDA(cudaGetLastError());
+            ctx->launches_build += 1;
+            sl.nlev = 0;
+        }
+        if (l < 0 || b1 == b0) continue;
+        if (small) {
+            sl.level[sl.nlev] = l; sl.b0[sl.nlev] = (u32)b0; sl.b1[sl.nlev] = (u32)b1;
+            sl.slot_end[sl.nlev] = ctx->lv.slot_base[l + 2];
+            ++sl.nlev;
+        } else {
+            moments_kernel<<<blocks_for(b1 - b0, 128), 128, 0, st>>>(b0, b1, l, ctx->lv.slot_base[l + 2], MA);
+            BH_CUDA(cudaGetLastError());
+            ctx->launches_build += 1;
+        }
+    }
+    return BH_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -341,34 +378,8 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
         ctx->launches_build += 1 + 3 + 1 + 1;   // count, scan, totals, assign
         BH_CUDA(cudaEventRecord(ctx->ev[EV_TOPO], st));
 
-        // ---- a5: moments, deepest level first; runs of small levels share one single-block launch ----
-        MomentArgs MA;
-        MA.sv = ctx->sv; MA.nlo = ctx->nlo.as<u32>(); MA.nfirst = ctx->nfirst.as<u32>();
-        MA.node_slot = ctx->node_slot.as<u32>(); MA.rec64 = ctx->rec64.as<double4>();
-        MA.delta64 = ctx->delta64.as<double>(); MA.rec = ctx->rec.as<float4>(); MA.aux = ctx->aux.as<WalkAux>();
-        MA.max_bucket = &ds->max_bucket; MA.x0 = cube[0]; MA.y0 = cube[1]; MA.z0 = cube[2]; MA.L = cube[3];
-        SmallLevels sl;
-        sl.nlev = 0;
-        for (int l = ctx->maxlevel; l >= -1; --l) {
-            const i64 b0 = l >= 0 ? ctx->lv.node_base[l] : 0, b1 = l >= 0 ? ctx->lv.node_base[l + 1] : 0;
-            const bool small = l >= 0 && b1 - b0 <= kSmallLevelNodes;
-            if ((!small || l < 0) && sl.nlev > 0) {          // flush the pending run of small levels
-                moments_small_kernel<<<1, kMomSmallThreads, 0, st>>>(sl, MA);
-                BH_CUDA(cudaGetLastError());
-                ctx->launches_build += 1;
-                sl.nlev = 0;
-            }
-            if (l < 0 || b1 == b0) continue;
-            if (small) {
-                sl.level[sl.nlev] = l; sl.b0[sl.nlev] = (u32)b0; sl.b1[sl.nlev] = (u32)b1;
-                sl.slot_end[sl.nlev] = ctx->lv.slot_base[l + 2];
-                ++sl.nlev;
-            } else {
-                moments_kernel<<<blocks_for(b1 - b0, 128), 128, 0, st>>>(b0, b1, l, ctx->lv.slot_base[l + 2], MA);
-                BH_CUDA(cudaGetLastError());
-                ctx->launches_build += 1;
-            }
-        }
+        // ---- a5: moments ----
+        { int rc = launch_moments(ctx); if (rc != BH_OK) return rc; }
     } else {
         BH_CUDA(cudaEventRecord(ctx->ev[EV_PERM], st));
         BH_CUDA(cudaEventRecord(ctx->ev[EV_TOPO], st));
@@ -376,6 +387,29 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
     BH_CUDA(cudaEventRecord(ctx->ev[EV_MOM], st));
     ctx->ev_build = true;
     ctx->built = true;
+    return BH_OK;
+}
+
+int bh_update_masses(bh_ctx* ctx, const double* m)
+{
+    if (!ctx || !m) return BH_ERR_INVALID_ARG;
+    if (!ctx->built) return BH_ERR_NOT_BUILT;
+    BH_CUDA(cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    ctx->walked = false;
+    ctx->counts_valid = false;
+    ctx->direct_ready = false;
+    ctx->launches_build = 0;
+    BH_CUDA(cudaEventRecord(ctx->ev[EV_B0], st));
+    for (int k = EV_KEYS; k <= EV_TOPO; ++k) BH_CUDA(cudaEventRecord(ctx->ev[k], st));
+    if (ctx->n >= 2) {
+        mass_update_kernel<<<blocks_for(ctx->n, 256), 256, 0, st>>>(ctx->sv, ctx->leaf_slot.as<u32>(), m, ctx->n,
+                                                                   ctx->rec64.as<double4>(), ctx->rec.as<float4>());
+        BH_CUDA(cudaGetLastError());
+        ctx->launches_build += 1;
+        { int rc = launch_moments(ctx); if (rc != BH_OK) return rc; }
+    }
+    BH_CUDA(cudaEventRecord(ctx->ev[EV_MOM], st));
     return BH_OK;
 }
 

@@ -382,6 +382,20 @@ direct_prepare_kernel(const SortedView sv, const u32* __restrict__ leaf_slot,
     slot_of[sv_idx(sv, s)] = (u32)s;
 }
 
+// ---- bh_update_masses: new masses for the cells of the last build (positions, and so the tree, unchanged) ----
+// 8 B gathered per cell; the mass fields of its fp64 and fp32 slot records are rewritten.
+__global__ void __launch_bounds__(256)
+mass_update_kernel(const SortedView sv, const u32* __restrict__ leaf_slot, const double* __restrict__ m, i64 n,
+                   double4* __restrict__ rec64, float4* __restrict__ rec)
+{
+    const i64 s = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    const double pm = __ldg(m + sv_idx(sv, s));
+    const u32 slot = leaf_slot[s];
+    rec64[slot].w = pm;
+    rec[slot].w = (float)pm;
+}
+
 // sorted keys and permutation as plain arrays (bh_export_tree)
 __global__ void __launch_bounds__(256)
 export_sorted_kernel(const SortedView sv, i64 n, u64* __restrict__ keys, u32* __restrict__ perm)

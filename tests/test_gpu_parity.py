@@ -227,3 +227,33 @@ def test_solve_host_matches_device_path(bh):
     phi_d = ctx.potential(0.5).cpu().numpy()
     phi_h = bh.Context(0).solve_host(w.x, w.y, w.z, w.m, w.cube, 0.5)
     assert np.array_equal(phi_d, phi_h)
+
+
+@pytest.mark.parametrize("w", [CASES[1], CASES[4], CASES[6]], ids=lambda w: w.name)
+def test_update_masses_equals_rebuild(bh, oracle, w):
+    """bh_update_masses (NEXT-2): new masses on the same cells reuse keys / sort / topology
+    and give what a fresh build with those masses gives, bit for bit; and both match the oracle."""
+    rng = np.random.Generator(np.random.PCG64(84))
+    m2 = w.m * rng.uniform(0.25, 4.0, w.n)
+    m2[rng.integers(0, w.n, 5)] = 0.0                                  # a few massless cells
+    ctx = _build(bh, w)
+    ctx.potential(0.5, w.G)                                            # the tree has been used before
+    ctx.update_masses(_dev(m2))
+    phi_u = ctx.potential(0.5, w.G).cpu().numpy()
+    cnt_u = ctx.last_group_counts().cpu().numpy()
+    t_u = _tree_np(ctx)
+    w2 = wl.Workload(w.name + "_m2", w.x, w.y, w.z, m2, cube=w.cube)
+    ctx2 = _build(bh, w2)
+    phi_r = ctx2.potential(0.5, w.G).cpu().numpy()
+    t_r = _tree_np(ctx2)
+    assert np.array_equal(phi_u, phi_r)
+    for k in ("keys", "perm", "level", "lo", "hi", "M", "Rx", "Ry", "Rz", "delta"):
+        assert np.array_equal(t_u[k], t_r[k]), k
+    ot = oracle.OracleTree(w.x, w.y, w.z, m2, w.cube)
+    ref, ocnt = ot.potential(0.5, w.G, mac_fp32=True, want_counts=True)
+    assert np.array_equal(cnt_u, ocnt)
+    _phi_check(phi_u, ref)
+    sub = ctx.potential_direct(w.G).cpu().numpy()                      # the direct sum sees the new masses too
+    dref = oracle.direct(w.x, w.y, w.z, m2, w.G)
+    nz = dref != 0
+    assert np.max(np.abs(sub[nz] - dref[nz]) / np.abs(dref[nz])) <= 1e-12
