@@ -253,7 +253,8 @@ def test_update_masses_equals_rebuild(bh, oracle, w):
     ref, ocnt = ot.potential(0.5, w.G, mac_fp32=True, want_counts=True)
     assert np.array_equal(cnt_u, ocnt)
     _phi_check(phi_u, ref)
-    sub = ctx.potential_direct(w.G).cpu().numpy()                      # the direct sum sees the new masses too
-    dref = oracle.direct(w.x, w.y, w.z, m2, w.G)
+    tg = rng.integers(0, w.n, 64)                                      # the direct sum sees the new masses too
+    sub = ctx.potential_direct(w.G, targets=torch.from_numpy(tg).cuda()).cpu().numpy()
+    dref = oracle.direct(w.x, w.y, w.z, m2, w.G, targets=tg)
     nz = dref != 0
     assert np.max(np.abs(sub[nz] - dref[nz]) / np.abs(dref[nz])) <= 1e-12
