@@ -154,3 +154,56 @@ def test_config3_turb256_bench_configuration(bh, oracle):
     # properties that hold at any size: every potential is finite and negative (all masses are positive)
     phi = ctx.potential(0.5, w.G).cpu().numpy()
     assert np.all(np.isfinite(phi)) and np.all(phi < 0)
+
+
+def test_large_grid_512_properties(bh):
+    """134 M cells (512^3 uniform grid, equal masses): well past BASELINE's largest config.  The oracle cannot
+    build this in seconds, so the checks are properties that hold at any size: node count (n-1)/7, depth 8,
+    3 sort passes, root moments, the mirror symmetry of Phi, and sampled targets against the fp64 direct sum."""
+    ng = 512
+    n = ng ** 3
+    free, _ = torch.cuda.mem_get_info()
+    if free < 40 * (1 << 30):
+        pytest.skip("needs 40 GB of free device memory")
+    ax = (torch.arange(ng, dtype=torch.float64, device="cuda") + 0.5) / ng
+    x = ax.view(ng, 1, 1).expand(ng, ng, ng).reshape(-1).contiguous()
+    y = ax.view(1, ng, 1).expand(ng, ng, ng).reshape(-1).contiguous()
+    z = ax.view(1, 1, ng).expand(ng, ng, ng).reshape(-1).contiguous()
+    m = torch.full((n,), 1.0 / n, dtype=torch.float64, device="cuda")
+    ctx = bh.Context(0)
+    ctx.build(x, y, z, m, (0.0, 0.0, 0.0, 1.0))
+    st = ctx.get_stats()
+    assert st.n_nodes == (n - 1) // 7 and st.depth == 8 and st.sort_passes == 4 and st.n_clamped == 0
+    t = ctx.export_tree()
+    assert abs(float(t["M"][0]) - 1.0) <= 1e-12
+    for k in ("Rx", "Ry", "Rz"):
+        assert abs(float(t[k][0]) - 0.5) <= 1e-12
+    keys = t["keys"].view(torch.int64)
+    assert bool((keys[1:] > keys[:-1]).all())                     # strictly ascending: all keys distinct
+    del t, keys
+    phi = ctx.potential(0.5, 1.0)
+    st = ctx.get_stats()
+    assert 1000 < st.interactions / n < 2600
+    p3 = phi.view(ng, ng, ng)
+    for dim in (0, 1, 2):                                         # the cube of equal masses is mirror symmetric
+        assert float((p3 - p3.flip(dim)).abs().max()) <= 2e-5 * float(phi.abs().max())
+    rng = np.random.Generator(np.random.PCG64(512))
+    tg = torch.from_numpy(np.sort(rng.choice(n, 64, replace=False)).astype(np.int64)).cuda()
+    direct = ctx.potential_direct(1.0, targets=tg)
+    rel = ((phi[tg] - direct) / direct).abs()
+    assert float(rel.max()) <= 5e-3                               # the tree code's own error at theta = 0.5
+    centre = float(phi.view(ng, ng, ng)[ng // 2, ng // 2, ng // 2])
+    assert abs(centre + analytic.CUBE_SELF) <= 2e-3 * analytic.CUBE_SELF   # -Phi at the centre of a unit cube of unit mass
+
+
+def test_size_limits(bh):
+    """n >= 2^30 is refused before anything is touched (30-bit tile counters of the sort); n >= 2^31 is invalid."""
+    ctx = bh.Context(0)
+    one = torch.zeros(1, dtype=torch.float64, device="cuda")
+    L = bh.lib()
+    import ctypes
+    cube = (ctypes.c_double * 4)(0.0, 0.0, 0.0, 1.0)
+    p = one.data_ptr()
+    assert L.bh_build(ctx._h, p, p, p, p, 1 << 30, cube) == -5    # BH_ERR_TOO_LARGE
+    assert L.bh_build(ctx._h, p, p, p, p, 1 << 31, cube) == -1    # BH_ERR_INVALID_ARG
+    assert L.bh_build(ctx._h, p, p, p, p, 0, cube) == -1
