@@ -101,10 +101,10 @@ int bh_set_option(bh_ctx* ctx, int key, int value);
  *                L > 0.  A coordinate outside the cube is clamped into the edge cell and counted
  *                (bh_stats.n_clamped); NaN coordinates quantise to 0.
  * Steps, all on the device: 63-bit Morton keys (DESIGN.md K-rules) -> stable LSD radix sort of
- * (key, index) -> permutation of the cells into sorted order -> octree topology from the sorted
- * keys (one cell per leaf, single-child chains kept, identical keys form a level-21 bucket leaf;
- * DESIGN.md T-rules) -> bottom-up level-by-level M, R (Eq. 5), delta = |R - geometric centre|
- * in fp64 (DESIGN.md M-rules).
+ * (key, index) -> octree topology from the sorted keys (one cell per leaf, single-child chains kept,
+ * identical keys form a level-21 bucket leaf; DESIGN.md T-rules), the cell data being gathered into
+ * tree order in the same pass -> bottom-up level-by-level M, R (Eq. 5), delta = |R - geometric
+ * centre| in fp64 (DESIGN.md M-rules).
  * Synchronises the stream twice internally to read back (a) which key bits vary and (b) the node
  * count per level; everything else is asynchronous. */
 int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, const double* m,

@@ -42,7 +42,6 @@ struct DeviceScalars {          // small device-resident results read back by th
     u32 topo_rows[kTopoDigits + 1];   // row starts of the scanned level histogram + grand total
     u32 scan_total;
     u32 max_bucket;
-    u32 walk_overflow;
     unsigned long long totals[5];
 };
 

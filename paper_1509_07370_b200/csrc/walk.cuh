@@ -10,17 +10,20 @@
 //    result is the one of DESIGN.md W1-W4 -- but they share the traversal: a stack entry carries
 //    the set of groups that still need the subtree, and a node both groups accept (about 3/4 of
 //    all list entries on the grid workloads) is fetched from shared memory once and evaluated for
-//    both targets with packed fp32x2 arithmetic (FADD2/FFMA2, sm_100; one MUFU.RSQ per interaction).
+//    both targets (packed fp32x2 arithmetic FADD2/FFMA2, sm_100; one MUFU.RSQ per interaction).
 //  * The traversal is lane-parallel: each step pops up to 4 stack entries and tests their <= 32
 //    children at once, one child per lane.  The vote ("all members have d^2 > r_c^2") is decided
 //    without touching the members whenever the group's bounding box proves it: fp32 rounding is
 //    monotone, so the fp32 d^2 evaluated at the box's nearest (farthest) point bounds every
 //    member's fp32 d^2 from below (above).  Only nodes between the two bounds take the per-member
 //    test + __all_sync vote.
-//  * Accepted nodes and leaf cells go to interaction lists in shared memory: U2 (both groups,
-//    float4 records, packed across the two targets), UA / UB (one group only, SoA, packed across
-//    two entries), and C (leaf cells inside a group's bounding box -- the only ones that can be a
-//    target's own cell or coincide with it -- evaluated with the zero-distance mask of W3).
+//  * Accepted nodes and leaf cells go to interaction lists in shared memory: U2 (both groups),
+//    UA / UB (one group only) -- all SoA and evaluated two ENTRIES per packed instruction against a
+//    scalar target coordinate, U2 for the lane's two targets from the same loads -- and C (leaf
+//    cells inside a group's bounding box -- the only ones that can be a target's own cell or
+//    coincide with it -- evaluated with the zero-distance mask of W3).
+//  * The member votes of one step are batched: each lane collects its member's failures as a bit
+//    per undecided node and one OR-reduction per group replaces a vote per node.
 //  * Partial sums are fp32 over one list flush (<= 128 entries, 4 accumulators) and are flushed
 //    into an fp64 sum per target, which keeps the summation error near 1e-7 relative.
 //  * Phi is written straight to the original cell order (step a7 is fused: no extra pass).
