@@ -23,17 +23,15 @@ constexpr u32 kFlagAgg = 1u << 30, kFlagPrefix = 2u << 30, kValMask = (1u << 30)
 // distinct digits the warp holds (match.any slows down with every distinct value)
 __device__ __forceinline__ u32 digit_peers(u32 d)
 {
-    u32 peers = 0xffffffffu;
+    u32 differ = 0u;                             // lanes whose digit differs from this lane's in some bit
     #pragma unroll
     for (int b = 0; b < 8; ++b) {
-        const bool bit = (d >> b) & 1u;
-        const u32 bal = __ballot_sync(0xffffffffu, bit);
-        peers &= bit ? bal : ~bal;
+        const int s = (int)(d << (31 - b)) >> 31;            // all ones iff bit b of d is set
+        const u32 bal = __ballot_sync(0xffffffffu, s < 0);
+        differ |= bal ^ (u32)s;
     }
-    return peers;
+    return ~differ;
 }
-
-
 
 struct SortPlan {
     int npasses;
@@ -124,10 +122,17 @@ radix_onesweep_kernel(const u64* __restrict__ kin, const u32* __restrict__ vin, 
     u64 key[kSortItems];
     u32 rank[kSortItems];
     const i64 wbase = base + (i64)warp * (32 * kSortItems);
-    #pragma unroll
-    for (int i = 0; i < kSortItems; ++i) {
-        const i64 e = wbase + i * 32 + lane;
-        key[i] = e < n ? ld_stream(kin + e) : ~0ULL;       // padding takes the top digit, last in the tile
+    const bool full = base + kSortTile <= n;               // every tile but the last: no bounds checks
+    if (full) {
+        const u64* src = kin + wbase + lane;
+        #pragma unroll
+        for (int i = 0; i < kSortItems; ++i) key[i] = ld_stream(src + i * 32);
+    } else {
+        #pragma unroll
+        for (int i = 0; i < kSortItems; ++i) {
+            const i64 e = wbase + i * 32 + lane;
+            key[i] = e < n ? ld_stream(kin + e) : ~0ULL;   // padding takes the top digit, last in the tile
+        }
     }
     // stable rank inside the warp chunk: items are visited in memory order
     const u32 lt = (1u << lane) - 1u;
@@ -147,7 +152,7 @@ radix_onesweep_kernel(const u64* __restrict__ kin, const u32* __restrict__ vin, 
         #pragma unroll
         for (int i = 0; i < kSortItems; ++i) {   // the values arrive while the digit offsets are worked out
             const i64 e = wbase + i * 32 + lane;
-            val[i] = e < n ? ld_stream(vin + e) : 0u;
+            val[i] = (full || e < n) ? ld_stream(vin + e) : 0u;
         }
     }
     __syncthreads();
