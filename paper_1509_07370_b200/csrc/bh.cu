@@ -81,6 +81,7 @@ struct bh_ctx {
     DevBuf nlo, nfirst, node_slot, delta64;
     // per slot
     DevBuf rec64, rec, aux;
+    i64 aux_dirty_nn = -1;                // aux is zero except on node_slot[0, aux_dirty_nn); -1: unknown, clear all
     // walk
     DevBuf gcount;
     DevBuf scalars;                       // DeviceScalars
@@ -361,24 +362,38 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
             return BH_ERR_CUDA;
         }
 
+        // aux must be zero on every leaf slot; only the node slots of the previous build are not
+        {
+            const bool grow = sizeof(WalkAux) * (size_t)nslots > ctx->aux.cap;
+            const i64 dirty = ctx->aux_dirty_nn;
+            ctx->aux_dirty_nn = -1;                            // until this build's moments are launched
+            if (!grow && dirty > 0) {
+                aux_clear_kernel<<<blocks_for(dirty, 256), 256, 0, st>>>(ctx->node_slot.as<u32>(), dirty,
+                                                                        ctx->aux.as<WalkAux>());
+                BH_CUDA(cudaGetLastError());
+                ctx->launches_build += 1;
+            }
+            BH_CUDA(ctx->aux.ensure(sizeof(WalkAux) * nslots));
+            if (grow || dirty < 0) BH_CUDA(cudaMemsetAsync(ctx->aux.p, 0, ctx->aux.cap, st));
+        }
         BH_CUDA(ctx->nlo.ensure(sizeof(u32) * nn));
         BH_CUDA(ctx->nfirst.ensure(sizeof(u32) * (nn + 4)));
         BH_CUDA(ctx->node_slot.ensure(sizeof(u32) * nn));
         BH_CUDA(ctx->delta64.ensure(sizeof(double) * nn));
         BH_CUDA(ctx->rec64.ensure(sizeof(double4) * nslots));
         BH_CUDA(ctx->rec.ensure(sizeof(float4) * nslots));
-        BH_CUDA(ctx->aux.ensure(sizeof(WalkAux) * nslots));
 
         topo_assign_kernel<<<tgrid, kTopoThreads, 0, st>>>(
             ctx->clev.as<signed char>(), n, ctx->sv, x, y, z, m, hist, nchunks, (u32)nslots,
             ctx->leaf_slot.as<u32>(), ctx->node_slot.as<u32>(), ctx->nfirst.as<u32>(), ctx->nlo.as<u32>(),
-            ctx->rec64.as<double4>(), ctx->rec.as<float4>(), ctx->aux.as<WalkAux>());
+            ctx->rec64.as<double4>(), ctx->rec.as<float4>());
         BH_CUDA(cudaGetLastError());
         ctx->launches_build += 1 + 3 + 1 + 1;   // count, scan, totals, assign
         BH_CUDA(cudaEventRecord(ctx->ev[EV_TOPO], st));
 
         // ---- a5: moments ----
         { int rc = launch_moments(ctx); if (rc != BH_OK) return rc; }
+        ctx->aux_dirty_nn = nn;
     } else {
         BH_CUDA(cudaEventRecord(ctx->ev[EV_PERM], st));
         BH_CUDA(cudaEventRecord(ctx->ev[EV_TOPO], st));

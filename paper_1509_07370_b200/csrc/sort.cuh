@@ -19,6 +19,14 @@ constexpr int kRadix = 256;
 constexpr int kMaxPasses = 8;
 constexpr u32 kFlagAgg = 1u << 30, kFlagPrefix = 2u << 30, kValMask = (1u << 30) - 1u;   // tile status words
 
+constexpr int kLookWin = 4;                      // tile status words a look-back step fetches at once
+__device__ __forceinline__ u32 ld_status(const u32* p)
+{
+    u32 v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
 // lanes of the warp whose 8-bit digit equals this lane's: eight ballots, independent of how many
 // distinct digits the warp holds (match.any slows down with every distinct value)
 __device__ __forceinline__ u32 digit_peers(u32 d)
@@ -49,7 +57,7 @@ radix_hist_strided_kernel(const u64* __restrict__ keys, i64 n, const SortPlan pl
     __shared__ u32 h[kMaxPasses * kRadix];
     for (int i = threadIdx.x; i < plan.npasses * kRadix; i += kSortThreads) h[i] = 0;
     __syncthreads();
-    constexpr int kRows = 4;                              // rows of 32 keys a warp keeps in flight
+    constexpr int kRows = 8;                              // rows of 32 keys a warp keeps in flight
     const i64 stride = (i64)gridDim.x * kSortThreads * kRows;
     const u32 lane = threadIdx.x & 31;
     for (i64 wb = ((i64)blockIdx.x * kSortThreads + (threadIdx.x & ~31)) * kRows; wb < n; wb += stride) {   // warp-uniform
@@ -59,15 +67,20 @@ radix_hist_strided_kernel(const u64* __restrict__ keys, i64 n, const SortPlan pl
         #pragma unroll
         for (int r = 0; r < kRows; ++r) {
             const bool valid = wb + 32 * r + lane < n;
-            const u32 vmask = __ballot_sync(0xffffffffu, valid);
+            const bool fullrow = wb + 32 * r + 32 <= n;                      // warp-uniform
+            // key bits on which the row's keys differ: two OR-reductions serve every pass.
+            // Neighbouring cells mostly share their upper digits: one atomic for the whole row then.
+            const u64 k0 = __shfl_sync(0xffffffffu, k[r], 0);
+            const u64 xr = k[r] ^ k0;
+            const u32 dlo = __reduce_or_sync(0xffffffffu, (u32)xr);
+            const u32 dhi = __reduce_or_sync(0xffffffffu, (u32)(xr >> 32));
+            const u64 differ = ((u64)dhi << 32) | dlo;
             #pragma unroll
             for (int p = 0; p < kMaxPasses; ++p) {      // static indices keep the plan in constant memory
                 if (p >= plan.npasses) break;
                 const u32 d = (u32)(k[r] >> plan.shift[p]) & plan.mask[p];
-                // neighbouring cells mostly share their upper digits: one atomic for the whole row then
-                int same;
-                __match_all_sync(0xffffffffu, d, &same);
-                if (same && vmask == 0xffffffffu) {
+                const bool same = ((u32)(differ >> plan.shift[p]) & plan.mask[p]) == 0u;
+                if (same && fullrow) {
                     if (lane == 0) atomicAdd(&h[p * kRadix + d], 32u);
                 } else if (valid) {
                     atomicAdd(&h[p * kRadix + d], 1u);
@@ -169,12 +182,24 @@ radix_onesweep_kernel(const u64* __restrict__ kin, const u32* __restrict__ vin, 
         const u32 gstart = block_excl_scan_256(ghist[d], total, S.s_warp);  // global start of digit d
         u32 before = 0;
         if (tile > 0) {
-            for (int t = tile - 1;; --t) {
-                volatile const u32* pt = status + (size_t)t * kRadix + d;
-                u32 v;
-                do { v = *pt; } while ((v >> 30) == 0u);
-                before += v & kValMask;
-                if (v & kFlagPrefix) break;
+            // look-back in windows of kLookWin tiles: the window's status words are fetched together
+            // (independent loads, one L2 round trip), then consumed nearest tile first
+            bool done = false;
+            for (int t0 = tile - 1; !done; t0 -= kLookWin) {
+                u32 v[kLookWin];
+                #pragma unroll
+                for (int j = 0; j < kLookWin; ++j) {
+                    const int t = t0 - j > 0 ? t0 - j : 0;
+                    v[j] = ld_status(status + (size_t)t * kRadix + d);
+                }
+                #pragma unroll
+                for (int j = 0; j < kLookWin; ++j) {
+                    if (done) break;
+                    u32 w = v[j];
+                    while ((w >> 30) == 0u) w = ld_status(status + (size_t)(t0 - j) * kRadix + d);
+                    before += w & kValMask;
+                    if (w & kFlagPrefix) done = true;      // tile 0 always publishes a prefix
+                }
             }
             *st = kFlagPrefix | (before + run);
         }

@@ -59,14 +59,10 @@ __global__ void __launch_bounds__(kTopoThreads)
 topo_count_kernel(const SortedView sv, i64 n, signed char* __restrict__ clev, u32* __restrict__ hist,
                   i64 nchunks)
 {
-    __shared__ u32 h[kTopoThreads / 32][kTopoDigits + 3];
     const u32 lane = lane_id();
     const int warp = threadIdx.x >> 5;
     const i64 chunk = (i64)blockIdx.x * (kTopoThreads / 32) + warp;
-    if (chunk >= nchunks) return;                      // whole warp leaves; only warp-level sync below
-    u32* hw = h[warp];
-    for (int d = lane; d < kTopoDigits; d += 32) hw[d] = 0u;
-    __syncwarp();
+    if (chunk >= nchunks) return;                      // whole warp leaves; only warp-level primitives below
     const i64 wbase = chunk * kTopoChunk;
     // c(s) of the chunk's cells: every load is issued before the first use (indices clamped, results
     // masked), so a warp has its whole chunk in flight at once
@@ -100,38 +96,38 @@ topo_count_kernel(const SortedView sv, i64 n, signed char* __restrict__ clev, u3
         cprev = xp == 0ULL ? kMaxLevel : (__clzll((long long)xp) - 1) / 3;
     }
     if (wbase == 0) cprev = -1;
+    // level masks of the chunk's cells stay in registers; the histogram rows are then one add-reduction
+    // per level that occurs in the chunk (a handful), not atomics per cell
+    u32 em[kTopoItems], im[kTopoItems];
+    u32 ue = 0u;
     #pragma unroll
     for (int i = 0; i < kTopoItems; ++i) {
-        if (wbase + 32 * i >= n) break;
-        {
-            const i64 s = wbase + 32 * i + lane;
-            const bool valid = s < n;
-            const int cs = (valid && s + 1 < n) ? c[i] : -1;
-            int cp = __shfl_up_sync(0xffffffffu, cs, 1);
-            if (lane == 0) cp = cprev;
-            cprev = __shfl_sync(0xffffffffu, cs, 31);
-            if (valid) clev[s] = (signed char)cs;
-            // leaf entity: usually the same level for the whole row -> one shared atomic
-            const int leafL = valid ? (cp > cs ? cp : cs) + 1 : -1;
-            const int l0 = __shfl_sync(0xffffffffu, leafL, 0);
-            const u32 vmask = __ballot_sync(0xffffffffu, valid);
-            const u32 same = __ballot_sync(0xffffffffu, leafL == l0);
-            if ((same & vmask) == vmask) {
-                if (lane == 0 && vmask) atomicAdd(&hw[l0], (u32)__popc(vmask));
-            } else if (valid) {
-                atomicAdd(&hw[leafL], 1u);
-            }
-            // internal nodes started by this cell: levels cp+1 .. cs (few lanes, few levels)
-            if (valid) {
-                for (int l = cp + 1; l <= cs; ++l) {
-                    atomicAdd(&hw[l], 1u);
-                    atomicAdd(&hw[kSlotLevels + l], 1u);
-                }
-            }
+        const i64 s = wbase + 32 * i + lane;
+        const bool valid = s < n;
+        const int cs = (valid && s + 1 < n) ? c[i] : -1;
+        int cp = __shfl_up_sync(0xffffffffu, cs, 1);
+        if (lane == 0) cp = cprev;
+        cprev = __shfl_sync(0xffffffffu, cs, 31);
+        em[i] = 0u; im[i] = 0u;
+        if (valid) {
+            clev[s] = (signed char)cs;
+            entity_masks(cp, cs, im[i], em[i]);
         }
+        ue |= em[i];
     }
-    __syncwarp();
-    for (int d = lane; d < kTopoDigits; d += 32) hist[(i64)d * nchunks + chunk] = hw[d];
+    u32 U = __reduce_or_sync(0xffffffffu, ue);
+    u32 myE = 0u, myI = 0u;                            // lane l: entities / internal nodes of level l
+    while (U) {
+        const int l = __ffs(U) - 1;
+        U &= U - 1u;
+        u32 v = 0u;                                    // entities in the low half, nodes in the high half (<= 256 each)
+        #pragma unroll
+        for (int i = 0; i < kTopoItems; ++i) v += ((em[i] >> l) & 1u) + (((im[i] >> l) & 1u) << 16);
+        const u32 tot = __reduce_add_sync(0xffffffffu, v);
+        if ((int)lane == l) { myE = tot & 0xffffu; myI = tot >> 16; }
+    }
+    if (lane < (u32)kSlotLevels) hist[(i64)lane * nchunks + chunk] = myE;
+    if (lane < (u32)kNumLevels) hist[(i64)(kSlotLevels + lane) * nchunks + chunk] = myI;
 }
 
 // row starts of the scanned histogram (+ the grand total) for the host: out[d] = scanned[d * nchunks]
@@ -147,14 +143,15 @@ __global__ void topo_totals_kernel(const u32* __restrict__ scanned, i64 nchunks,
 // `scanned` = exclusive scan of the count kernel's histogram (row-major over [digit][chunk]), so
 // scanned[l][chunk] is the slot of the chunk's first level-l entity and scanned[23 + l][chunk] - nslots
 // the canonical id of its first level-l node.  Per cell: 4 B idx + 1 B c + 32 B gathered; written
-// 4 B slot + 32 B fp64 record + 16 B fp32 record + 16 B aux; per node 12 B.
+// 4 B slot + 32 B fp64 record + 16 B fp32 record; per node 12 B.  The aux record of a leaf slot is
+// all zero and is NOT written here: the context keeps aux zero everywhere except on the node slots of
+// the last build, which aux_clear_kernel resets before the next one.
 __global__ void __launch_bounds__(kTopoThreads)
 topo_assign_kernel(const signed char* __restrict__ clev, i64 n, const SortedView sv,
                    const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
                    const double* __restrict__ m, const u32* __restrict__ scanned, i64 nchunks, u32 nslots,
                    u32* __restrict__ leaf_slot, u32* __restrict__ node_slot, u32* __restrict__ nfirst,
-                   u32* __restrict__ nlo, double4* __restrict__ rec64, float4* __restrict__ rec,
-                   WalkAux* __restrict__ aux)
+                   u32* __restrict__ nlo, double4* __restrict__ rec64, float4* __restrict__ rec)
 {
     const u32 lane = lane_id();
     const u32 lt = (1u << lane) - 1u;
@@ -165,7 +162,6 @@ topo_assign_kernel(const signed char* __restrict__ clev, i64 n, const SortedView
     u32 cntT = lane < (u32)kSlotLevels ? scanned[(i64)lane * nchunks + chunk] : 0u;
     u32 cntI = lane < (u32)kNumLevels ? scanned[(i64)(kSlotLevels + lane) * nchunks + chunk] - nslots : 0u;
     int carry = wbase > 0 ? (int)clev[wbase - 1] : -1;
-    const uint4 leaf_aux = make_uint4(0u, 0u, 0u, 0u);
     u32 oi[kTopoItems];                        // the chunk's permutation entries and c(s), fetched up front so
     int ci[kTopoItems];                        // that a row's gathers do not wait behind them
     #pragma unroll
@@ -221,9 +217,16 @@ topo_assign_kernel(const signed char* __restrict__ clev, i64 n, const SortedView
             st_stream(o64, make_double2(px, py));
             st_stream(o64 + 1, make_double2(pz, pm));
             st_stream(rec + myslot, make_float4((float)px, (float)py, (float)pz, (float)pm));
-            st_stream(reinterpret_cast<uint4*>(aux) + myslot, leaf_aux);
         }
     }
+}
+
+// aux[node_slot[b]] = 0 for the nodes of the previous build (16 B per node instead of 16 B per slot)
+__global__ void __launch_bounds__(256)
+aux_clear_kernel(const u32* __restrict__ node_slot, i64 nn, WalkAux* __restrict__ aux)
+{
+    const i64 b = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b < nn) reinterpret_cast<uint4*>(aux)[node_slot[b]] = make_uint4(0u, 0u, 0u, 0u);
 }
 
 // first index in [a, hi) whose key is >= limit (hi if none); gallops from a
