@@ -27,18 +27,41 @@ __device__ __forceinline__ u32 ld_status(const u32* p)
     return v;
 }
 
-// lanes of the warp whose 8-bit digit equals this lane's: eight ballots, independent of how many
-// distinct digits the warp holds (match.any slows down with every distinct value)
-__device__ __forceinline__ u32 digit_peers(u32 d)
+// lanes of the warp whose 8-bit digit equals this lane's, by ballots over the digit bits in `vary`
+// (warp-uniform; must contain every bit on which the warp's digits differ).  Eight ballots when all
+// bits vary (match.any slows down with every distinct value instead); cells that are neighbours in
+// memory share most key bits, so a warp of grid data in original order needs only 2-3.
+__device__ __forceinline__ u32 digit_peers_on(u32 d, u32 vary)
 {
     u32 differ = 0u;                             // lanes whose digit differs from this lane's in some bit
-    #pragma unroll
-    for (int b = 0; b < 8; ++b) {
-        const int s = (int)(d << (31 - b)) >> 31;            // all ones iff bit b of d is set
-        const u32 bal = __ballot_sync(0xffffffffu, s < 0);
-        differ |= bal ^ (u32)s;
+    if (vary == 0xffu) {
+        #pragma unroll
+        for (int b = 0; b < 8; ++b) {
+            const int s = (int)(d << (31 - b)) >> 31;            // all ones iff bit b of d is set
+            const u32 bal = __ballot_sync(0xffffffffu, s < 0);
+            differ |= bal ^ (u32)s;
+        }
+    } else {
+        while (vary) {
+            const int b = __ffs(vary) - 1;
+            vary &= vary - 1u;
+            const int s = (int)(d << (31 - b)) >> 31;
+            const u32 bal = __ballot_sync(0xffffffffu, s < 0);
+            differ |= bal ^ (u32)s;
+        }
     }
     return ~differ;
+}
+__device__ __forceinline__ u32 digit_peers(u32 d)
+{
+    return digit_peers_on(d, __reduce_or_sync(0xffffffffu, d ^ __shfl_sync(0xffffffffu, d, 0)));
+}
+
+// shared-memory add without a return value, 32-bit shared address
+__device__ __forceinline__ void red_shared_add_if(u32 saddr, u32 v, bool on)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p red.shared.add.u32 [%0], %1;\n\t}"
+                 :: "r"(saddr), "r"(v), "r"((u32)on) : "memory");
 }
 
 struct SortPlan {
@@ -60,31 +83,37 @@ radix_hist_strided_kernel(const u64* __restrict__ keys, i64 n, const SortPlan pl
     constexpr int kRows = 8;                              // rows of 32 keys a warp keeps in flight
     const i64 stride = (i64)gridDim.x * kSortThreads * kRows;
     const u32 lane = threadIdx.x & 31;
+    u32 hbase = (u32)__cvta_generic_to_shared(h);
+    asm volatile("" : "+r"(hbase));                       // keep the shared base in a register
     for (i64 wb = ((i64)blockIdx.x * kSortThreads + (threadIdx.x & ~31)) * kRows; wb < n; wb += stride) {   // warp-uniform
         u64 k[kRows];
         #pragma unroll
         for (int r = 0; r < kRows; ++r) k[r] = wb + 32 * r + lane < n ? ld_stream(keys + wb + 32 * r + lane) : 0ULL;
+        const bool fullblk = wb + 32 * kRows <= n;            // warp-uniform
         #pragma unroll
-        for (int r = 0; r < kRows; ++r) {
-            const bool valid = wb + 32 * r + lane < n;
-            const bool fullrow = wb + 32 * r + 32 <= n;                      // warp-uniform
-            // key bits on which the row's keys differ: two OR-reductions serve every pass.
-            // Neighbouring cells mostly share their upper digits: one atomic for the whole row then.
-            const u64 k0 = __shfl_sync(0xffffffffu, k[r], 0);
-            const u64 xr = k[r] ^ k0;
-            const u32 dlo = __reduce_or_sync(0xffffffffu, (u32)xr);
-            const u32 dhi = __reduce_or_sync(0xffffffffu, (u32)(xr >> 32));
-            const u64 differ = ((u64)dhi << 32) | dlo;
+        for (int p = 0; p < kMaxPasses; ++p) {          // static indices keep the plan in constant memory
+            if (p >= plan.npasses) break;
+            const int sh = plan.shift[p];
+            const u32 mk = plan.mask[p];
+            u32 d[kRows];
+            bool alleq = true;
             #pragma unroll
-            for (int p = 0; p < kMaxPasses; ++p) {      // static indices keep the plan in constant memory
-                if (p >= plan.npasses) break;
-                const u32 d = (u32)(k[r] >> plan.shift[p]) & plan.mask[p];
-                const bool same = ((u32)(differ >> plan.shift[p]) & plan.mask[p]) == 0u;
-                if (same && fullrow) {
-                    if (lane == 0) atomicAdd(&h[p * kRadix + d], 32u);
-                } else if (valid) {
-                    atomicAdd(&h[p * kRadix + d], 1u);
-                }
+            for (int r = 0; r < kRows; ++r) {
+                d[r] = (u32)(k[r] >> sh) & mk;
+                alleq = alleq && d[r] == d[0];
+            }
+            // Cells that are neighbours in memory share most key bits: a lane's keys of the 8 rows (32
+            // elements apart) usually carry the same digit, and the upper digits are the same for the
+            // whole block -- then one shared atomic per lane, or one per warp, counts all 256 keys.
+            // (Same-address shared atomics are served one lane at a time, so this matters.)
+            if (fullblk && __all_sync(0xffffffffu, alleq)) {
+                int uni;
+                __match_all_sync(0xffffffffu, d[0], &uni);
+                red_shared_add_if(hbase + ((p * kRadix + d[0]) << 2), uni ? 32u * kRows : (u32)kRows, uni ? lane == 0 : true);
+            } else {
+                #pragma unroll
+                for (int r = 0; r < kRows; ++r)
+                    red_shared_add_if(hbase + ((p * kRadix + d[r]) << 2), 1u, wb + 32 * r + lane < n);
             }
         }
     }
@@ -152,7 +181,8 @@ radix_onesweep_kernel(const u64* __restrict__ kin, const u32* __restrict__ vin, 
     #pragma unroll
     for (int i = 0; i < kSortItems; ++i) {
         const u32 d = (u32)(key[i] >> shift) & mask;
-        const u32 peers = digit_peers(d);
+        // first pass: the input is in memory order, neighbours share most digit bits
+        const u32 peers = (MODE == kPackedFirst || MODE == kGenericFirst) ? digit_peers(d) : digit_peers_on(d, 0xffu);
         const u32 cnt = S.wcnt[warp][d];
         __syncwarp();
         const u32 r = __popc(peers & lt);

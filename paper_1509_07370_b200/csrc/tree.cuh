@@ -72,11 +72,17 @@ topo_count_kernel(const SortedView sv, i64 n, signed char* __restrict__ clev, u3
     if (sv.packed) {
         const u32* w = reinterpret_cast<const u32*>(sv.packed);
         u32 x[kTopoItems];
-        #pragma unroll
-        for (int i = 0; i < kTopoItems; ++i) {
-            const i64 s = wbase + 32 * i + lane;
-            const i64 s0 = s < last ? s : last, s1 = s + 1 < last ? s + 1 : last;
-            x[i] = w[2 * s0 + 1] ^ w[2 * s1 + 1];
+        if (wbase + kTopoChunk < n) {                  // interior chunk: no clamping (warp-uniform)
+            const u32* wp = w + 2 * (wbase + lane) + 1;
+            #pragma unroll
+            for (int i = 0; i < kTopoItems; ++i) x[i] = wp[64 * i] ^ wp[64 * i + 2];
+        } else {
+            #pragma unroll
+            for (int i = 0; i < kTopoItems; ++i) {
+                const i64 s = wbase + 32 * i + lane;
+                const i64 s0 = s < last ? s : last, s1 = s + 1 < last ? s + 1 : last;
+                x[i] = w[2 * s0 + 1] ^ w[2 * s1 + 1];
+            }
         }
         const u32 xp = wbase > 0 ? (w[2 * wbase - 1] ^ w[2 * wbase + 1]) : 0u;
         #pragma unroll
@@ -100,20 +106,34 @@ topo_count_kernel(const SortedView sv, i64 n, signed char* __restrict__ clev, u3
     // per level that occurs in the chunk (a handful), not atomics per cell
     u32 em[kTopoItems], im[kTopoItems];
     u32 ue = 0u;
-    #pragma unroll
-    for (int i = 0; i < kTopoItems; ++i) {
-        const i64 s = wbase + 32 * i + lane;
-        const bool valid = s < n;
-        const int cs = (valid && s + 1 < n) ? c[i] : -1;
-        int cp = __shfl_up_sync(0xffffffffu, cs, 1);
-        if (lane == 0) cp = cprev;
-        cprev = __shfl_sync(0xffffffffu, cs, 31);
-        em[i] = 0u; im[i] = 0u;
-        if (valid) {
-            clev[s] = (signed char)cs;
+    if (wbase + kTopoChunk < n) {                      // interior chunk: every cell and its successor exist
+        signed char* cl = clev + wbase + lane;
+        #pragma unroll
+        for (int i = 0; i < kTopoItems; ++i) {
+            const int cs = c[i];
+            int cp = __shfl_up_sync(0xffffffffu, cs, 1);
+            if (lane == 0) cp = cprev;
+            cprev = __shfl_sync(0xffffffffu, cs, 31);
+            cl[32 * i] = (signed char)cs;
             entity_masks(cp, cs, im[i], em[i]);
+            ue |= em[i];
         }
-        ue |= em[i];
+    } else {
+        #pragma unroll
+        for (int i = 0; i < kTopoItems; ++i) {
+            const i64 s = wbase + 32 * i + lane;
+            const bool valid = s < n;
+            const int cs = (valid && s + 1 < n) ? c[i] : -1;
+            int cp = __shfl_up_sync(0xffffffffu, cs, 1);
+            if (lane == 0) cp = cprev;
+            cprev = __shfl_sync(0xffffffffu, cs, 31);
+            em[i] = 0u; im[i] = 0u;
+            if (valid) {
+                clev[s] = (signed char)cs;
+                entity_masks(cp, cs, im[i], em[i]);
+            }
+            ue |= em[i];
+        }
     }
     u32 U = __reduce_or_sync(0xffffffffu, ue);
     u32 myE = 0u, myI = 0u;                            // lane l: entities / internal nodes of level l
