@@ -81,6 +81,8 @@ struct bh_ctx {
     DevBuf nlo, nfirst, node_slot, delta64;
     // per slot
     DevBuf rec64, rec, aux;
+    KeyReduce plan_hint = {};             // key OR / AND of the last build: the next build sorts on them
+    bool plan_hint_valid = false;         // without waiting for its own (checked at the second read-back)
     i64 aux_dirty_nn = -1;                // aux is zero except on node_slot[0, aux_dirty_nn); -1: unknown, clear all
     // walk
     DevBuf gcount;
@@ -275,12 +277,22 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
     }
     ctx->direct_ready = false;
 
+    BH_CUDA(cudaEventRecord(ctx->ev[EV_B0], st));
+    // The sort plan (which key bits vary) and the constant key bits come from the OR / AND of all keys.
+    // A solver called every time step sees the same mesh again and again, so the first
+    // attempt takes them from the previous build and runs keys -> sort -> count without a host round
+    // trip; the real OR / AND arrive with the second read-back and must match, else the build is redone
+    // from the keys with the values just read (any plan yields memory-safe, merely useless, passes).
+    i64 nchunks = 0;
+    unsigned tgrid = 0;
+    for (int attempt = 0;; ++attempt) {
+    const bool speculate = attempt == 0 && ctx->plan_hint_valid;
+    ctx->launches_build = 0;
     BH_CUDA(cudaMemsetAsync(ds, 0, sizeof(DeviceScalars), st));
     {   // key_and starts as all ones
         const u64 ones = ~0ULL;
         BH_CUDA(cudaMemcpyAsync(&ds->keyred.key_and, &ones, sizeof(u64), cudaMemcpyHostToDevice, st));
     }
-    BH_CUDA(cudaEventRecord(ctx->ev[EV_B0], st));
 
     // ---- a1: Morton keys ----
     const double s = 2097152.0 / cube[3];      // K1: s = 2^21 / L in fp64
@@ -299,9 +311,12 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
 
     // read-back 1: which key bits vary (decides the radix passes) and the clamp count
     BH_CUDA(cudaMemcpyAsync(&ctx->h_scalars->keyred, &ds->keyred, sizeof(KeyReduce), cudaMemcpyDeviceToHost, st));
-    BH_CUDA(cudaStreamSynchronize(st));
-    ctx->n_clamped = (i64)ctx->h_scalars->keyred.n_clamped;
-    const SortPlan plan = make_sort_plan(ctx->h_scalars->keyred.key_or ^ ctx->h_scalars->keyred.key_and);
+    KeyReduce kr = ctx->plan_hint;
+    if (!speculate) {
+        BH_CUDA(cudaStreamSynchronize(st));
+        kr = ctx->h_scalars->keyred;
+    }
+    const SortPlan plan = make_sort_plan(kr.key_or ^ kr.key_and);
     ctx->sort_passes = plan.npasses;
 
     // ---- a2: radix sort of (key, index) ----
@@ -321,7 +336,7 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
         else if (plan.packed) {
             sv.packed = kres;
             sv.lo = plan.lo;
-            sv.cbits = ctx->h_scalars->keyred.key_and & ~(0xffffffffULL << plan.lo);
+            sv.cbits = kr.key_and & ~(0xffffffffULL << plan.lo);
         } else {
             sv.keys = kres;
             sv.idx = odd ? ctx->idxB.as<u32>() : ctx->idxA.as<u32>();
@@ -333,8 +348,8 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
     ctx->nn = 0; ctx->nslots = 0; ctx->depth = 0; ctx->maxlevel = 0; ctx->max_bucket = 1;
     memset(&ctx->lv, 0, sizeof(ctx->lv));
     if (n >= 2) {
-        const i64 nchunks = topo_chunks(n);
-        const unsigned tgrid = blocks_for(nchunks, kTopoThreads / 32);
+        nchunks = topo_chunks(n);
+        tgrid = blocks_for(nchunks, kTopoThreads / 32);
         u32* hist = ctx->hist.as<u32>();
         topo_count_kernel<<<tgrid, kTopoThreads, 0, st>>>(ctx->sv, n, ctx->clev.as<signed char>(), hist, nchunks);
         BH_CUDA(cudaGetLastError());
@@ -345,8 +360,20 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
         // read-back 2: entities and nodes per level (sizes every node / slot array)
         BH_CUDA(cudaMemcpyAsync(ctx->h_scalars->topo_rows, ds->topo_rows, sizeof(u32) * (kTopoDigits + 1),
                                 cudaMemcpyDeviceToHost, st));
-        BH_CUDA(cudaEventRecord(ctx->ev[EV_PERM], st));
-        BH_CUDA(cudaStreamSynchronize(st));
+    }
+    BH_CUDA(cudaEventRecord(ctx->ev[EV_PERM], st));
+    BH_CUDA(cudaStreamSynchronize(st));
+    {
+        const KeyReduce& real = ctx->h_scalars->keyred;
+        const bool hit = real.key_or == kr.key_or && real.key_and == kr.key_and;
+        ctx->plan_hint = real;
+        ctx->plan_hint_valid = true;
+        ctx->n_clamped = (i64)real.n_clamped;
+        if (hit) break;
+    }
+    }   // attempt
+    if (n >= 2) {
+        u32* hist = ctx->hist.as<u32>();
         const u32* rows = ctx->h_scalars->topo_rows;
         const i64 nslots = rows[kSlotLevels];                 // entities of all levels = n + n_nodes
         const i64 nn = (i64)rows[kTopoDigits] - nslots;
@@ -395,7 +422,6 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
         { int rc = launch_moments(ctx); if (rc != BH_OK) return rc; }
         ctx->aux_dirty_nn = nn;
     } else {
-        BH_CUDA(cudaEventRecord(ctx->ev[EV_PERM], st));
         BH_CUDA(cudaEventRecord(ctx->ev[EV_TOPO], st));
     }
     BH_CUDA(cudaEventRecord(ctx->ev[EV_MOM], st));

@@ -258,3 +258,27 @@ def test_update_masses_equals_rebuild(bh, oracle, w):
     dref = oracle.direct(w.x, w.y, w.z, m2, w.G, targets=tg)
     nz = dref != 0
     assert np.max(np.abs(sub[nz] - dref[nz]) / np.abs(dref[nz])) <= 1e-12
+
+
+def test_context_reuse_across_inputs(bh, oracle):
+    """One context, many builds: the sort plan speculated from the previous build (hit when the same
+    input comes again, miss and redo when another one comes) and the aux records kept zero between
+    builds must leave every build identical to one made in a fresh context."""
+    ctx = bh.Context(0)
+    seq = [CASES[0], CASES[0], CASES[1], CASES[4], CASES[6], CASES[6], CASES[2], CASES[0], DEEP_CHAINS, CASES[3]]
+    for w in seq:
+        ctx.build(_dev(w.x), _dev(w.y), _dev(w.z), _dev(w.m), w.cube)
+        t = _tree_np(ctx)
+        ot = oracle.OracleTree(w.x, w.y, w.z, w.m, w.cube)
+        ok, op = ot.sorted_keys_perm()
+        assert np.array_equal(t["keys"], ok), w.name
+        assert np.array_equal(t["perm"], op), w.name
+        on = ot.nodes()
+        for k in ("level", "prefix", "lo", "hi", "nchild"):
+            assert np.array_equal(t[k].astype(np.int64), on[k].astype(np.int64)), (w.name, k)
+        if w is DEEP_CHAINS:
+            continue
+        phi = ctx.potential(w.theta, w.G).cpu().numpy()
+        ref, ocnt = ot.potential(w.theta, w.G, mac_fp32=True, want_counts=True)
+        _phi_check(phi, ref)
+        assert np.array_equal(ctx.last_group_counts().cpu().numpy(), ocnt), w.name
