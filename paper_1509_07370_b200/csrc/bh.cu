@@ -285,6 +285,7 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
     // from the keys with the values just read (any plan yields memory-safe, merely useless, passes).
     i64 nchunks = 0;
     unsigned tgrid = 0;
+    int aux_cleared = 0;
     for (int attempt = 0;; ++attempt) {
     const bool speculate = attempt == 0 && ctx->plan_hint_valid;
     ctx->launches_build = 0;
@@ -362,7 +363,16 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
                                 cudaMemcpyDeviceToHost, st));
     }
     BH_CUDA(cudaEventRecord(ctx->ev[EV_PERM], st));
-    BH_CUDA(cudaStreamSynchronize(st));
+    // aux must be zero on every leaf slot; only the node slots of the previous build are not.  Clearing
+    // them runs on the device while the host waits for the read-back and prepares the next launches.
+    if (ctx->aux_dirty_nn > 0) {
+        aux_clear_kernel<<<blocks_for(ctx->aux_dirty_nn, 256), 256, 0, st>>>(ctx->node_slot.as<u32>(), ctx->aux_dirty_nn,
+                                                                            ctx->aux.as<WalkAux>());
+        BH_CUDA(cudaGetLastError());
+        ctx->aux_dirty_nn = 0;
+        aux_cleared = 1;
+    }
+    BH_CUDA(cudaEventSynchronize(ctx->ev[EV_PERM]));
     {
         const KeyReduce& real = ctx->h_scalars->keyred;
         const bool hit = real.key_or == kr.key_or && real.key_and == kr.key_and;
@@ -389,19 +399,12 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
             return BH_ERR_CUDA;
         }
 
-        // aux must be zero on every leaf slot; only the node slots of the previous build are not
         {
             const bool grow = sizeof(WalkAux) * (size_t)nslots > ctx->aux.cap;
-            const i64 dirty = ctx->aux_dirty_nn;
-            ctx->aux_dirty_nn = -1;                            // until this build's moments are launched
-            if (!grow && dirty > 0) {
-                aux_clear_kernel<<<blocks_for(dirty, 256), 256, 0, st>>>(ctx->node_slot.as<u32>(), dirty,
-                                                                        ctx->aux.as<WalkAux>());
-                BH_CUDA(cudaGetLastError());
-                ctx->launches_build += 1;
-            }
             BH_CUDA(ctx->aux.ensure(sizeof(WalkAux) * nslots));
-            if (grow || dirty < 0) BH_CUDA(cudaMemsetAsync(ctx->aux.p, 0, ctx->aux.cap, st));
+            if (grow || ctx->aux_dirty_nn < 0) BH_CUDA(cudaMemsetAsync(ctx->aux.p, 0, ctx->aux.cap, st));
+            ctx->aux_dirty_nn = -1;                            // unknown until this build's moments are launched
+            ctx->launches_build += aux_cleared;
         }
         BH_CUDA(ctx->nlo.ensure(sizeof(u32) * nn));
         BH_CUDA(ctx->nfirst.ensure(sizeof(u32) * (nn + 4)));
