@@ -455,3 +455,100 @@ int orc_direct(const double *x, const double *y, const double *z, const double *
     }
     return 0;
 }
+
+/* ---- Find Essential Nodes (§3.2.4, Fig. 7) -------------
+ * The local tree pruned against a remote domain: "Nodes and data cells are treated as essential if
+ * they pass the opening angle test ... a slightly modified version of the opening angle criterion ...
+ * we refer to the minimum distance d_c between the nodes center of mass and the VN".
+ * Reading (E1-E4): the remote domain ("VN" extent) is the axis-aligned box [blo, bhi];
+ * d_c = distance from the node's centre of mass R to the nearest point of the box (0 inside it).
+ * Depth-first from the root: an internal node with d_c > l/theta (+ delta with Eq. 4) is essential
+ * and is sent as ONE point mass (R, M); otherwise it is opened and its children are examined; a
+ * leaf cell reached through an opened parent is essential as it is; a level-21 bucket is always
+ * opened (all its cells are sent).  theta = 0 opens everything (all n cells are sent).  Decisions
+ * in fp64, compared as d_c^2 > r_c^2 (strict), every product and sum rounded separately.
+ * Output: entries in ascending (level, first sorted cell) order -- level of a leaf cell = its
+ * parent's level + 1 -- as rec[4k..4k+3] = (x, y, z, m) ("exchange array ... 4N entries", Fig. 4),
+ * plus (optionally) level[k], lo[k], hi[k] (sorted cell range the entry stands for).
+ * Returns the number of entries (they never exceed n), or < 0 on a bad argument. */
+typedef struct { int32_t level; int64_t lo, hi; double r[4]; } orc_ess;
+
+static int cmp_ess(const void *a, const void *b)
+{
+    const orc_ess *p = (const orc_ess *)a, *q = (const orc_ess *)b;
+    if (p->level != q->level) return p->level < q->level ? -1 : 1;
+    if (p->lo != q->lo) return p->lo < q->lo ? -1 : 1;
+    return 0;
+}
+
+static double box_dist2(const double R[3], const double *blo, const double *bhi)
+{
+    double d2 = 0.0;
+    for (int a = 0; a < 3; ++a) {
+        double d = 0.0;
+        if (R[a] < blo[a]) d = blo[a] - R[a];
+        else if (R[a] > bhi[a]) d = R[a] - bhi[a];
+        d2 = d2 + d * d;
+    }
+    return d2;
+}
+
+int64_t orc_essential_nodes(const orc_tree *t, const double *blo, const double *bhi, double theta, int mac,
+                            double *rec, int32_t *level, int64_t *lo, int64_t *hi)
+{
+    if (!t || !blo || !bhi || !rec || !(theta >= 0.0)) return -1;
+    for (int a = 0; a < 3; ++a) if (!(blo[a] <= bhi[a])) return -1;
+    int64_t n = t->n;
+    orc_ess *out = (orc_ess *)malloc(sizeof(orc_ess) * (size_t)(n > 0 ? n : 1));
+    if (!out) return -2;
+    int64_t cnt = 0;
+    if (n == 1) { /* a lone cell has no tree (T-rule 1): it is sent as it is */
+        orc_ess e = {1, 0, 1, {t->x[0], t->y[0], t->z[0], t->m[0]}};
+        out[cnt++] = e;
+    }
+    int64_t stack[8 * (ORC_MAXLEVEL + 2)];
+    int32_t slev[8 * (ORC_MAXLEVEL + 2)]; /* level of the stacked child reference */
+    int sp = 0;
+    if (n >= 2) { stack[sp] = 0; slev[sp] = 0; ++sp; }
+    while (sp > 0) {
+        --sp;
+        int64_t e = stack[sp];
+        int32_t lev = slev[sp];
+        if (e <= -2) { /* leaf cell */
+            int64_t j = -(e + 2);
+            orc_ess q = {lev, j, j + 1, {t->x[j], t->y[j], t->z[j], t->m[j]}};
+            out[cnt++] = q;
+            continue;
+        }
+        const orc_node *nd = &t->node[e];
+        if (nd->level == ORC_MAXLEVEL) { /* bucket: always opened */
+            for (int64_t j = nd->lo; j < nd->hi; ++j) {
+                orc_ess q = {ORC_MAXLEVEL + 1, j, j + 1, {t->x[j], t->y[j], t->z[j], t->m[j]}};
+                out[cnt++] = q;
+            }
+            continue;
+        }
+        int accept = 0;
+        if (theta > 0.0) {
+            double rc = nd->size / theta;
+            if (mac == ORC_MAC_BARNES94) rc = rc + nd->delta;
+            accept = box_dist2(nd->R, blo, bhi) > rc * rc;
+        }
+        if (accept) {
+            orc_ess q = {nd->level, nd->lo, nd->hi, {nd->R[0], nd->R[1], nd->R[2], nd->M}};
+            out[cnt++] = q;
+            continue;
+        }
+        for (int c = 7; c >= 0; --c)
+            if (nd->child[c] != -1) { stack[sp] = nd->child[c]; slev[sp] = nd->level + 1; ++sp; }
+    }
+    qsort(out, (size_t)cnt, sizeof(orc_ess), cmp_ess);
+    for (int64_t k = 0; k < cnt; ++k) {
+        for (int a = 0; a < 4; ++a) rec[4 * k + a] = out[k].r[a];
+        if (level) level[k] = out[k].level;
+        if (lo) lo[k] = out[k].lo;
+        if (hi) hi[k] = out[k].hi;
+    }
+    free(out);
+    return cnt;
+}

@@ -51,6 +51,8 @@ def _L():
         lib.orc_potential.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_int, C.c_int,
                                       C.c_int64, C.c_int64, dp, i64p]
         lib.orc_direct.argtypes = [dp, dp, dp, dp, C.c_int64, C.c_double, i64p, C.c_int64, dp]
+        lib.orc_essential_nodes.argtypes = [C.c_void_p, dp, dp, C.c_double, C.c_int, dp, i32p, i64p, i64p]
+        lib.orc_essential_nodes.restype = C.c_int64
         _lib = lib
     return _lib
 
@@ -154,3 +156,19 @@ class OracleTree:
         if rc != 0:
             raise ValueError("orc_potential: invalid argument")
         return (phi, counts) if want_counts else phi
+
+    def essential_nodes(self, box_lo, box_hi, theta, mac=MAC_BARNES94, want_ranges=False):
+        """Find Essential Nodes: this tree pruned against the remote domain box
+        [box_lo, box_hi] with the minimum-distance criterion.  Returns rec[k, 4] = (x, y, z, m) in
+        ascending (level, first sorted cell) order and, if asked, (level, lo, hi) per entry."""
+        blo, bhi = _f64(box_lo), _f64(box_hi)
+        rec = np.empty((max(self.n, 1), 4), dtype=np.float64)
+        lev = np.empty(max(self.n, 1), dtype=np.int32)
+        lo = np.empty(max(self.n, 1), dtype=np.int64)
+        hi = np.empty(max(self.n, 1), dtype=np.int64)
+        k = _L().orc_essential_nodes(self._h, _p(blo, C.c_double), _p(bhi, C.c_double), float(theta), int(mac),
+                                     _p(rec, C.c_double), _p(lev, C.c_int32), _p(lo, C.c_int64), _p(hi, C.c_int64))
+        if k < 0:
+            raise ValueError("orc_essential_nodes: invalid argument")
+        rec = rec[:k].copy()
+        return (rec, lev[:k].copy(), lo[:k].copy(), hi[:k].copy()) if want_ranges else rec
