@@ -105,8 +105,9 @@ int bh_set_option(bh_ctx* ctx, int key, int value);
  * identical keys form a level-21 bucket leaf; DESIGN.md T-rules), the cell data being gathered into
  * tree order in the same pass -> bottom-up level-by-level M, R (Eq. 5), delta = |R - geometric
  * centre| in fp64 (DESIGN.md M-rules).
- * Synchronises the stream twice internally to read back (a) which key bits vary and (b) the node
- * count per level; everything else is asynchronous. */
+ * Synchronises the stream internally to read back (a) which key bits vary and (b) the node count per
+ * level -- once when the keys vary on the same bits as in the previous build of this context (the sort
+ * is then started on that assumption and checked afterwards), twice otherwise. */
 int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, const double* m,
              int64_t n, const double cube[4]);
 
@@ -117,6 +118,34 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
  * bh_potential gives bit-identical results to a fresh bh_build with these masses.
  *   m : DEVICE, const double[n], original cell order; borrowed until the stream has passed the call. */
 int bh_update_masses(bh_ctx* ctx, const double* m);
+
+/* bh_essential_nodes: Find Essential Nodes (§3.2.4, Fig. 7) -- the tree of the last
+ * bh_build pruned against a REMOTE DOMAIN, the first half of the locally-essential-tree exchange
+ * (PAPER.md:66, 104-118).  The remote domain (the paper's "VN" with its size) is the axis-aligned box
+ * [box_lo, box_hi]; d_c is the distance from a node's centre of mass to the nearest point of that box
+ * (0 inside).  From the root: an internal node with d_c > l/theta (BH_MAC_BH86) or d_c > l/theta + delta
+ * (BH_MAC_BARNES94, the paper's choice; set with bh_set_option) is essential and is emitted as ONE
+ * point mass (R, M); otherwise it is opened; a leaf cell under an opened node is emitted as it is; a
+ * level-21 bucket is always opened.  theta = 0 emits all n cells.  Decisions are taken in fp64 on the
+ * fp64 moments, so the selected set equals the oracle's exactly.
+ *   box_lo, box_hi : HOST, const double[3], box_lo[a] <= box_hi[a].
+ *   out            : DEVICE, double[4 * cap], 16-byte aligned: entry k = (x, y, z, m) at out[4k..4k+3]
+ *                    (the paper's "exchange array ... holding 4N entries", Fig. 4), in ascending
+ *                    (tree level, first sorted cell) order.  May be NULL when cap == 0 (size query).
+ *   count          : HOST, receives the number of essential entries (1 ... n).
+ * Returns BH_ERR_TOO_LARGE (with *count set, the first cap entries written) when count > cap.
+ * Synchronises the stream once to read the count back. */
+int bh_essential_nodes(bh_ctx* ctx, const double box_lo[3], const double box_hi[3], double theta,
+                       double* out, int64_t cap, int64_t* count);
+
+/* bh_set_num_targets: only the cells with ORIGINAL index < ntargets are targets of the following
+ * bh_potential calls; the others are sources only (-1, the default: every cell is a target).  This is
+ * how a locally essential tree is walked ("Essential Nodes are treated as data cells
+ * during the tree build"): the caller builds over its own cells followed by the received essential
+ * entries and sets ntargets = number of its own cells.  Groups are still 32 consecutive cells of the
+ * sorted order and every member votes (W-rules unchanged, results identical); groups without a target
+ * are skipped, and phi needs only ntargets entries. */
+int bh_set_num_targets(bh_ctx* ctx, int64_t ntargets);
 
 /* bh_potential: Phi_i = -G sum_j m_j/|r_i - r_j| over the nodes and leaf cells the group walk of
  * PAPER.md:176-178 selects (DESIGN.md W-rules).

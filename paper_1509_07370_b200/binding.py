@@ -15,7 +15,7 @@ BH_DIRECT_ALL_MAX = 1 << 18
 EXPORTED_SYMBOLS = (
     "bh_create", "bh_destroy", "bh_strerror", "bh_last_cuda_error", "bh_set_option", "bh_build", "bh_potential",
     "bh_potential_direct", "bh_solve_host", "bh_tree_sizes", "bh_export_tree", "bh_last_group_counts",
-    "bh_last_interactions", "bh_get_stats", "bh_update_masses",
+    "bh_last_interactions", "bh_get_stats", "bh_update_masses", "bh_essential_nodes", "bh_set_num_targets",
 )
 
 
@@ -61,6 +61,9 @@ def lib():
         L.bh_set_option.argtypes = [vp, i32, i32]
         L.bh_build.argtypes = [vp, dp, dp, dp, dp, i64, C.POINTER(C.c_double)]
         L.bh_update_masses.argtypes = [vp, dp]
+        L.bh_essential_nodes.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_double, dp, i64,
+                                         C.POINTER(i64)]
+        L.bh_set_num_targets.argtypes = [vp, i64]
         L.bh_potential.argtypes = [vp, C.c_double, C.c_double, dp]
         L.bh_potential_direct.argtypes = [vp, C.c_double, dp, i64, dp]
         L.bh_solve_host.argtypes = [vp, dp, dp, dp, dp, i64, C.POINTER(C.c_double), C.c_double, C.c_double, dp]
@@ -148,10 +151,34 @@ class Context:
             raise ValueError("m must have the length of the last build")
         self._check(self._L.bh_update_masses(self._h, self._dev(m, self._torch.float64)))
 
+    def essential_nodes(self, box_lo, box_hi, theta: float, cap: int = 0):
+        """bh_essential_nodes: the last build's tree pruned against the remote box; returns a CUDA tensor
+        [count, 4] = (x, y, z, m) per essential entry.  `cap`: first guess of the count (0: query first)."""
+        torch = self._torch
+        lo = (C.c_double * 3)(*[float(v) for v in box_lo])
+        hi = (C.c_double * 3)(*[float(v) for v in box_hi])
+        cnt = C.c_int64(0)
+        TOO_LARGE = -5
+        while True:
+            out = torch.empty((max(cap, 1), 4), dtype=torch.float64, device=f"cuda:{self.device}")
+            rc = self._L.bh_essential_nodes(self._h, lo, hi, float(theta), self._dev(out, torch.float64) if cap else None,
+                                            cap, C.byref(cnt))
+            if rc == TOO_LARGE and cnt.value > cap:
+                cap = int(cnt.value)
+                continue
+            self._check(rc)
+            return out[: cnt.value]
+
+    def set_num_targets(self, ntargets: int):
+        """bh_set_num_targets: cells with original index < ntargets are targets, the rest sources only (-1: all)."""
+        self._check(self._L.bh_set_num_targets(self._h, int(ntargets)))
+        self._ntargets = int(ntargets)
+
     def potential(self, theta: float, G: float = 1.0, out=None):
         torch = self._torch
         if out is None:
-            out = torch.empty(self.n, dtype=torch.float64, device=f"cuda:{self.device}")
+            nt = getattr(self, "_ntargets", -1)
+            out = torch.empty(self.n if nt < 0 else min(nt, self.n), dtype=torch.float64, device=f"cuda:{self.device}")
         self._check(self._L.bh_potential(self._h, float(theta), float(G), self._dev(out, torch.float64)))
         return out
 

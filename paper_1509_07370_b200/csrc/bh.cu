@@ -11,6 +11,7 @@
 #include "common.cuh"
 #include "direct.cuh"
 #include "keys.cuh"
+#include "let.cuh"
 #include "scan.cuh"
 #include "sort.cuh"
 #include "tree.cuh"
@@ -85,6 +86,8 @@ struct bh_ctx {
     bool plan_hint_valid = false;         // without waiting for its own (checked at the second read-back)
     i64 aux_dirty_nn = -1;                // aux is zero except on node_slot[0, aux_dirty_nn); -1: unknown, clear all
     // walk
+    i64 ntargets = -1;                    // bh_set_num_targets: cells [0, ntargets) are targets; -1 = all
+    DevBuf ess_state, ess_emit;           // bh_essential_nodes: per-slot flags
     DevBuf gcount;
     DevBuf scalars;                       // DeviceScalars
     DeviceScalars* h_scalars = nullptr;   // pinned host mirror
@@ -232,7 +235,7 @@ int bh_destroy(bh_ctx* ctx)
     DevBuf* all[] = {&ctx->keysA, &ctx->keysB, &ctx->idxA, &ctx->idxB, &ctx->clev, &ctx->leaf_slot, &ctx->leaf64,
                      &ctx->slot_of, &ctx->hist, &ctx->scan_scratch, &ctx->nlo, &ctx->nfirst, &ctx->node_slot,
                      &ctx->delta64, &ctx->rec64, &ctx->rec, &ctx->aux, &ctx->gcount, &ctx->scalars, &ctx->stage[0],
-                     &ctx->stage[1], &ctx->stage[2], &ctx->stage[3], &ctx->stage_phi};
+                     &ctx->stage[1], &ctx->stage[2], &ctx->stage[3], &ctx->stage_phi, &ctx->ess_state, &ctx->ess_emit};
     for (DevBuf* b : all) b->release();
     if (ctx->h_scalars) cudaFreeHost(ctx->h_scalars);
     for (int i = 0; i < EV_COUNT; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
@@ -425,6 +428,11 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
         { int rc = launch_moments(ctx); if (rc != BH_OK) return rc; }
         ctx->aux_dirty_nn = nn;
     } else {
+        // n = 1: no tree (T-rule 1); the lone cell's record is kept for bh_essential_nodes
+        BH_CUDA(ctx->rec64.ensure(sizeof(double4)));
+        const double* src[4] = {x, y, z, m};
+        for (int a = 0; a < 4; ++a)
+            BH_CUDA(cudaMemcpyAsync(ctx->rec64.as<double>() + a, src[a], sizeof(double), cudaMemcpyDeviceToDevice, st));
         BH_CUDA(cudaEventRecord(ctx->ev[EV_TOPO], st));
     }
     BH_CUDA(cudaEventRecord(ctx->ev[EV_MOM], st));
@@ -454,6 +462,79 @@ int bh_update_masses(bh_ctx* ctx, const double* m)
     }
     BH_CUDA(cudaEventRecord(ctx->ev[EV_MOM], st));
     return BH_OK;
+}
+
+int bh_set_num_targets(bh_ctx* ctx, int64_t ntargets)
+{
+    if (!ctx || ntargets < -1) return BH_ERR_INVALID_ARG;
+    ctx->ntargets = ntargets;
+    ctx->walked = false;
+    ctx->counts_valid = false;
+    return BH_OK;
+}
+
+int bh_essential_nodes(bh_ctx* ctx, const double box_lo[3], const double box_hi[3], double theta, double* out,
+                       int64_t cap, int64_t* count)
+{
+    if (!ctx || !box_lo || !box_hi || !count || cap < 0 || (cap > 0 && !out) || !(theta >= 0.0)) return BH_ERR_INVALID_ARG;
+    for (int a = 0; a < 3; ++a) if (!(box_lo[a] <= box_hi[a])) return BH_ERR_INVALID_ARG;
+    if (cap > 0 && !aligned16(out)) return BH_ERR_INVALID_ARG;
+    if (!ctx->built) return BH_ERR_NOT_BUILT;
+    BH_CUDA(cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    *count = 0;
+    if (ctx->n == 1) {                       // a lone cell is sent as it is
+        *count = 1;
+        if (cap < 1) return BH_ERR_TOO_LARGE;
+        BH_CUDA(cudaMemcpyAsync(out, ctx->rec64.p, sizeof(double) * 4, cudaMemcpyDeviceToDevice, st));
+        return BH_OK;
+    }
+    DeviceScalars* ds = ctx->scalars.as<DeviceScalars>();
+    const i64 nslots = ctx->nslots;
+    BH_CUDA(ctx->ess_state.ensure((size_t)nslots + 16));
+    BH_CUDA(ctx->ess_emit.ensure(sizeof(u32) * ((size_t)nslots + 4)));
+    BH_CUDA(ctx->scan_scratch.ensure(sizeof(u32) * (scan_scratch_elems(nslots) + 4)));
+    BH_CUDA(cudaMemsetAsync(ctx->ess_state.p, 0, (size_t)nslots, st));
+    BH_CUDA(cudaMemsetAsync(ctx->ess_emit.p, 0, sizeof(u32) * (size_t)nslots, st));
+    BH_CUDA(cudaMemsetAsync(ctx->ess_state.p, 1, 1, st));        // the root (slot 0) is tested like any node
+    EssArgs A;
+    A.nfirst = ctx->nfirst.as<u32>(); A.node_slot = ctx->node_slot.as<u32>(); A.rec64 = ctx->rec64.as<double4>();
+    A.delta64 = ctx->delta64.as<double>(); A.aux = ctx->aux.as<WalkAux>();
+    A.state = ctx->ess_state.as<unsigned char>(); A.emit = ctx->ess_emit.as<u32>();
+    for (int a = 0; a < 3; ++a) { A.blo[a] = box_lo[a]; A.bhi[a] = box_hi[a]; }
+    A.theta = theta; A.L = ctx->cube[3]; A.mac = ctx->mac;
+    SmallLevels sl;
+    sl.nlev = 0;
+    for (int l = 0; l <= ctx->maxlevel + 1; ++l) {      // root side first; one extra turn flushes the last run
+        const bool last = l > ctx->maxlevel;
+        const i64 b0 = last ? 0 : ctx->lv.node_base[l], b1 = last ? 0 : ctx->lv.node_base[l + 1];
+        const bool small = !last && b1 - b0 <= kEssSmallNodes;
+        if ((!small || last) && sl.nlev > 0) {
+            ess_small_kernel<<<1, 1024, 0, st>>>(sl, A);
+            BH_CUDA(cudaGetLastError());
+            sl.nlev = 0;
+        }
+        if (last || b1 == b0) continue;
+        if (small) {
+            sl.level[sl.nlev] = l; sl.b0[sl.nlev] = (u32)b0; sl.b1[sl.nlev] = (u32)b1;
+            sl.slot_end[sl.nlev] = ctx->lv.slot_base[l + 2];
+            ++sl.nlev;
+        } else {
+            ess_level_kernel<<<blocks_for(b1 - b0, 256), 256, 0, st>>>(b0, b1, l, ctx->lv.slot_base[l + 2], A);
+            BH_CUDA(cudaGetLastError());
+        }
+    }
+    BH_CUDA(exclusive_scan_u32(ctx->ess_emit.as<u32>(), ctx->ess_emit.as<u32>(), nslots, ctx->scan_scratch.as<u32>(),
+                               &ds->scan_total, st));
+    if (cap > 0) {
+        ess_gather_kernel<<<blocks_for(nslots, 256), 256, 0, st>>>(ctx->ess_emit.as<u32>(), nslots, &ds->scan_total,
+                                                                  ctx->rec64.as<double4>(), out, cap);
+        BH_CUDA(cudaGetLastError());
+    }
+    BH_CUDA(cudaMemcpyAsync(&ctx->h_scalars->scan_total, &ds->scan_total, sizeof(u32), cudaMemcpyDeviceToHost, st));
+    BH_CUDA(cudaStreamSynchronize(st));
+    *count = (int64_t)ctx->h_scalars->scan_total;
+    return *count > cap ? BH_ERR_TOO_LARGE : BH_OK;
 }
 
 }  // extern "C" (reopened below)
@@ -486,6 +567,7 @@ int launch_walk(bh_ctx* ctx, double theta, double G, double* phi, int group, int
     P.mac = mac;
     P.negG = -G;
     P.stack_cap = 0;
+    P.ntargets = ctx->ntargets < 0 ? 0xffffffffu : (u32)(ctx->ntargets < n ? ctx->ntargets : n);
     if (group == 32) {
         i64 cap = (i64)kStackPerLevel * (ctx->maxlevel + 2) + 32;
         cap = (cap + 1) & ~1LL;

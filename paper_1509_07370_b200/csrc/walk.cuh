@@ -58,6 +58,7 @@ struct WalkParams {
     int mac;                  // BH_MAC_*
     double negG;
     int stack_cap;            // entries per warp
+    u32 ntargets;             // only cells with original index < ntargets are targets (bh_set_num_targets)
 };
 
 __host__ __device__ inline size_t walk_smem_per_warp(int stack_cap)
@@ -236,6 +237,18 @@ walk_pair_kernel(const WalkParams P)
     const int ntB = hasB ? (int)min((i64)32, P.n - gB * 32) : 0;
     const bool liveA = (int)lane < ntA, liveB = (int)lane < ntB;
     const i64 sA = gA * 32 + lane, sB = gB * 32 + lane;
+    if (P.ntargets != 0xffffffffu) {
+        // source-only cells (essential nodes received from other domains) sit in long runs
+        // of the sorted order: a pair of groups without a single target has nothing to compute
+        const bool want = (liveA && sv_idx(P.sv, sA) < P.ntargets) || (liveB && sv_idx(P.sv, sB) < P.ntargets);
+        if (!__any_sync(0xffffffffu, want)) {
+            if (COUNT && lane == 0) {
+                P.gcount[gA] = make_uint4(0u, 0u, 0u, 0u);
+                if (hasB) P.gcount[gB] = make_uint4(0u, 0u, 0u, 0u);
+            }
+            return;
+        }
+    }
     const float4 tA = __ldg(P.rec + __ldg(P.leaf_slot + (liveA ? sA : gA * 32)));
     const float4 tB = __ldg(P.rec + __ldg(P.leaf_slot + (liveB ? sB : (hasB ? gB * 32 : gA * 32))));
     Box2 box;                                         // bounding boxes of the live targets of A and B
@@ -414,8 +427,8 @@ walk_pair_kernel(const WalkParams P)
     }
     if (nC > 0) eval_c(C, Cm, nC, npx, npy, npz, accA, accB);
     // ---- a7: Phi_t = -G * sum, written in the original cell order (W-rule 4) ----
-    if (liveA) P.phi[sv_idx(P.sv, sA)] = P.negG * accA;
-    if (liveB) P.phi[sv_idx(P.sv, sB)] = P.negG * accB;
+    if (liveA) { const u32 o = sv_idx(P.sv, sA); if (o < P.ntargets) P.phi[o] = P.negG * accA; }
+    if (liveB) { const u32 o = sv_idx(P.sv, sB); if (o < P.ntargets) P.phi[o] = P.negG * accB; }
 }
 
 // ---- BH_OPT_GROUP = 1 (W5): every target walks alone --------------------------------------------
@@ -429,6 +442,7 @@ walk_single_kernel(const WalkParams P)
 {
     const i64 s = (i64)blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= P.n) return;
+    if (sv_idx(P.sv, s) >= P.ntargets) { P.gcount[s] = make_uint4(0u, 0u, 0u, 0u); return; }
     const float4 tp = __ldg(P.rec + __ldg(P.leaf_slot + s));
     u32 st_first[kSingleStack], st_count[kSingleStack];
     int sp = 0;
