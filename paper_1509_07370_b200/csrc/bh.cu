@@ -221,6 +221,10 @@ int bh_create(bh_ctx** out, int device, void* cuda_stream)
                                       227 * 1024)) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(walk)"); break; }
         if ((e = cudaFuncSetAttribute(walk_pair_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       227 * 1024)) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(walk count)"); break; }
+        if ((e = cudaFuncSetAttribute(walk_pair_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      227 * 1024)) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(walk subset)"); break; }
+        if ((e = cudaFuncSetAttribute(walk_pair_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      227 * 1024)) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(walk subset count)"); break; }
     } while (0);
     if (rc != BH_OK) { bh_destroy(ctx); return rc; }
     *out = ctx;
@@ -575,8 +579,13 @@ int launch_walk(bh_ctx* ctx, double theta, double G, double* phi, int group, int
         if (smem > 227 * 1024) return BH_ERR_TOO_LARGE;
         P.stack_cap = (int)cap;
         const i64 npairs = (ngroups + 1) / 2;
-        if (count_only)
+        const bool subset = P.ntargets != 0xffffffffu;
+        if (count_only && subset)
+            walk_pair_kernel<true, true><<<blocks_for(npairs, kWalkWarps), kWalkWarps * 32, smem, st>>>(P);
+        else if (count_only)
             walk_pair_kernel<true><<<blocks_for(npairs, kWalkWarps), kWalkWarps * 32, smem, st>>>(P);
+        else if (subset)
+            walk_pair_kernel<false, true><<<blocks_for(npairs, kWalkWarps), kWalkWarps * 32, smem, st>>>(P);
         else
             walk_pair_kernel<false><<<blocks_for(npairs, kWalkWarps), kWalkWarps * 32, smem, st>>>(P);
     } else {

@@ -211,7 +211,9 @@ __device__ __forceinline__ void box_d2(const float4 q, const Box2& b, float2& d2
 // COUNT = true : the same traversal and the same decisions, but it only counts (W6): per group
 //                {internal nodes accepted, leaf cells summed, internal nodes opened, nodes that
 //                needed the per-member test}; no lists, no arithmetic on masses, no Phi.
-template <bool COUNT>
+// SUBSET = true: only cells with original index < P.ntargets are targets (bh_set_num_targets); the
+//                default instantiation carries none of that code.
+template <bool COUNT, bool SUBSET = false>
 __global__ void __launch_bounds__(kWalkWarps * 32, 3)
 walk_pair_kernel(const WalkParams P)
 {
@@ -237,7 +239,7 @@ walk_pair_kernel(const WalkParams P)
     const int ntB = hasB ? (int)min((i64)32, P.n - gB * 32) : 0;
     const bool liveA = (int)lane < ntA, liveB = (int)lane < ntB;
     const i64 sA = gA * 32 + lane, sB = gB * 32 + lane;
-    if (P.ntargets != 0xffffffffu) {
+    if (SUBSET) {
         // source-only cells (essential nodes received from other domains) sit in long runs
         // of the sorted order: a pair of groups without a single target has nothing to compute
         const bool want = (liveA && sv_idx(P.sv, sA) < P.ntargets) || (liveB && sv_idx(P.sv, sB) < P.ntargets);
@@ -427,8 +429,8 @@ walk_pair_kernel(const WalkParams P)
     }
     if (nC > 0) eval_c(C, Cm, nC, npx, npy, npz, accA, accB);
     // ---- a7: Phi_t = -G * sum, written in the original cell order (W-rule 4) ----
-    if (liveA) { const u32 o = sv_idx(P.sv, sA); if (o < P.ntargets) P.phi[o] = P.negG * accA; }
-    if (liveB) { const u32 o = sv_idx(P.sv, sB); if (o < P.ntargets) P.phi[o] = P.negG * accB; }
+    if (liveA) { const u32 o = sv_idx(P.sv, sA); if (!SUBSET || o < P.ntargets) P.phi[o] = P.negG * accA; }
+    if (liveB) { const u32 o = sv_idx(P.sv, sB); if (!SUBSET || o < P.ntargets) P.phi[o] = P.negG * accB; }
 }
 
 // ---- BH_OPT_GROUP = 1 (W5): every target walks alone --------------------------------------------

@@ -116,16 +116,17 @@ def test_let_equals_oracle_procedure_and_direct_sum(bh, oracle, w, P):
     phis, sent = let.let_potential_serial(dparts, w.cube, theta, w.G, mac=mac)
     ophis, osent = _oracle_let(oracle, w, parts, theta, mac)
     assert sent == osent
-    exact = oracle.direct(w.x, w.y, w.z, w.m, w.G)
+    rng = np.random.default_rng(7)
     for i, p, op in zip(parts, phis, ophis):
         p = p.cpu().numpy()
         assert p.shape == op.shape
         nz = op != 0
         rel = np.abs(p[nz] - op[nz]) / np.abs(op[nz])
         assert rel.max() <= 1e-4 and np.median(rel) <= 1e-6, (rel.max(), np.median(rel))
-        ex = exact[i]
+        sub = rng.choice(len(i), size=min(256, len(i)), replace=False)     # direct sum on a sample of the domain's cells
+        ex = oracle.direct(w.x, w.y, w.z, w.m, w.G, targets=i[sub].astype(np.int64))
         nz = ex != 0
-        err = np.abs(p[nz] - ex[nz]) / np.abs(ex[nz])
+        err = np.abs(p[sub][nz] - ex[nz]) / np.abs(ex[nz])
         assert err.max() < 1e-2 and np.median(err) < 2e-3, (err.max(), np.median(err))    # theta = 0.5
     # far fewer entries travel than cells exist (the point of the LET)
     assert sum(map(sum, sent)) < (P - 1) * w.n
