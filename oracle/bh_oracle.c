@@ -324,7 +324,9 @@ int orc_export_nodes(const orc_tree *t, int32_t *level, uint64_t *prefix, int64_
 /* ---- walk (W-rules) ---------------------------------------------------------------------------- */
 /* A leaf cell j reached through an opened parent: every member t != j adds m_j/|r_t - r_j|
  * (Eq. 2, j != i by sorted slot; distinct cells at zero distance are skipped, W-rule 3). */
-static void add_leaf_cell(const orc_tree *t, int64_t j, int64_t t0, int nt, double *acc)
+/* g (may be NULL): per member 3 sums of m_j (r_j - r_t)/d^3, the acceleration before the factor G
+ * (NEXT-4: g_t = -grad Phi_t = -G sum_j m_j (r_t - r_j)/|r_t - r_j|^3). */
+static void add_leaf_cell(const orc_tree *t, int64_t j, int64_t t0, int nt, double *acc, double *g)
 {
     for (int a = 0; a < nt; ++a) {
         int64_t s = t0 + a;
@@ -333,6 +335,10 @@ static void add_leaf_cell(const orc_tree *t, int64_t j, int64_t t0, int nt, doub
         double d2 = dx * dx + dy * dy + dz * dz;
         if (d2 == 0.0) continue;
         acc[a] += t->m[j] / sqrt(d2);
+        if (g) {
+            double w = t->m[j] / (d2 * sqrt(d2));
+            g[3 * a + 0] -= w * dx; g[3 * a + 1] -= w * dy; g[3 * a + 2] -= w * dz;
+        }
     }
 }
 
@@ -372,8 +378,9 @@ static int group_accepts(const orc_tree *t, const orc_node *nd, double theta, in
 /* Walks groups [group_begin, group_end) of `group` consecutive sorted targets (W-rule 1).
  * phi_orig: length n, ORIGINAL order; only the walked targets are written.
  * counts (may be NULL): per walked group {accepted nodes, leaf cells summed, opened nodes}. */
-int orc_potential(const orc_tree *t, double theta, double G, int mac, int group, int mac_fp32,
-                  int64_t group_begin, int64_t group_end, double *phi_orig, int64_t *counts)
+static int walk_groups(const orc_tree *t, double theta, double G, int mac, int group, int mac_fp32,
+                       int64_t group_begin, int64_t group_end, double *phi_orig, int64_t *counts,
+                       double *acc_orig /* NULL or [3n]: (gx, gy, gz) per cell, ORIGINAL order */)
 {
     if (!t || !phi_orig || !(theta >= 0.0) || group < 1) return -1;
     int64_t n = t->n;
@@ -384,26 +391,28 @@ int orc_potential(const orc_tree *t, double theta, double G, int mac, int group,
      * depth-first: at most 7 waiting siblings per level plus the current entry */
     int64_t stack[8 * (ORC_MAXLEVEL + 2)];
     double *acc = (double *)malloc(sizeof(double) * (size_t)group);
-    if (!acc) return -2;
+    double *gr = acc_orig ? (double *)malloc(sizeof(double) * 3 * (size_t)group) : NULL;
+    if (!acc || (acc_orig && !gr)) { free(acc); free(gr); return -2; }
     for (int64_t g = group_begin; g < group_end; ++g) {
         int64_t t0 = g * group, t1 = t0 + group;
         if (t1 > n) t1 = n;
         int nt = (int)(t1 - t0);
         for (int a = 0; a < nt; ++a) acc[a] = 0.0;
+        if (gr) for (int a = 0; a < 3 * nt; ++a) gr[a] = 0.0;
         int64_t n_acc = 0, n_leaf = 0, n_open = 0;
         int sp = 0;
         if (n >= 2) stack[sp++] = 0; /* root tested like any other node (W-rule 2); n = 1: Phi = 0 */
         while (sp > 0) {
             int64_t e = stack[--sp];
             if (e <= -2) { /* leaf cell */
-                add_leaf_cell(t, -(e + 2), t0, nt, acc);
+                add_leaf_cell(t, -(e + 2), t0, nt, acc, gr);
                 ++n_leaf;
                 continue;
             }
             const orc_node *nd = &t->node[e];
             if (nd->level == ORC_MAXLEVEL) { /* bucket leaf: all its cells summed directly (T-rule 3) */
                 for (int64_t j = nd->lo; j < nd->hi; ++j) {
-                    add_leaf_cell(t, j, t0, nt, acc);
+                    add_leaf_cell(t, j, t0, nt, acc, gr);
                     ++n_leaf;
                 }
                 continue;
@@ -413,6 +422,11 @@ int orc_potential(const orc_tree *t, double theta, double G, int mac, int group,
                     int64_t s = t0 + a;
                     double dx = t->x[s] - nd->R[0], dy = t->y[s] - nd->R[1], dz = t->z[s] - nd->R[2];
                     acc[a] += nd->M / sqrt(dx * dx + dy * dy + dz * dz);
+                    if (gr) { /* the node acts as the point mass (R, M) */
+                        double d2 = dx * dx + dy * dy + dz * dz;
+                        double w = nd->M / (d2 * sqrt(d2));
+                        gr[3 * a + 0] -= w * dx; gr[3 * a + 1] -= w * dy; gr[3 * a + 2] -= w * dz;
+                    }
                 }
                 ++n_acc;
                 continue;
@@ -422,13 +436,33 @@ int orc_potential(const orc_tree *t, double theta, double G, int mac, int group,
                 if (nd->child[c] != -1) stack[sp++] = nd->child[c];
         }
         for (int a = 0; a < nt; ++a) phi_orig[t->perm[t0 + a]] = -G * acc[a]; /* W-rule 4 */
+        if (gr)
+            for (int a = 0; a < nt; ++a)
+                for (int k = 0; k < 3; ++k) acc_orig[3 * (int64_t)t->perm[t0 + a] + k] = G * gr[3 * a + k];
         if (counts) {
             int64_t *c = counts + 3 * (g - group_begin);
             c[0] = n_acc; c[1] = n_leaf; c[2] = n_open;
         }
     }
     free(acc);
+    free(gr);
     return 0;
+}
+
+int orc_potential(const orc_tree *t, double theta, double G, int mac, int group, int mac_fp32,
+                  int64_t group_begin, int64_t group_end, double *phi_orig, int64_t *counts)
+{
+    return walk_groups(t, theta, G, mac, group, mac_fp32, group_begin, group_end, phi_orig, counts, NULL);
+}
+
+/* NEXT-4 (the paper returns Phi and lets the host code difference it):
+ * the same walk, the same interaction lists, additionally g_t = -grad Phi_t evaluated on every
+ * accepted node and leaf cell as the gradient of its monopole term: -G M (r_t - R)/|r_t - R|^3. */
+int orc_field(const orc_tree *t, double theta, double G, int mac, int group, int mac_fp32,
+              int64_t group_begin, int64_t group_end, double *phi_orig, double *acc_orig, int64_t *counts)
+{
+    if (!acc_orig) return -1;
+    return walk_groups(t, theta, G, mac, group, mac_fp32, group_begin, group_end, phi_orig, counts, acc_orig);
 }
 
 /* ---- direct summation, Eq. 2 written out ------------------------------------------
@@ -551,4 +585,29 @@ int64_t orc_essential_nodes(const orc_tree *t, const double *blo, const double *
     }
     free(out);
     return cnt;
+}
+
+/* ---- direct summation of the acceleration (NEXT-4): g_i = -grad Phi_i of Eq. 2 written out ---------
+ * g_i = -G sum_{j != i} m_j (r_i - r_j)/|r_i - r_j|^3, acc[3a..3a+2] for the a-th target (original
+ * indices; targets == NULL: all n).  Sources in original order; zero-distance pairs skipped. */
+int orc_direct_acc(const double *x, const double *y, const double *z, const double *m, int64_t n, double G,
+                   const int64_t *targets, int64_t nt, double *acc)
+{
+    if (!x || !y || !z || !m || !acc || n <= 0) return -1;
+    int64_t count = targets ? nt : n;
+    for (int64_t a = 0; a < count; ++a) {
+        int64_t i = targets ? targets[a] : a;
+        if (i < 0 || i >= n) return -1;
+        double sx = 0.0, sy = 0.0, sz = 0.0;
+        for (int64_t j = 0; j < n; ++j) {
+            if (j == i) continue;
+            double dx = x[i] - x[j], dy = y[i] - y[j], dz = z[i] - z[j];
+            double d2 = dx * dx + dy * dy + dz * dz;
+            if (d2 == 0.0) continue;
+            double w = m[j] / (d2 * sqrt(d2));
+            sx -= w * dx; sy -= w * dy; sz -= w * dz;
+        }
+        acc[3 * a + 0] = G * sx; acc[3 * a + 1] = G * sy; acc[3 * a + 2] = G * sz;
+    }
+    return 0;
 }

@@ -51,6 +51,9 @@ def _L():
         lib.orc_potential.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_int, C.c_int,
                                       C.c_int64, C.c_int64, dp, i64p]
         lib.orc_direct.argtypes = [dp, dp, dp, dp, C.c_int64, C.c_double, i64p, C.c_int64, dp]
+        lib.orc_field.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_int, C.c_int,
+                                  C.c_int64, C.c_int64, dp, dp, i64p]
+        lib.orc_direct_acc.argtypes = [dp, dp, dp, dp, C.c_int64, C.c_double, i64p, C.c_int64, dp]
         lib.orc_essential_nodes.argtypes = [C.c_void_p, dp, dp, C.c_double, C.c_int, dp, i32p, i64p, i64p]
         lib.orc_essential_nodes.restype = C.c_int64
         _lib = lib
@@ -102,6 +105,20 @@ def direct(x, y, z, m, G=1.0, targets=None):
     if rc != 0:
         raise ValueError("orc_direct: invalid argument")
     return phi
+
+
+def direct_acc(x, y, z, m, G=1.0, targets=None):
+    """g_i = -grad Phi_i of Eq. 2 written out: -G sum_{j!=i} m_j (r_i-r_j)/|r_i-r_j|^3; returns [count, 3]."""
+    x, y, z, m = _f64(x), _f64(y), _f64(z), _f64(m)
+    n = x.shape[0]
+    t = None if targets is None else np.ascontiguousarray(targets, dtype=np.int64)
+    cnt = n if t is None else t.shape[0]
+    acc = np.empty((cnt, 3), dtype=np.float64)
+    rc = _L().orc_direct_acc(_p(x, C.c_double), _p(y, C.c_double), _p(z, C.c_double), _p(m, C.c_double), n, G,
+                             None if t is None else _p(t, C.c_int64), cnt, _p(acc, C.c_double))
+    if rc != 0:
+        raise ValueError("orc_direct_acc: invalid argument")
+    return acc
 
 
 class OracleTree:
@@ -172,3 +189,14 @@ class OracleTree:
             raise ValueError("orc_essential_nodes: invalid argument")
         rec = rec[:k].copy()
         return (rec, lev[:k].copy(), lo[:k].copy(), hi[:k].copy()) if want_ranges else rec
+
+    def field(self, theta, G=1.0, mac=MAC_BH86, group=32, mac_fp32=False):
+        """NEXT-4: the group walk returning (phi[n], acc[n, 3]) in ORIGINAL order; acc = -grad phi evaluated
+        on the same interaction lists (monopole gradient of every accepted node and leaf cell)."""
+        phi = np.full(self.n, np.nan)
+        acc = np.full((self.n, 3), np.nan)
+        rc = _L().orc_field(self._h, float(theta), float(G), int(mac), int(group), int(bool(mac_fp32)),
+                            0, -1, _p(phi, C.c_double), _p(acc, C.c_double), None)
+        if rc != 0:
+            raise ValueError("orc_field: invalid argument")
+        return phi, acc
