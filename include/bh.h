@@ -156,6 +156,16 @@ int bh_set_num_targets(bh_ctx* ctx, int64_t ntargets);
  * fp64 sums.  The opening decision of a node is taken in fp32 exactly as DESIGN.md W8 states. */
 int bh_potential(bh_ctx* ctx, double theta, double G, double* phi);
 
+/* bh_field: bh_potential plus the acceleration g_i = -grad Phi_i in the same walk (
+ * the paper returns Phi only and lets the host code difference it).  The interaction lists,
+ * the opening decisions and the arithmetic of Phi are exactly those of bh_potential (phi is bit-equal);
+ * every accepted node and leaf cell additionally contributes the gradient of its monopole term,
+ *   g_i = -G sum_j m_j (r_i - r_j) / |r_i - r_j|^3     (j != i; zero-distance pairs skipped),
+ * evaluated in fp32 with blocked accumulation into fp64 like Phi.
+ *   phi : DEVICE, double[n] (or [ntargets]), original order.
+ *   acc : DEVICE, double[3 n] (or [3 ntargets]): (gx, gy, gz) of cell i at acc[3i .. 3i+2]. */
+int bh_field(bh_ctx* ctx, double theta, double G, double* phi, double* acc);
+
 /* bh_potential_direct: Eq. 2 written out in fp64,
  * Phi_i = -G sum_{j != i} m_j/|r_i - r_j| over ALL n cells of the last build.
  *   targets : DEVICE, const int64_t[nt] original cell indices in [0, n), or NULL for all n cells

@@ -190,13 +190,16 @@ class OracleTree:
         rec = rec[:k].copy()
         return (rec, lev[:k].copy(), lo[:k].copy(), hi[:k].copy()) if want_ranges else rec
 
-    def field(self, theta, G=1.0, mac=MAC_BH86, group=32, mac_fp32=False):
+    def field(self, theta, G=1.0, mac=MAC_BH86, group=32, mac_fp32=False, groups=None):
         """NEXT-4: the group walk returning (phi[n], acc[n, 3]) in ORIGINAL order; acc = -grad phi evaluated
-        on the same interaction lists (monopole gradient of every accepted node and leaf cell)."""
+        on the same interaction lists (monopole gradient of every accepted node and leaf cell).
+        `groups` = (begin, end) restricts the walk; cells not walked stay NaN."""
+        ng = (self.n + group - 1) // group
+        gb, ge = (0, ng) if groups is None else groups
         phi = np.full(self.n, np.nan)
         acc = np.full((self.n, 3), np.nan)
         rc = _L().orc_field(self._h, float(theta), float(G), int(mac), int(group), int(bool(mac_fp32)),
-                            0, -1, _p(phi, C.c_double), _p(acc, C.c_double), None)
+                            gb, ge, _p(phi, C.c_double), _p(acc, C.c_double), None)
         if rc != 0:
             raise ValueError("orc_field: invalid argument")
         return phi, acc

@@ -15,7 +15,7 @@ BH_DIRECT_ALL_MAX = 1 << 18
 EXPORTED_SYMBOLS = (
     "bh_create", "bh_destroy", "bh_strerror", "bh_last_cuda_error", "bh_set_option", "bh_build", "bh_potential",
     "bh_potential_direct", "bh_solve_host", "bh_tree_sizes", "bh_export_tree", "bh_last_group_counts",
-    "bh_last_interactions", "bh_get_stats", "bh_update_masses", "bh_essential_nodes", "bh_set_num_targets",
+    "bh_last_interactions", "bh_get_stats", "bh_update_masses", "bh_essential_nodes", "bh_set_num_targets", "bh_field",
 )
 
 
@@ -65,6 +65,7 @@ def lib():
                                          C.POINTER(i64)]
         L.bh_set_num_targets.argtypes = [vp, i64]
         L.bh_potential.argtypes = [vp, C.c_double, C.c_double, dp]
+        L.bh_field.argtypes = [vp, C.c_double, C.c_double, dp, dp]
         L.bh_potential_direct.argtypes = [vp, C.c_double, dp, i64, dp]
         L.bh_solve_host.argtypes = [vp, dp, dp, dp, dp, i64, C.POINTER(C.c_double), C.c_double, C.c_double, dp]
         L.bh_tree_sizes.argtypes = [vp, C.POINTER(i64), C.POINTER(i64), C.POINTER(i64)]
@@ -181,6 +182,17 @@ class Context:
             out = torch.empty(self.n if nt < 0 else min(nt, self.n), dtype=torch.float64, device=f"cuda:{self.device}")
         self._check(self._L.bh_potential(self._h, float(theta), float(G), self._dev(out, torch.float64)))
         return out
+
+    def field(self, theta: float, G: float = 1.0):
+        """bh_field: (phi[n], acc[n, 3]) -- the potential and g = -grad phi from the same walk."""
+        torch = self._torch
+        nt = getattr(self, "_ntargets", -1)
+        cnt = self.n if nt < 0 else min(nt, self.n)
+        phi = torch.empty(cnt, dtype=torch.float64, device=f"cuda:{self.device}")
+        acc = torch.empty((cnt, 3), dtype=torch.float64, device=f"cuda:{self.device}")
+        self._check(self._L.bh_field(self._h, float(theta), float(G), self._dev(phi, torch.float64),
+                                     self._dev(acc, torch.float64)))
+        return phi, acc
 
     def potential_direct(self, G: float = 1.0, targets=None, out=None):
         torch = self._torch

@@ -223,6 +223,10 @@ int bh_create(bh_ctx** out, int device, void* cuda_stream)
                                       227 * 1024)) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(walk count)"); break; }
         if ((e = cudaFuncSetAttribute(walk_pair_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       227 * 1024)) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(walk subset)"); break; }
+        if ((e = cudaFuncSetAttribute(walk_pair_kernel<false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      227 * 1024)) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(walk field)"); break; }
+        if ((e = cudaFuncSetAttribute(walk_pair_kernel<false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      227 * 1024)) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(walk field subset)"); break; }
         if ((e = cudaFuncSetAttribute(walk_pair_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       227 * 1024)) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(walk subset count)"); break; }
     } while (0);
@@ -547,7 +551,8 @@ namespace {
 
 // Launches the walk of the last build on the context's stream.  count_only: the traversal of
 // walk_pair_kernel<true> (same decisions, no arithmetic on masses), filling ctx->gcount.
-int launch_walk(bh_ctx* ctx, double theta, double G, double* phi, int group, int mac, bool count_only)
+int launch_walk(bh_ctx* ctx, double theta, double G, double* phi, int group, int mac, bool count_only,
+                double* acc = nullptr)
 {
     cudaStream_t st = ctx->stream;
     const i64 n = ctx->n;
@@ -555,6 +560,7 @@ int launch_walk(bh_ctx* ctx, double theta, double G, double* phi, int group, int
     BH_CUDA(ctx->gcount.ensure(sizeof(uint4) * ngroups));
     if (n == 1) {   // T-rule 1: a lone cell has no tree; Phi = 0
         if (!count_only) BH_CUDA(cudaMemsetAsync(phi, 0, sizeof(double), st));
+        if (!count_only && acc) BH_CUDA(cudaMemsetAsync(acc, 0, 3 * sizeof(double), st));
         BH_CUDA(cudaMemsetAsync(ctx->gcount.p, 0, sizeof(uint4), st));
         return BH_OK;
     }
@@ -564,6 +570,7 @@ int launch_walk(bh_ctx* ctx, double theta, double G, double* phi, int group, int
     P.leaf_slot = ctx->leaf_slot.as<u32>();
     P.sv = ctx->sv;
     P.phi = phi;
+    P.acc = acc;
     P.gcount = ctx->gcount.as<uint4>();
     P.n = n;
     P.ngroups = ngroups;
@@ -584,6 +591,10 @@ int launch_walk(bh_ctx* ctx, double theta, double G, double* phi, int group, int
             walk_pair_kernel<true, true><<<blocks_for(npairs, kWalkWarps), kWalkWarps * 32, smem, st>>>(P);
         else if (count_only)
             walk_pair_kernel<true><<<blocks_for(npairs, kWalkWarps), kWalkWarps * 32, smem, st>>>(P);
+        else if (acc && subset)
+            walk_pair_kernel<false, true, true><<<blocks_for(npairs, kWalkWarps), kWalkWarps * 32, smem, st>>>(P);
+        else if (acc)
+            walk_pair_kernel<false, false, true><<<blocks_for(npairs, kWalkWarps), kWalkWarps * 32, smem, st>>>(P);
         else if (subset)
             walk_pair_kernel<false, true><<<blocks_for(npairs, kWalkWarps), kWalkWarps * 32, smem, st>>>(P);
         else
@@ -609,7 +620,7 @@ int ensure_counts(bh_ctx* ctx)
 
 extern "C" {
 
-int bh_potential(bh_ctx* ctx, double theta, double G, double* phi)
+static int potential_impl(bh_ctx* ctx, double theta, double G, double* phi, double* acc)
 {
     if (!ctx || !phi || !(theta >= 0.0) || isnan(G)) return BH_ERR_INVALID_ARG;
     if (!ctx->built) return BH_ERR_NOT_BUILT;
@@ -619,7 +630,7 @@ int bh_potential(bh_ctx* ctx, double theta, double G, double* phi)
     ctx->launches_walk = 0;
     ctx->walked = false;
     BH_CUDA(cudaEventRecord(ctx->ev[EV_W0], st));
-    int rc = launch_walk(ctx, theta, G, phi, group, ctx->mac, false);
+    int rc = launch_walk(ctx, theta, G, phi, group, ctx->mac, false, acc);
     if (rc != BH_OK) return rc;
     ctx->launches_walk = ctx->n > 1 ? 1 : 0;
     BH_CUDA(cudaEventRecord(ctx->ev[EV_W1], st));
@@ -630,6 +641,17 @@ int bh_potential(bh_ctx* ctx, double theta, double G, double* phi)
     ctx->walk_mac = ctx->mac;
     ctx->counts_valid = group != 32 || ctx->n == 1;   // the per-target walk and n = 1 fill gcount themselves
     return BH_OK;
+}
+
+int bh_potential(bh_ctx* ctx, double theta, double G, double* phi)
+{
+    return potential_impl(ctx, theta, G, phi, nullptr);
+}
+
+int bh_field(bh_ctx* ctx, double theta, double G, double* phi, double* acc)
+{
+    if (!acc) return BH_ERR_INVALID_ARG;
+    return potential_impl(ctx, theta, G, phi, acc);
 }
 
 int bh_potential_direct(bh_ctx* ctx, double G, const int64_t* targets, int64_t nt, double* phi)

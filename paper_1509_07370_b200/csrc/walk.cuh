@@ -51,6 +51,7 @@ struct WalkParams {
     const u32* leaf_slot;     // [n] slot of sorted cell s (the targets are read from rec)
     SortedView sv;            // sorted cells: original index of sorted slot s
     double* phi;              // [n] original order
+    double* acc;              // bh_field only: [3n] (gx, gy, gz) per cell, original order
     uint4* gcount;            // [ngroups] {accepted, leaf, opened, exact-tested}
     i64 n;
     i64 ngroups;
@@ -160,6 +161,110 @@ __device__ __forceinline__ void eval_c(const float4* __restrict__ L, const u32* 
     accB += (double)s.y;
 }
 
+// ---- NEXT-4 (bh_field): the same lists, Phi with the same arithmetic, plus g = -grad Phi ----------
+// Every entry contributes the gradient of its monopole term: sum of w * (r_j - r_t), w = m/d^3 =
+// (m * rinv) * (rinv * rinv); three packed multiplies and three packed fmas more per entry pair.
+struct Grad2 { float2 x0, x1, y0, y1, z0, z1; };
+__device__ __forceinline__ Grad2 grad_zero()
+{
+    Grad2 g; g.x0 = g.x1 = g.y0 = g.y1 = g.z0 = g.z1 = splat2(0.f); return g;
+}
+__device__ __forceinline__ void grad_flush(const Grad2& g, double* acc3)
+{
+    acc3[0] += ((double)g.x0.x + (double)g.x0.y) + ((double)g.x1.x + (double)g.x1.y);
+    acc3[1] += ((double)g.y0.x + (double)g.y0.y) + ((double)g.y1.x + (double)g.y1.y);
+    acc3[2] += ((double)g.z0.x + (double)g.z0.y) + ((double)g.z1.x + (double)g.z1.y);
+}
+
+__device__ __forceinline__ void quad_body_g(const float4 x, const float4 y, const float4 z, const float4 m,
+                                            const Tgt2& t, float2& s0, float2& s1, Grad2& g)
+{
+    const float2 dx0 = __fadd2_rn(make_float2(x.x, x.y), t.x), dx1 = __fadd2_rn(make_float2(x.z, x.w), t.x);
+    const float2 dy0 = __fadd2_rn(make_float2(y.x, y.y), t.y), dy1 = __fadd2_rn(make_float2(y.z, y.w), t.y);
+    const float2 dz0 = __fadd2_rn(make_float2(z.x, z.y), t.z), dz1 = __fadd2_rn(make_float2(z.z, z.w), t.z);
+    float2 d0 = __ffma2_rn(dx0, dx0, splat2(kTinyD2));
+    float2 d1 = __ffma2_rn(dx1, dx1, splat2(kTinyD2));
+    d0 = __ffma2_rn(dy0, dy0, d0);
+    d1 = __ffma2_rn(dy1, dy1, d1);
+    d0 = __ffma2_rn(dz0, dz0, d0);
+    d1 = __ffma2_rn(dz1, dz1, d1);
+    const float2 r0 = make_float2(rsqrt_approx(d0.x), rsqrt_approx(d0.y));
+    const float2 r1 = make_float2(rsqrt_approx(d1.x), rsqrt_approx(d1.y));
+    const float2 m0 = make_float2(m.x, m.y), m1 = make_float2(m.z, m.w);
+    s0 = __ffma2_rn(m0, r0, s0);
+    s1 = __ffma2_rn(m1, r1, s1);
+    const float2 w0 = __fmul2_rn(__fmul2_rn(m0, r0), __fmul2_rn(r0, r0));
+    const float2 w1 = __fmul2_rn(__fmul2_rn(m1, r1), __fmul2_rn(r1, r1));
+    g.x0 = __ffma2_rn(dx0, w0, g.x0); g.x1 = __ffma2_rn(dx1, w1, g.x1);
+    g.y0 = __ffma2_rn(dy0, w0, g.y0); g.y1 = __ffma2_rn(dy1, w1, g.y1);
+    g.z0 = __ffma2_rn(dz0, w0, g.z0); g.z1 = __ffma2_rn(dz1, w1, g.z1);
+}
+
+template <int CAP>
+__device__ __forceinline__ double eval_soa_g(const float* __restrict__ L, int cnt, const Tgt2& t, double* acc3)
+{
+    const float4* X = reinterpret_cast<const float4*>(L);
+    const float4* Y = reinterpret_cast<const float4*>(L + CAP);
+    const float4* Z = reinterpret_cast<const float4*>(L + 2 * CAP);
+    const float4* M = reinterpret_cast<const float4*>(L + 3 * CAP);
+    float2 s0 = splat2(0.f), s1 = splat2(0.f);
+    Grad2 g = grad_zero();
+    const int nq = (cnt + 3) >> 2;
+    #pragma unroll 2
+    for (int q = 0; q < nq; ++q) quad_body_g(X[q], Y[q], Z[q], M[q], t, s0, s1, g);
+    grad_flush(g, acc3);
+    return ((double)s0.x + (double)s0.y) + ((double)s1.x + (double)s1.y);
+}
+
+template <int CAP>
+__device__ __forceinline__ void eval_soa2_g(const float* __restrict__ L, int cnt, const Tgt2& tA, const Tgt2& tB,
+                                            double& accA, double& accB, double* gA, double* gB)
+{
+    const float4* X = reinterpret_cast<const float4*>(L);
+    const float4* Y = reinterpret_cast<const float4*>(L + CAP);
+    const float4* Z = reinterpret_cast<const float4*>(L + 2 * CAP);
+    const float4* M = reinterpret_cast<const float4*>(L + 3 * CAP);
+    float2 a0 = splat2(0.f), a1 = splat2(0.f), b0 = splat2(0.f), b1 = splat2(0.f);
+    Grad2 ga = grad_zero(), gb = grad_zero();
+    const int nq = (cnt + 3) >> 2;
+    for (int q = 0; q < nq; ++q) {
+        const float4 x = X[q], y = Y[q], z = Z[q], m = M[q];
+        quad_body_g(x, y, z, m, tA, a0, a1, ga);
+        quad_body_g(x, y, z, m, tB, b0, b1, gb);
+    }
+    accA += ((double)a0.x + (double)a0.y) + ((double)a1.x + (double)a1.y);
+    accB += ((double)b0.x + (double)b0.y) + ((double)b1.x + (double)b1.y);
+    grad_flush(ga, gA);
+    grad_flush(gb, gB);
+}
+
+__device__ __forceinline__ void eval_c_g(const float4* __restrict__ L, const u32* __restrict__ Lm, int cnt,
+                                         const float2 npx, const float2 npy, const float2 npz, double& accA,
+                                         double& accB, double* gA, double* gB)
+{
+    float2 s = splat2(0.f), gx = splat2(0.f), gy = splat2(0.f), gz = splat2(0.f);
+    for (int e = 0; e < cnt; ++e) {
+        const float4 v = L[e];
+        const u32 mk = Lm[e];
+        const float2 dx = __fadd2_rn(splat2(v.x), npx);
+        const float2 dy = __fadd2_rn(splat2(v.y), npy);
+        const float2 dz = __fadd2_rn(splat2(v.z), npz);
+        float2 d2 = __fmul2_rn(dx, dx);
+        d2 = __ffma2_rn(dy, dy, d2);
+        d2 = __ffma2_rn(dz, dz, d2);
+        float2 r = make_float2(rsqrt_approx(d2.x), rsqrt_approx(d2.y));
+        r.x = (d2.x >= 1.17549435e-38f && (mk & 1u)) ? r.x : 0.f;
+        r.y = (d2.y >= 1.17549435e-38f && (mk & 2u)) ? r.y : 0.f;
+        s = __ffma2_rn(splat2(v.w), r, s);
+        const float2 w = __fmul2_rn(__fmul2_rn(splat2(v.w), r), __fmul2_rn(r, r));
+        gx = __ffma2_rn(dx, w, gx); gy = __ffma2_rn(dy, w, gy); gz = __ffma2_rn(dz, w, gz);
+    }
+    accA += (double)s.x;
+    accB += (double)s.y;
+    gA[0] += (double)gx.x; gA[1] += (double)gy.x; gA[2] += (double)gz.x;
+    gB[0] += (double)gx.y; gB[1] += (double)gy.y; gB[2] += (double)gz.y;
+}
+
 template <int CAP>
 __device__ __forceinline__ void soa_store(float* L, int e, float4 r)
 {
@@ -213,8 +318,9 @@ __device__ __forceinline__ void box_d2(const float4 q, const Box2& b, float2& d2
 //                needed the per-member test}; no lists, no arithmetic on masses, no Phi.
 // SUBSET = true: only cells with original index < P.ntargets are targets (bh_set_num_targets); the
 //                default instantiation carries none of that code.
-template <bool COUNT, bool SUBSET = false>
-__global__ void __launch_bounds__(kWalkWarps * 32, 3)
+// ACC = true   : bh_field -- additionally g = -grad Phi on the same lists (NEXT-4); its own register budget.
+template <bool COUNT, bool SUBSET = false, bool ACC = false>
+__global__ void __launch_bounds__(kWalkWarps * 32, ACC ? 2 : 3)
 walk_pair_kernel(const WalkParams P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -263,6 +369,7 @@ walk_pair_kernel(const WalkParams P)
     TB.x = splat2(-tB.x); TB.y = splat2(-tB.y); TB.z = splat2(-tB.z);
 
     double accA = 0.0, accB = 0.0;
+    double grA[3] = {0.0, 0.0, 0.0}, grB[3] = {0.0, 0.0, 0.0};   // ACC: sums of w (r_j - r_t)
     int nU2 = 0, nUA = 0, nUB = 0, nC = 0;          // list fill (warp-uniform)
     u32 cAccA = 0, cLeafA = 0, cOpenA = 0, cExA = 0;  // COUNT: per-lane partial counters
     u32 cAccB = 0, cLeafB = 0, cOpenB = 0, cExB = 0;
@@ -379,23 +486,25 @@ walk_pair_kernel(const WalkParams P)
             if (nU2 >= kU2Cap - kStepMax) {
                 soa_pad<kU2Cap>(U2, nU2);
                 __syncwarp();
-                eval_soa2<kU2Cap>(U2, nU2, TA, TB, accA, accB);
+                if (ACC) eval_soa2_g<kU2Cap>(U2, nU2, TA, TB, accA, accB, grA, grB);
+                else eval_soa2<kU2Cap>(U2, nU2, TA, TB, accA, accB);
                 nU2 = 0;
             }
             if (nUA >= kU1Cap - kStepMax) {
                 soa_pad<kU1Cap>(UA, nUA);
                 __syncwarp();
-                accA += eval_soa<kU1Cap>(UA, nUA, TA);
+                accA += ACC ? eval_soa_g<kU1Cap>(UA, nUA, TA, grA) : eval_soa<kU1Cap>(UA, nUA, TA);
                 nUA = 0;
             }
             if (nUB >= kU1Cap - kStepMax) {
                 soa_pad<kU1Cap>(UB, nUB);
                 __syncwarp();
-                accB += eval_soa<kU1Cap>(UB, nUB, TB);
+                accB += ACC ? eval_soa_g<kU1Cap>(UB, nUB, TB, grB) : eval_soa<kU1Cap>(UB, nUB, TB);
                 nUB = 0;
             }
             if (nC >= kCCap - kStepMax) {
-                eval_c(C, Cm, nC, npx, npy, npz, accA, accB);
+                if (ACC) eval_c_g(C, Cm, nC, npx, npy, npz, accA, accB, grA, grB);
+                else eval_c(C, Cm, nC, npx, npy, npz, accA, accB);
                 nC = 0;
             }
             __syncwarp();
@@ -415,22 +524,39 @@ walk_pair_kernel(const WalkParams P)
     if (nU2 > 0) {
         soa_pad<kU2Cap>(U2, nU2);
         __syncwarp();
-        eval_soa2<kU2Cap>(U2, nU2, TA, TB, accA, accB);
+        if (ACC) eval_soa2_g<kU2Cap>(U2, nU2, TA, TB, accA, accB, grA, grB);
+        else eval_soa2<kU2Cap>(U2, nU2, TA, TB, accA, accB);
     }
     if (nUA > 0) {
         soa_pad<kU1Cap>(UA, nUA);
         __syncwarp();
-        accA += eval_soa<kU1Cap>(UA, nUA, TA);
+        accA += ACC ? eval_soa_g<kU1Cap>(UA, nUA, TA, grA) : eval_soa<kU1Cap>(UA, nUA, TA);
     }
     if (nUB > 0) {
         soa_pad<kU1Cap>(UB, nUB);
         __syncwarp();
-        accB += eval_soa<kU1Cap>(UB, nUB, TB);
+        accB += ACC ? eval_soa_g<kU1Cap>(UB, nUB, TB, grB) : eval_soa<kU1Cap>(UB, nUB, TB);
     }
-    if (nC > 0) eval_c(C, Cm, nC, npx, npy, npz, accA, accB);
+    if (nC > 0) {
+        if (ACC) eval_c_g(C, Cm, nC, npx, npy, npz, accA, accB, grA, grB);
+        else eval_c(C, Cm, nC, npx, npy, npz, accA, accB);
+    }
     // ---- a7: Phi_t = -G * sum, written in the original cell order (W-rule 4) ----
-    if (liveA) { const u32 o = sv_idx(P.sv, sA); if (!SUBSET || o < P.ntargets) P.phi[o] = P.negG * accA; }
-    if (liveB) { const u32 o = sv_idx(P.sv, sB); if (!SUBSET || o < P.ntargets) P.phi[o] = P.negG * accB; }
+    // bh_field: g_t = -grad Phi_t = G * sum w (r_j - r_t)
+    if (liveA) {
+        const u32 o = sv_idx(P.sv, sA);
+        if (!SUBSET || o < P.ntargets) {
+            P.phi[o] = P.negG * accA;
+            if (ACC) { P.acc[3 * (size_t)o] = -P.negG * grA[0]; P.acc[3 * (size_t)o + 1] = -P.negG * grA[1]; P.acc[3 * (size_t)o + 2] = -P.negG * grA[2]; }
+        }
+    }
+    if (liveB) {
+        const u32 o = sv_idx(P.sv, sB);
+        if (!SUBSET || o < P.ntargets) {
+            P.phi[o] = P.negG * accB;
+            if (ACC) { P.acc[3 * (size_t)o] = -P.negG * grB[0]; P.acc[3 * (size_t)o + 1] = -P.negG * grB[1]; P.acc[3 * (size_t)o + 2] = -P.negG * grB[2]; }
+        }
+    }
 }
 
 // ---- BH_OPT_GROUP = 1 (W5): every target walks alone --------------------------------------------
@@ -452,6 +578,8 @@ walk_single_kernel(const WalkParams P)
     double acc = 0.0;
     float part = 0.f;
     int npart = 0;
+    double g[3] = {0.0, 0.0, 0.0};
+    float gp[3] = {0.f, 0.f, 0.f};
     u32 c_acc = 0, c_leaf = 0, c_open = 0;
     while (sp > 0) {
         const u32 slot = st_first[sp - 1];
@@ -477,12 +605,24 @@ walk_single_kernel(const WalkParams P)
             }
         }
         if (use) {
-            part = __fmaf_rn(r.w, rsqrt_approx(d2), part);
-            if (++npart == 32) { acc += (double)part; part = 0.f; npart = 0; }
+            const float ri = rsqrt_approx(d2);
+            part = __fmaf_rn(r.w, ri, part);
+            if (P.acc) {                                   // bh_field: w (r_j - r_t), w = m / d^3
+                const float wgt = __fmul_rn(__fmul_rn(r.w, ri), __fmul_rn(ri, ri));
+                gp[0] = __fmaf_rn(-dx, wgt, gp[0]); gp[1] = __fmaf_rn(-dy, wgt, gp[1]); gp[2] = __fmaf_rn(-dz, wgt, gp[2]);
+            }
+            if (++npart == 32) {
+                acc += (double)part; part = 0.f; npart = 0;
+                g[0] += (double)gp[0]; g[1] += (double)gp[1]; g[2] += (double)gp[2];
+                gp[0] = gp[1] = gp[2] = 0.f;
+            }
         }
     }
     acc += (double)part;
-    P.phi[sv_idx(P.sv, s)] = P.negG * acc;
+    const u32 o = sv_idx(P.sv, s);
+    P.phi[o] = P.negG * acc;
+    if (P.acc)
+        for (int k = 0; k < 3; ++k) P.acc[3 * (size_t)o + k] = -P.negG * (g[k] + (double)gp[k]);
     P.gcount[s] = make_uint4(c_acc, c_leaf, c_open, 0u);
 }
 
