@@ -260,6 +260,17 @@ def run_ours(args):
     t_ess = ra.elapsed_time(rb) / args.steps / 1e3
     ctx.set_mac(0)
 
+    # ---- NEXT-4: bh_field, Phi and g = -grad Phi from one walk (3 packed mul + 3 packed fma more per entry pair) ----
+    ctx.build(*d, w.cube)
+    ctx.field(w.theta, w.G)
+    torch.cuda.synchronize()
+    ra.record()
+    for _ in range(args.steps):
+        ctx.field(w.theta, w.G)
+    rb.record()
+    torch.cuda.synchronize()
+    t_field = ra.elapsed_time(rb) / args.steps / 1e3
+
     # ---- e2e: the public host-buffer call, copies inside the timed region ----
     e2e_steps = max(1, min(args.steps, 5))
     phi_host = torch.empty(n, dtype=torch.float64).pin_memory()
@@ -295,6 +306,9 @@ def run_ours(args):
         "walk_interactions_per_s": world * inter / t_walk,
         "interactions_per_target": inter / n,
         "ms_build": t_build * 1e3, "ms_walk": t_walk * 1e3, "ms_update_masses": t_refit * 1e3,
+        "field": {"ms_walk": t_field * 1e3, "interactions_per_s": world * st.interactions / t_field,
+                  "flops_per_interaction": 22, "frac_fp32": st.interactions * 22 / t_field / 1e12 / (
+                      st_sms(local) * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12)},
         "essential_nodes": {"box": "face-neighbour cube of the same size", "theta": w.theta, "mac": "eq4",
                             "entries": n_ess, "ms": t_ess * 1e3},
         "build_passes_ms": {"keys": st.ms_keys, "sort": st.ms_sort, "count": st.ms_count,
