@@ -209,26 +209,26 @@ int bh_create(bh_ctx** out, int device, void* cuda_stream)
         if (rc) break;
         if ((e = ctx->scalars.ensure(sizeof(DeviceScalars))) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaMalloc"); break; }
         if ((e = cudaMallocHost(&ctx->h_scalars, sizeof(DeviceScalars))) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaMallocHost"); break; }
-        if ((e = cudaFuncSetAttribute(radix_onesweep_kernel<kGeneric>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)sort_smem_bytes(false))) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(sort)"); break; }
-        if ((e = cudaFuncSetAttribute(radix_onesweep_kernel<kGenericFirst>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)sort_smem_bytes(false))) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(sort)"); break; }
-        if ((e = cudaFuncSetAttribute(radix_onesweep_kernel<kPacked>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)sort_smem_bytes(true))) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(sort)"); break; }
-        if ((e = cudaFuncSetAttribute(radix_onesweep_kernel<kPackedFirst>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)sort_smem_bytes(true))) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(sort)"); break; }
-        if ((e = cudaFuncSetAttribute(walk_pair_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      227 * 1024)) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(walk)"); break; }
-        if ((e = cudaFuncSetAttribute(walk_pair_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      227 * 1024)) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(walk count)"); break; }
-        if ((e = cudaFuncSetAttribute(walk_pair_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      227 * 1024)) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(walk subset)"); break; }
-        if ((e = cudaFuncSetAttribute(walk_pair_kernel<false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      227 * 1024)) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(walk field)"); break; }
-        if ((e = cudaFuncSetAttribute(walk_pair_kernel<false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      227 * 1024)) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(walk field subset)"); break; }
-        if ((e = cudaFuncSetAttribute(walk_pair_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      227 * 1024)) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaFuncSetAttribute(walk subset count)"); break; }
+        // kernels whose dynamic shared memory exceeds the 48 KB default
+        const int walk_smem = 227 * 1024;
+        const struct { const void* fn; int bytes; const char* what; } big_smem[] = {
+            {(const void*)radix_onesweep_kernel<kGenericFirst>, (int)sort_smem_bytes(false), "sort"},
+            {(const void*)radix_onesweep_kernel<kGeneric>, (int)sort_smem_bytes(false), "sort"},
+            {(const void*)radix_onesweep_kernel<kPackedFirst>, (int)sort_smem_bytes(true), "sort"},
+            {(const void*)radix_onesweep_kernel<kPacked>, (int)sort_smem_bytes(true), "sort"},
+            {(const void*)walk_pair_kernel<false>, walk_smem, "walk"},
+            {(const void*)walk_pair_kernel<true>, walk_smem, "walk count"},
+            {(const void*)walk_pair_kernel<false, true>, walk_smem, "walk subset"},
+            {(const void*)walk_pair_kernel<true, true>, walk_smem, "walk subset count"},
+            {(const void*)walk_pair_kernel<false, false, true>, walk_smem, "walk field"},
+            {(const void*)walk_pair_kernel<false, true, true>, walk_smem, "walk field subset"},
+        };
+        for (const auto& k : big_smem) {
+            if ((e = cudaFuncSetAttribute(k.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, k.bytes)) != cudaSuccess) {
+                rc = cuda_fail(ctx, e, k.what);
+                break;
+            }
+        }
     } while (0);
     if (rc != BH_OK) { bh_destroy(ctx); return rc; }
     *out = ctx;
@@ -298,100 +298,100 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
     unsigned tgrid = 0;
     int aux_cleared = 0;
     for (int attempt = 0;; ++attempt) {
-    const bool speculate = attempt == 0 && ctx->plan_hint_valid;
-    ctx->launches_build = 0;
-    BH_CUDA(cudaMemsetAsync(ds, 0, sizeof(DeviceScalars), st));
-    {   // key_and starts as all ones
-        const u64 ones = ~0ULL;
-        BH_CUDA(cudaMemcpyAsync(&ds->keyred.key_and, &ones, sizeof(u64), cudaMemcpyHostToDevice, st));
-    }
-
-    // ---- a1: Morton keys ----
-    const double s = 2097152.0 / cube[3];      // K1: s = 2^21 / L in fp64
-    {
-        const int grid = persistent_grid(ctx, 8);
-        if (aligned16(x) && aligned16(y) && aligned16(z))
-            morton_keys_kernel<2><<<grid, 256, 0, st>>>(x, y, z, n, cube[0], cube[1], cube[2], s,
-                                                        ctx->keysA.as<u64>(), &ds->keyred);
-        else
-            morton_keys_kernel<1><<<grid, 256, 0, st>>>(x, y, z, n, cube[0], cube[1], cube[2], s,
-                                                        ctx->keysA.as<u64>(), &ds->keyred);
-        BH_CUDA(cudaGetLastError());
-    }
-    ctx->launches_build += 1;
-    BH_CUDA(cudaEventRecord(ctx->ev[EV_KEYS], st));
-
-    // read-back 1: which key bits vary (decides the radix passes) and the clamp count
-    BH_CUDA(cudaMemcpyAsync(&ctx->h_scalars->keyred, &ds->keyred, sizeof(KeyReduce), cudaMemcpyDeviceToHost, st));
-    KeyReduce kr = ctx->plan_hint;
-    if (!speculate) {
-        BH_CUDA(cudaStreamSynchronize(st));
-        kr = ctx->h_scalars->keyred;
-    }
-    const SortPlan plan = make_sort_plan(kr.key_or ^ kr.key_and);
-    ctx->sort_passes = plan.npasses;
-
-    // ---- a2: radix sort of (key, index) ----
-    if (plan.npasses > 0 && !plan.packed) {      // the permutation is stored only when a key window of 32 bits is too narrow
-        BH_CUDA(ctx->idxA.ensure(sizeof(u32) * n));
-        BH_CUDA(ctx->idxB.ensure(sizeof(u32) * n));
-    }
-    BH_CUDA(radix_sort_pairs(ctx->keysA.as<u64>(), ctx->idxA.as<u32>(), ctx->keysB.as<u64>(), ctx->idxB.as<u32>(), n,
-                             plan, ctx->hist.as<u32>(), persistent_grid(ctx, 8), st));
-    ctx->launches_build += plan.npasses ? 1 + plan.npasses : 0;   // histogram + one kernel per pass
-    {
-        const bool odd = plan.npasses & 1;
-        const u64* kres = odd ? ctx->keysB.as<u64>() : ctx->keysA.as<u64>();
-        SortedView& sv = ctx->sv;
-        sv.packed = nullptr; sv.keys = nullptr; sv.idx = nullptr; sv.cbits = 0; sv.lo = 0;
-        if (plan.npasses == 0) sv.keys = kres;                      // identity: all keys equal
-        else if (plan.packed) {
-            sv.packed = kres;
-            sv.lo = plan.lo;
-            sv.cbits = kr.key_and & ~(0xffffffffULL << plan.lo);
-        } else {
-            sv.keys = kres;
-            sv.idx = odd ? ctx->idxB.as<u32>() : ctx->idxA.as<u32>();
+        const bool speculate = attempt == 0 && ctx->plan_hint_valid;
+        ctx->launches_build = 0;
+        BH_CUDA(cudaMemsetAsync(ds, 0, sizeof(DeviceScalars), st));
+        {   // key_and starts as all ones
+            const u64 ones = ~0ULL;
+            BH_CUDA(cudaMemcpyAsync(&ds->keyred.key_and, &ones, sizeof(u64), cudaMemcpyHostToDevice, st));
         }
-    }
-    BH_CUDA(cudaEventRecord(ctx->ev[EV_SORT], st));
 
-    // ---- a4: topology (a3, the permutation of the cell data, is fused into the assigning kernel) ----
-    ctx->nn = 0; ctx->nslots = 0; ctx->depth = 0; ctx->maxlevel = 0; ctx->max_bucket = 1;
-    memset(&ctx->lv, 0, sizeof(ctx->lv));
-    if (n >= 2) {
-        nchunks = topo_chunks(n);
-        tgrid = blocks_for(nchunks, kTopoThreads / 32);
-        u32* hist = ctx->hist.as<u32>();
-        topo_count_kernel<<<tgrid, kTopoThreads, 0, st>>>(ctx->sv, n, ctx->clev.as<signed char>(), hist, nchunks);
-        BH_CUDA(cudaGetLastError());
-        BH_CUDA(exclusive_scan_u32(hist, hist, (i64)kTopoDigits * nchunks, ctx->scan_scratch.as<u32>(),
-                                   &ds->scan_total, st));
-        topo_totals_kernel<<<1, 64, 0, st>>>(hist, nchunks, &ds->scan_total, ds->topo_rows);
-        BH_CUDA(cudaGetLastError());
-        // read-back 2: entities and nodes per level (sizes every node / slot array)
-        BH_CUDA(cudaMemcpyAsync(ctx->h_scalars->topo_rows, ds->topo_rows, sizeof(u32) * (kTopoDigits + 1),
-                                cudaMemcpyDeviceToHost, st));
-    }
-    BH_CUDA(cudaEventRecord(ctx->ev[EV_PERM], st));
-    // aux must be zero on every leaf slot; only the node slots of the previous build are not.  Clearing
-    // them runs on the device while the host waits for the read-back and prepares the next launches.
-    if (ctx->aux_dirty_nn > 0) {
-        aux_clear_kernel<<<blocks_for(ctx->aux_dirty_nn, 256), 256, 0, st>>>(ctx->node_slot.as<u32>(), ctx->aux_dirty_nn,
-                                                                            ctx->aux.as<WalkAux>());
-        BH_CUDA(cudaGetLastError());
-        ctx->aux_dirty_nn = 0;
-        aux_cleared = 1;
-    }
-    BH_CUDA(cudaEventSynchronize(ctx->ev[EV_PERM]));
-    {
-        const KeyReduce& real = ctx->h_scalars->keyred;
-        const bool hit = real.key_or == kr.key_or && real.key_and == kr.key_and;
-        ctx->plan_hint = real;
-        ctx->plan_hint_valid = true;
-        ctx->n_clamped = (i64)real.n_clamped;
-        if (hit) break;
-    }
+        // ---- a1: Morton keys ----
+        const double s = 2097152.0 / cube[3];      // K1: s = 2^21 / L in fp64
+        {
+            const int grid = persistent_grid(ctx, 8);
+            if (aligned16(x) && aligned16(y) && aligned16(z))
+                morton_keys_kernel<2><<<grid, 256, 0, st>>>(x, y, z, n, cube[0], cube[1], cube[2], s,
+                                                            ctx->keysA.as<u64>(), &ds->keyred);
+            else
+                morton_keys_kernel<1><<<grid, 256, 0, st>>>(x, y, z, n, cube[0], cube[1], cube[2], s,
+                                                            ctx->keysA.as<u64>(), &ds->keyred);
+            BH_CUDA(cudaGetLastError());
+        }
+        ctx->launches_build += 1;
+        BH_CUDA(cudaEventRecord(ctx->ev[EV_KEYS], st));
+
+        // read-back 1: which key bits vary (decides the radix passes) and the clamp count
+        BH_CUDA(cudaMemcpyAsync(&ctx->h_scalars->keyred, &ds->keyred, sizeof(KeyReduce), cudaMemcpyDeviceToHost, st));
+        KeyReduce kr = ctx->plan_hint;
+        if (!speculate) {
+            BH_CUDA(cudaStreamSynchronize(st));
+            kr = ctx->h_scalars->keyred;
+        }
+        const SortPlan plan = make_sort_plan(kr.key_or ^ kr.key_and);
+        ctx->sort_passes = plan.npasses;
+
+        // ---- a2: radix sort of (key, index) ----
+        if (plan.npasses > 0 && !plan.packed) {      // the permutation is stored only when a key window of 32 bits is too narrow
+            BH_CUDA(ctx->idxA.ensure(sizeof(u32) * n));
+            BH_CUDA(ctx->idxB.ensure(sizeof(u32) * n));
+        }
+        BH_CUDA(radix_sort_pairs(ctx->keysA.as<u64>(), ctx->idxA.as<u32>(), ctx->keysB.as<u64>(), ctx->idxB.as<u32>(), n,
+                                 plan, ctx->hist.as<u32>(), persistent_grid(ctx, 8), st));
+        ctx->launches_build += plan.npasses ? 1 + plan.npasses : 0;   // histogram + one kernel per pass
+        {
+            const bool odd = plan.npasses & 1;
+            const u64* kres = odd ? ctx->keysB.as<u64>() : ctx->keysA.as<u64>();
+            SortedView& sv = ctx->sv;
+            sv.packed = nullptr; sv.keys = nullptr; sv.idx = nullptr; sv.cbits = 0; sv.lo = 0;
+            if (plan.npasses == 0) sv.keys = kres;                      // identity: all keys equal
+            else if (plan.packed) {
+                sv.packed = kres;
+                sv.lo = plan.lo;
+                sv.cbits = kr.key_and & ~(0xffffffffULL << plan.lo);
+            } else {
+                sv.keys = kres;
+                sv.idx = odd ? ctx->idxB.as<u32>() : ctx->idxA.as<u32>();
+            }
+        }
+        BH_CUDA(cudaEventRecord(ctx->ev[EV_SORT], st));
+
+        // ---- a4: topology (a3, the permutation of the cell data, is fused into the assigning kernel) ----
+        ctx->nn = 0; ctx->nslots = 0; ctx->depth = 0; ctx->maxlevel = 0; ctx->max_bucket = 1;
+        memset(&ctx->lv, 0, sizeof(ctx->lv));
+        if (n >= 2) {
+            nchunks = topo_chunks(n);
+            tgrid = blocks_for(nchunks, kTopoThreads / 32);
+            u32* hist = ctx->hist.as<u32>();
+            topo_count_kernel<<<tgrid, kTopoThreads, 0, st>>>(ctx->sv, n, ctx->clev.as<signed char>(), hist, nchunks);
+            BH_CUDA(cudaGetLastError());
+            BH_CUDA(exclusive_scan_u32(hist, hist, (i64)kTopoDigits * nchunks, ctx->scan_scratch.as<u32>(),
+                                       &ds->scan_total, st));
+            topo_totals_kernel<<<1, 64, 0, st>>>(hist, nchunks, &ds->scan_total, ds->topo_rows);
+            BH_CUDA(cudaGetLastError());
+            // read-back 2: entities and nodes per level (sizes every node / slot array)
+            BH_CUDA(cudaMemcpyAsync(ctx->h_scalars->topo_rows, ds->topo_rows, sizeof(u32) * (kTopoDigits + 1),
+                                    cudaMemcpyDeviceToHost, st));
+        }
+        BH_CUDA(cudaEventRecord(ctx->ev[EV_PERM], st));
+        // aux must be zero on every leaf slot; only the node slots of the previous build are not.  Clearing
+        // them runs on the device while the host waits for the read-back and prepares the next launches.
+        if (ctx->aux_dirty_nn > 0) {
+            aux_clear_kernel<<<blocks_for(ctx->aux_dirty_nn, 256), 256, 0, st>>>(ctx->node_slot.as<u32>(), ctx->aux_dirty_nn,
+                                                                                ctx->aux.as<WalkAux>());
+            BH_CUDA(cudaGetLastError());
+            ctx->aux_dirty_nn = 0;
+            aux_cleared = 1;
+        }
+        BH_CUDA(cudaEventSynchronize(ctx->ev[EV_PERM]));
+        {
+            const KeyReduce& real = ctx->h_scalars->keyred;
+            const bool hit = real.key_or == kr.key_or && real.key_and == kr.key_and;
+            ctx->plan_hint = real;
+            ctx->plan_hint_valid = true;
+            ctx->n_clamped = (i64)real.n_clamped;
+            if (hit) break;
+        }
     }   // attempt
     if (n >= 2) {
         u32* hist = ctx->hist.as<u32>();
