@@ -164,16 +164,16 @@ __device__ __forceinline__ void eval_c(const float4* __restrict__ L, const u32* 
 // ---- NEXT-4 (bh_field): the same lists, Phi with the same arithmetic, plus g = -grad Phi ----------
 // Every entry contributes the gradient of its monopole term: sum of w * (r_j - r_t), w = m/d^3 =
 // (m * rinv) * (rinv * rinv); three packed multiplies and three packed fmas more per entry pair.
-struct Grad2 { float2 x0, x1, y0, y1, z0, z1; };
+struct Grad2 { float2 x, y, z; };
 __device__ __forceinline__ Grad2 grad_zero()
 {
-    Grad2 g; g.x0 = g.x1 = g.y0 = g.y1 = g.z0 = g.z1 = splat2(0.f); return g;
+    Grad2 g; g.x = g.y = g.z = splat2(0.f); return g;
 }
 __device__ __forceinline__ void grad_flush(const Grad2& g, double* acc3)
 {
-    acc3[0] += ((double)g.x0.x + (double)g.x0.y) + ((double)g.x1.x + (double)g.x1.y);
-    acc3[1] += ((double)g.y0.x + (double)g.y0.y) + ((double)g.y1.x + (double)g.y1.y);
-    acc3[2] += ((double)g.z0.x + (double)g.z0.y) + ((double)g.z1.x + (double)g.z1.y);
+    acc3[0] += (double)g.x.x + (double)g.x.y;
+    acc3[1] += (double)g.y.x + (double)g.y.y;
+    acc3[2] += (double)g.z.x + (double)g.z.y;
 }
 
 __device__ __forceinline__ void quad_body_g(const float4 x, const float4 y, const float4 z, const float4 m,
@@ -195,9 +195,9 @@ __device__ __forceinline__ void quad_body_g(const float4 x, const float4 y, cons
     s1 = __ffma2_rn(m1, r1, s1);
     const float2 w0 = __fmul2_rn(__fmul2_rn(m0, r0), __fmul2_rn(r0, r0));
     const float2 w1 = __fmul2_rn(__fmul2_rn(m1, r1), __fmul2_rn(r1, r1));
-    g.x0 = __ffma2_rn(dx0, w0, g.x0); g.x1 = __ffma2_rn(dx1, w1, g.x1);
-    g.y0 = __ffma2_rn(dy0, w0, g.y0); g.y1 = __ffma2_rn(dy1, w1, g.y1);
-    g.z0 = __ffma2_rn(dz0, w0, g.z0); g.z1 = __ffma2_rn(dz1, w1, g.z1);
+    g.x = __ffma2_rn(dx1, w1, __ffma2_rn(dx0, w0, g.x));
+    g.y = __ffma2_rn(dy1, w1, __ffma2_rn(dy0, w0, g.y));
+    g.z = __ffma2_rn(dz1, w1, __ffma2_rn(dz0, w0, g.z));
 }
 
 template <int CAP>
@@ -320,7 +320,7 @@ __device__ __forceinline__ void box_d2(const float4 q, const Box2& b, float2& d2
 //                default instantiation carries none of that code.
 // ACC = true   : bh_field -- additionally g = -grad Phi on the same lists (NEXT-4); its own register budget.
 template <bool COUNT, bool SUBSET = false, bool ACC = false>
-__global__ void __launch_bounds__(kWalkWarps * 32, ACC ? 2 : 3)
+__global__ void __launch_bounds__(kWalkWarps * 32, 3)
 walk_pair_kernel(const WalkParams P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
