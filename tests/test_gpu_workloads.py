@@ -68,6 +68,20 @@ def _check_sampled(ctx, ot, w, theta, mac=0, nruns=12, per=24, max_tol=1e-4, med
     return phi, cnt
 
 
+def _check_essential(ctx, ot, w, theta=0.5):
+    """NEXT-1 at full size: the essential set for a face-neighbour domain and for a distant one equals the
+    oracle's entry for entry (selection in fp64 on bit-identical moments)."""
+    x0, y0, z0, L = w.cube
+    for mac in (1, 0):
+        ctx.set_mac(mac)
+        for lo, hi in (((x0 + L, y0, z0), (x0 + 2 * L, y0 + L, z0 + L)),
+                       ((x0 - 9 * L, y0 + 3 * L, z0), (x0 - 8 * L, y0 + 4 * L, z0 + L))):
+            got = ctx.essential_nodes(lo, hi, theta).cpu().numpy()
+            ref = ot.essential_nodes(lo, hi, theta, mac=mac)
+            assert got.shape == ref.shape and np.array_equal(got, ref), (mac, lo, got.shape, ref.shape)
+    ctx.set_mac(0)
+
+
 def _check_tree(ctx, ot, w):
     t = {k: v.cpu().numpy() for k, v in ctx.export_tree().items()}
     ok, op = ot.sorted_keys_perm()
@@ -125,6 +139,7 @@ def test_config2_amr_core_and_config4_theta_sweep(bh, oracle):
     ctx = _build(bh, w)
     ot = oracle.OracleTree(w.x, w.y, w.z, w.m, w.cube)
     _check_tree(ctx, ot, w)
+    _check_essential(ctx, ot, w)
     rng = np.random.Generator(np.random.PCG64(4096))
     tg = np.sort(rng.choice(w.n, 4096, replace=False)).astype(np.int64)
     direct = ctx.potential_direct(w.G, targets=torch.from_numpy(tg).cuda()).cpu().numpy()
@@ -149,6 +164,7 @@ def test_config3_turb256_bench_configuration(bh, oracle):
     _check_tree(ctx, ot, w)
     st = ctx.get_stats()
     assert st.n_nodes == (w.n - 1) // 7 and st.depth == 7 and st.sort_passes == 3
+    _check_essential(ctx, ot, w)
     _check_sampled(ctx, ot, w, 0.5, nruns=16, per=16)
     _check_sampled(ctx, ot, w, 0.5, mac=1, nruns=4, per=8)
     # properties that hold at any size: every potential is finite and negative (all masses are positive)
