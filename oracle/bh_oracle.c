@@ -21,11 +21,19 @@
  *                 only if EVERY member accepts it (the all() vote).
  *                 Phi_i = -G sum m_j/|r_i - r_j| (Eq. 2, without the printed 1/2: reading).
  *   orc_direct    Eq. 2 written out: Phi_i = -G sum_{j != i} m_j/|r_i - r_j|.
+ *   orc_essential_nodes  Find Essential Nodes (§3.2.4): the tree pruned against a remote
+ *                 domain box with the minimum-distance form of the opening test (E1-E4).
+ *   orc_field / orc_direct_acc  the acceleration g = -grad Phi on the walk's own interaction lists and by
+ *                 direct summation (the Phi arithmetic of orc_potential is untouched).
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): keys vs closed form on 2^k grids and a per-bit
  * interleave; tree vs a recursive brute-force partition in numpy; node counts (n-1)/7 on grids;
  * moments vs flat sums; theta=0 walk == direct sum bit for bit in sorted order; convergence with
- * theta; uniform-sphere and MacLaurin closed forms.  No function here is "parity unpinned".
+ * theta; uniform-sphere and MacLaurin closed forms; essential nodes vs a brute-force partition on integer
+ * coordinates, the 1..n limits of PAPER.md:106, mass conservation and the potential inside the box
+ * (tests/test_oracle_essential.py); accelerations vs a numpy brute force, the numerical gradient of the
+ * direct-sum potential, Newton's third law and the two-body / uniform-sphere closed forms
+ * (tests/test_oracle_field.py).  No function here is "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>
