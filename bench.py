@@ -271,6 +271,29 @@ def run_ours(args):
     torch.cuda.synchronize()
     t_field = ra.elapsed_time(rb) / args.steps / 1e3
 
+    # ---- optional (--let-domains P): the locally-essential-tree solve of P x-slab domains, one after the other on
+    # this GPU (paper_1509_07370_b200/let.py, let_potential_serial): what a P-GPU run computes, without the exchange ----
+    let_info = None
+    if args.let_domains > 1 and world == 1:
+        from paper_1509_07370_b200 import let as let_mod
+        order = torch.argsort(d[0], stable=True)
+        parts = []
+        for c in torch.tensor_split(order, args.let_domains):
+            c = torch.sort(c).values
+            parts.append(tuple(t[c].contiguous() for t in d))
+        let_mod.let_potential_serial(parts, w.cube, w.theta, w.G, mac=1, ctx=ctx)          # warm-up (buffers)
+        torch.cuda.synchronize()
+        ra.record()
+        phis, sent = let_mod.let_potential_serial(parts, w.cube, w.theta, w.G, mac=1, ctx=ctx)
+        rb.record()
+        torch.cuda.synchronize()
+        recv = [sum(sent[dd][e] for dd in range(args.let_domains)) for e in range(args.let_domains)]
+        let_info = {"domains": args.let_domains, "split": "equal-count slabs along x", "mac": "eq4", "theta": w.theta,
+                    "ms_all_domains_serial": ra.elapsed_time(rb), "cells_per_domain": n // args.let_domains,
+                    "entries_received_mean": sum(recv) / len(recv), "entries_received_max": max(recv),
+                    "entries_sent_total": sum(map(sum, sent))}
+        ctx.set_mac(0)
+
     # ---- e2e: the public host-buffer call, copies inside the timed region ----
     e2e_steps = max(1, min(args.steps, 5))
     phi_host = torch.empty(n, dtype=torch.float64).pin_memory()
@@ -328,6 +351,8 @@ def run_ours(args):
                 "d2h_bytes_per_step": 8 * n, "steps": e2e_steps, "api": "bh_solve_host (pinned host buffers)"},
         "gpu_launches": launches_per_step * args.steps,
     }
+    if let_info is not None:
+        line["let_serial"] = let_info
     if not args.no_cpu_baseline and world == 1:
         import oracle as orc
         orc.build_library()
@@ -374,6 +399,8 @@ def main():
     ap.add_argument("--theta", type=float, default=0.5)
     ap.add_argument("--ref-groups", type=int, default=4096, help="groups the oracle walks per step (sample)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--let-domains", type=int, default=0,
+                    help="also run the locally-essential-tree solve of this many slab domains serially on the GPU")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
