@@ -147,6 +147,13 @@ int bh_essential_nodes(bh_ctx* ctx, const double box_lo[3], const double box_hi[
  * are skipped, and phi needs only ntargets entries. */
 int bh_set_num_targets(bh_ctx* ctx, int64_t ntargets);
 
+/* bh_measure_fma_peak: a MEASURED denominator for the walk's roofline (the walk is bound by the plain FP32
+ * pipe; SURVEY.md §8(d) asks for the nominal peak and a measured FMA-chain peak side by side).  Runs, on the
+ * context's stream, a kernel in which every thread advances 8 independent chains of fp32 FMAs from registers
+ * -- packed (FFMA2, what the walk's evaluation issues) and scalar -- and returns the best of three timed
+ * repetitions each, in TFLOP/s (2 flops per FMA).  Measurement aid, not part of the path; synchronises. */
+int bh_measure_fma_peak(bh_ctx* ctx, double* tflops_packed, double* tflops_scalar);
+
 /* bh_potential: Phi_i = -G sum_j m_j/|r_i - r_j| over the nodes and leaf cells the group walk of
  * PAPER.md:176-178 selects (DESIGN.md W-rules).
  *   theta : >= 0; theta = 0 opens every node (the result is then the direct sum in fp32 terms).

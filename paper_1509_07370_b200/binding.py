@@ -15,7 +15,7 @@ BH_DIRECT_ALL_MAX = 1 << 18
 EXPORTED_SYMBOLS = (
     "bh_create", "bh_destroy", "bh_strerror", "bh_last_cuda_error", "bh_set_option", "bh_build", "bh_potential",
     "bh_potential_direct", "bh_solve_host", "bh_tree_sizes", "bh_export_tree", "bh_last_group_counts",
-    "bh_last_interactions", "bh_get_stats", "bh_update_masses", "bh_essential_nodes", "bh_set_num_targets", "bh_field",
+    "bh_last_interactions", "bh_get_stats", "bh_update_masses", "bh_essential_nodes", "bh_set_num_targets", "bh_field", "bh_measure_fma_peak",
 )
 
 
@@ -64,6 +64,7 @@ def lib():
         L.bh_essential_nodes.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_double, dp, i64,
                                          C.POINTER(i64)]
         L.bh_set_num_targets.argtypes = [vp, i64]
+        L.bh_measure_fma_peak.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.bh_potential.argtypes = [vp, C.c_double, C.c_double, dp]
         L.bh_field.argtypes = [vp, C.c_double, C.c_double, dp, dp]
         L.bh_potential_direct.argtypes = [vp, C.c_double, dp, i64, dp]
@@ -169,6 +170,12 @@ class Context:
                 continue
             self._check(rc)
             return out[: cnt.value]
+
+    def measure_fma_peak(self):
+        """bh_measure_fma_peak: (packed FFMA2, scalar FFMA) register-resident FMA-chain rates in TFLOP/s."""
+        a, b = C.c_double(0.0), C.c_double(0.0)
+        self._check(self._L.bh_measure_fma_peak(self._h, C.byref(a), C.byref(b)))
+        return a.value, b.value
 
     def set_num_targets(self, ntargets: int):
         """bh_set_num_targets: cells with original index < ntargets are targets, the rest sources only (-1: all)."""

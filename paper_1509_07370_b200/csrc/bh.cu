@@ -12,6 +12,7 @@
 #include "direct.cuh"
 #include "keys.cuh"
 #include "let.cuh"
+#include "peak.cuh"
 #include "scan.cuh"
 #include "sort.cuh"
 #include "tree.cuh"
@@ -469,6 +470,37 @@ int bh_update_masses(bh_ctx* ctx, const double* m)
         { int rc = launch_moments(ctx); if (rc != BH_OK) return rc; }
     }
     BH_CUDA(cudaEventRecord(ctx->ev[EV_MOM], st));
+    return BH_OK;
+}
+
+int bh_measure_fma_peak(bh_ctx* ctx, double* tflops_packed, double* tflops_scalar)
+{
+    if (!ctx || !tflops_packed || !tflops_scalar) return BH_ERR_INVALID_ARG;
+    BH_CUDA(cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    const int grid = persistent_grid(ctx, 8), iters = 1 << 15;
+    BH_CUDA(ctx->gcount.ensure(sizeof(float) * (size_t)grid * 256));
+    float* out = ctx->gcount.as<float>();
+    ctx->counts_valid = false;                       // gcount doubles as the sink of the chains
+    cudaEvent_t e0 = ctx->ev[EV_W0], e1 = ctx->ev[EV_W1];
+    ctx->ev_walk = false;
+    const double flops = (double)grid * 256.0 * iters * kPeakChains * 2.0 * 2.0;   // 2 lanes x (mul + add)
+    double* res[2] = {tflops_packed, tflops_scalar};
+    for (int v = 0; v < 2; ++v) {
+        float best = 1e30f;
+        for (int rep = 0; rep < 4; ++rep) {          // first repetition warms up
+            BH_CUDA(cudaEventRecord(e0, st));
+            if (v == 0) fp32_fma_chain_kernel<true><<<grid, 256, 0, st>>>(out, iters, 0.999f, 1e-3f);
+            else fp32_fma_chain_kernel<false><<<grid, 256, 0, st>>>(out, iters, 0.999f, 1e-3f);
+            BH_CUDA(cudaGetLastError());
+            BH_CUDA(cudaEventRecord(e1, st));
+            BH_CUDA(cudaStreamSynchronize(st));
+            float ms = 0.f;
+            BH_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+            if (rep > 0 && ms < best) best = ms;
+        }
+        *res[v] = flops / (best * 1e-3) / 1e12;
+    }
     return BH_OK;
 }
 

@@ -282,3 +282,13 @@ def test_context_reuse_across_inputs(bh, oracle):
         ref, ocnt = ot.potential(w.theta, w.G, mac_fp32=True, want_counts=True)
         _phi_check(phi, ref)
         assert np.array_equal(ctx.last_group_counts().cpu().numpy(), ocnt), w.name
+
+
+def test_measured_fma_peak_is_near_nominal(bh):
+    """bh_measure_fma_peak (the measured denominator of the walk's roofline): register-resident FMA chains
+    reach most of SMs x 128 lanes x 2 x clock and never exceed it."""
+    ctx = bh.Context(0)
+    packed, scalar = ctx.measure_fma_peak()
+    props = torch.cuda.get_device_properties(0)
+    nominal = props.multi_processor_count * 128 * 2 * 1.965e9 / 1e12       # at the B200's maximum SM clock
+    assert 0.5 * nominal <= scalar <= 1.05 * nominal and 0.5 * nominal <= packed <= 1.05 * nominal, (packed, scalar)
