@@ -231,6 +231,8 @@ def run_ours(args):
     dev_total = ev[0][0].elapsed_time(ev[-1][2]) / 1e3          # device time first event -> last event
     t_build = sum(e[0].elapsed_time(e[1]) for e in ev) / args.steps / 1e3
     t_walk = sum(e[1].elapsed_time(e[2]) for e in ev) / args.steps / 1e3
+    per_step = sorted(e[0].elapsed_time(e[2]) for e in ev)                  # build + walk of each timed step, ms
+    step_median, step_best = per_step[len(per_step) // 2], per_step[0]
     dev_total, elapsed, t_build, t_walk = ranks.max_over_ranks([dev_total, elapsed, t_build, t_walk], dev)
     st = ctx.get_stats()
 
@@ -332,6 +334,7 @@ def run_ours(args):
         "walk_interactions_per_s": world * inter / t_walk,
         "interactions_per_target": inter / n,
         "ms_build": t_build * 1e3, "ms_walk": t_walk * 1e3, "ms_update_masses": t_refit * 1e3,
+        "ms_step_median": step_median, "ms_step_best": step_best,
         "field": {"ms_walk": t_field * 1e3, "interactions_per_s": world * st.interactions / t_field,
                   "flops_per_interaction": 22, "frac_fp32": st.interactions * 22 / t_field / 1e12 / (
                       st_sms(local) * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12)},
