@@ -531,16 +531,16 @@ int bh_essential_nodes(bh_ctx* ctx, const double box_lo[3], const double box_hi[
     }
     DeviceScalars* ds = ctx->scalars.as<DeviceScalars>();
     const i64 nslots = ctx->nslots;
+    const i64 nblk = (nslots + kEssTile - 1) / kEssTile;
     BH_CUDA(ctx->ess_state.ensure((size_t)nslots + 16));
-    BH_CUDA(ctx->ess_emit.ensure(sizeof(u32) * ((size_t)nslots + 4)));
-    BH_CUDA(ctx->scan_scratch.ensure(sizeof(u32) * (scan_scratch_elems(nslots) + 4)));
+    BH_CUDA(ctx->ess_emit.ensure(sizeof(u32) * ((size_t)nblk + 4)));                 // essential slots per block
+    BH_CUDA(ctx->scan_scratch.ensure(sizeof(u32) * (scan_scratch_elems(nblk) + 4)));
     BH_CUDA(cudaMemsetAsync(ctx->ess_state.p, 0, (size_t)nslots, st));
-    BH_CUDA(cudaMemsetAsync(ctx->ess_emit.p, 0, sizeof(u32) * (size_t)nslots, st));
     BH_CUDA(cudaMemsetAsync(ctx->ess_state.p, 1, 1, st));        // the root (slot 0) is tested like any node
     EssArgs A;
     A.nfirst = ctx->nfirst.as<u32>(); A.node_slot = ctx->node_slot.as<u32>(); A.rec64 = ctx->rec64.as<double4>();
     A.delta64 = ctx->delta64.as<double>(); A.aux = ctx->aux.as<WalkAux>();
-    A.state = ctx->ess_state.as<unsigned char>(); A.emit = ctx->ess_emit.as<u32>();
+    A.state = ctx->ess_state.as<unsigned char>();
     for (int a = 0; a < 3; ++a) { A.blo[a] = box_lo[a]; A.bhi[a] = box_hi[a]; }
     A.theta = theta; A.L = ctx->cube[3]; A.mac = ctx->mac;
     SmallLevels sl;
@@ -564,11 +564,12 @@ int bh_essential_nodes(bh_ctx* ctx, const double box_lo[3], const double box_hi[
             BH_CUDA(cudaGetLastError());
         }
     }
-    BH_CUDA(exclusive_scan_u32(ctx->ess_emit.as<u32>(), ctx->ess_emit.as<u32>(), nslots, ctx->scan_scratch.as<u32>(),
-                               &ds->scan_total, st));
+    u32* blk = ctx->ess_emit.as<u32>();
+    ess_count_kernel<<<(unsigned)nblk, kEssThreads, 0, st>>>(A.state, nslots, blk);
+    BH_CUDA(cudaGetLastError());
+    BH_CUDA(exclusive_scan_u32(blk, blk, nblk, ctx->scan_scratch.as<u32>(), &ds->scan_total, st));
     if (cap > 0) {
-        ess_gather_kernel<<<blocks_for(nslots, 256), 256, 0, st>>>(ctx->ess_emit.as<u32>(), nslots, &ds->scan_total,
-                                                                  ctx->rec64.as<double4>(), out, cap);
+        ess_gather_kernel<<<(unsigned)nblk, kEssThreads, 0, st>>>(A.state, nslots, blk, ctx->rec64.as<double4>(), out, cap);
         BH_CUDA(cudaGetLastError());
     }
     BH_CUDA(cudaMemcpyAsync(&ctx->h_scalars->scan_total, &ds->scan_total, sizeof(u32), cudaMemcpyDeviceToHost, st));

@@ -9,18 +9,18 @@
 // Like the paper's kernel it runs level by level from the root ("called once for each depth ...
 // Neither atomic operations nor direct synchronization calls are used"), one thread per node of the
 // level; unlike it, levels of <= 1024 nodes share one single-block launch, and the index list is not
-// copied to the host: the records are compacted on the device (flag -> scan -> gather) in ascending
+// copied to the host: the records are compacted on the device (count -> scan -> gather) in ascending
 // slot order = ascending (level, first sorted cell), ready to be handed to the exchange.
 #pragma once
 #include "common.cuh"
+#include "scan.cuh"
 #include "tree.cuh"
 
 namespace bh {
 
 struct EssArgs {
     const u32* nfirst; const u32* node_slot; const double4* rec64; const double* delta64; const WalkAux* aux;
-    unsigned char* state;     // per slot: 1 = reached internal node (to be tested at its level)
-    u32* emit;                // per slot: 1 = essential
+    unsigned char* state;     // per slot: 1 = reached internal node (to be tested at its level), 2 = essential
     double blo[3], bhi[3];
     double theta, L;
     int mac;
@@ -48,13 +48,12 @@ __device__ __forceinline__ void ess_node(i64 b, i64 b1, int level, u32 slot_end,
         const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
         accept = d2 > __dmul_rn(rc, rc);
     }
-    if (accept) { A.emit[slot] = 1u; return; }
+    if (accept) { A.state[slot] = 2; return; }
     const u32 first = A.nfirst[b];
     const u32 cnt = (b + 1 < b1 ? A.nfirst[b + 1] : slot_end) - first;
     for (u32 j = 0; j < cnt; ++j) {
         const u32 c = first + j;
-        if (A.aux[c].count > 0u) A.state[c] = 1;      // internal child: tested when its level runs
-        else A.emit[c] = 1u;                          // leaf cell
+        A.state[c] = A.aux[c].count > 0u ? 1 : 2;     // internal child: tested when its level runs; leaf cell: essential
     }
 }
 
@@ -78,20 +77,60 @@ ess_small_kernel(const SmallLevels sl, const EssArgs A)
     }
 }
 
-// out[4k..4k+3] = (x, y, z, m) of the k-th essential slot; pos = exclusive scan of emit
-__global__ void __launch_bounds__(256)
-ess_gather_kernel(const u32* __restrict__ pos, i64 nslots, const u32* __restrict__ total_p,
+// ---- compaction of the essential slots, in slot order -------------------------------------------------
+// A block owns kEssTile consecutive slots, a thread 16 of them (one 16-byte load of state bytes).
+// ess_count_kernel: essential slots per block; (device scan of the block counts); ess_gather_kernel:
+// out[4k..4k+3] = (x, y, z, m) of the k-th essential slot.  19 MB of flags are read twice at 16.8 M cells.
+constexpr int kEssThreads = 256;
+constexpr int kEssTile = kEssThreads * 16;
+
+__device__ __forceinline__ uint4 ess_load_flags(const unsigned char* state, i64 s0, i64 nslots)
+{
+    if (s0 + 16 <= nslots) return *reinterpret_cast<const uint4*>(state + s0);
+    unsigned char b[16];
+    #pragma unroll
+    for (int i = 0; i < 16; ++i) b[i] = s0 + i < nslots ? state[s0 + i] : 0;
+    uint4 v;
+    memcpy(&v, b, 16);
+    return v;
+}
+__device__ __forceinline__ u32 ess_twos(u32 w) { return (w >> 1) & 0x01010101u; }   // bytes are 0, 1 or 2
+
+__global__ void __launch_bounds__(kEssThreads)
+ess_count_kernel(const unsigned char* __restrict__ state, i64 nslots, u32* __restrict__ block_count)
+{
+    __shared__ u32 s_warp[9];
+    const i64 s0 = ((i64)blockIdx.x * kEssThreads + threadIdx.x) * 16;
+    const uint4 v = ess_load_flags(state, s0, nslots);
+    const u32 c = __popc(ess_twos(v.x)) + __popc(ess_twos(v.y)) + __popc(ess_twos(v.z)) + __popc(ess_twos(v.w));
+    u32 total;
+    block_excl_scan_256(c, total, s_warp);
+    if (threadIdx.x == 0) block_count[blockIdx.x] = total;
+}
+
+__global__ void __launch_bounds__(kEssThreads)
+ess_gather_kernel(const unsigned char* __restrict__ state, i64 nslots, const u32* __restrict__ block_base,
                   const double4* __restrict__ rec64, double* __restrict__ out, i64 cap)
 {
-    const i64 s = (i64)blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= nslots) return;
-    const u32 p = pos[s];
-    const u32 nxt = s + 1 < nslots ? pos[s + 1] : *total_p;
-    if (nxt != p && (i64)p < cap) {
-        const double2* q = reinterpret_cast<const double2*>(rec64 + s);
-        double2* o = reinterpret_cast<double2*>(out + 4 * (i64)p);
-        o[0] = q[0];
-        o[1] = q[1];
+    __shared__ u32 s_warp[9];
+    const i64 s0 = ((i64)blockIdx.x * kEssThreads + threadIdx.x) * 16;
+    const uint4 v = ess_load_flags(state, s0, nslots);
+    const u32 w[4] = {ess_twos(v.x), ess_twos(v.y), ess_twos(v.z), ess_twos(v.w)};
+    const u32 c = __popc(w[0]) + __popc(w[1]) + __popc(w[2]) + __popc(w[3]);
+    u32 total;
+    i64 p = (i64)block_base[blockIdx.x] + block_excl_scan_256(c, total, s_warp);
+    if (c == 0u) return;
+    #pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        if ((w[i >> 2] >> (8 * (i & 3))) & 1u) {
+            if (p < cap) {
+                const double2* q = reinterpret_cast<const double2*>(rec64 + s0 + i);
+                double2* o = reinterpret_cast<double2*>(out + 4 * p);
+                o[0] = q[0];
+                o[1] = q[1];
+            }
+            ++p;
+        }
     }
 }
 
