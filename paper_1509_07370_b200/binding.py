@@ -155,12 +155,16 @@ class Context:
 
     def essential_nodes(self, box_lo, box_hi, theta: float, cap: int = 0):
         """bh_essential_nodes: the last build's tree pruned against the remote box; returns a CUDA tensor
-        [count, 4] = (x, y, z, m) per essential entry.  `cap`: first guess of the count (0: query first)."""
+        [count, 4] = (x, y, z, m) per essential entry.  `cap`: first guess of the count (0: a guess from this
+        context's previous selections, so that a repeated exchange does not run the selection twice)."""
         torch = self._torch
         lo = (C.c_double * 3)(*[float(v) for v in box_lo])
         hi = (C.c_double * 3)(*[float(v) for v in box_hi])
         cnt = C.c_int64(0)
         TOO_LARGE = -5
+        if cap <= 0:
+            n = getattr(self, "n", 0)
+            cap = getattr(self, "_ess_cap", 0) or min(n, max(4096, n // 8))
         while True:
             out = torch.empty((max(cap, 1), 4), dtype=torch.float64, device=f"cuda:{self.device}")
             rc = self._L.bh_essential_nodes(self._h, lo, hi, float(theta), self._dev(out, torch.float64) if cap else None,
@@ -169,7 +173,9 @@ class Context:
                 cap = int(cnt.value)
                 continue
             self._check(rc)
-            return out[: cnt.value]
+            self._ess_cap = max(getattr(self, "_ess_cap", 0), int(cnt.value * 1.25) + 64)
+            res = out[: cnt.value]
+            return res.clone() if cap > cnt.value + (cnt.value >> 2) + 4096 else res     # do not pin a much larger buffer
 
     def measure_fma_peak(self):
         """bh_measure_fma_peak: (packed FFMA2, scalar FFMA) register-resident FMA-chain rates in TFLOP/s."""
