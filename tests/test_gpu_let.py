@@ -34,7 +34,8 @@ BOXES = [((1.5, 0.2, 0.2), (2.0, 0.8, 0.8)), ((0.6, 0.6, 0.6), (0.9, 0.9, 0.9)),
 CASES = [wl.uniform_sphere(16), wl.random_points(4099, seed=2), wl.clustered_points(3000, seed=3),
          wl.with_duplicates(wl.random_points(500, seed=4), 40, seed=4),
          wl.with_duplicates(wl.random_points(500, seed=5), 40, seed=5, near=2e-3),
-         wl.amr_collapsing_core(nroot=2, max_level=3)]
+         wl.amr_collapsing_core(nroot=2, max_level=3),
+         wl.random_points(2, seed=5), wl.random_points(3, seed=6), wl.random_points(17, seed=7)]   # fewer slots than a tile
 
 
 @pytest.mark.parametrize("mac", [0, 1], ids=["eq3", "eq4"])
