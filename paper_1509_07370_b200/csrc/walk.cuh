@@ -36,7 +36,7 @@
 
 namespace bh {
 
-constexpr int kWalkWarps = 8;                 // warps (= group pairs) per CTA
+constexpr int kWalkWarps = 4;                 // warps (= group pairs) per CTA
 constexpr int kU2Cap = 128;                   // entries of the both-groups list (float4 each)
 constexpr int kU1Cap = 64;                    // entries of each one-group list (SoA x,y,z,m)
 constexpr int kCCap = 64;                     // entries of the checked list (float4 + group mask)
@@ -320,7 +320,7 @@ __device__ __forceinline__ void box_d2(const float4 q, const Box2& b, float2& d2
 //                default instantiation carries none of that code.
 // ACC = true   : bh_field -- additionally g = -grad Phi on the same lists (NEXT-4); its own register budget.
 template <bool COUNT, bool SUBSET = false, bool ACC = false>
-__global__ void __launch_bounds__(kWalkWarps * 32, 3)
+__global__ void __launch_bounds__(kWalkWarps * 32, 24 / kWalkWarps)
 walk_pair_kernel(const WalkParams P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
