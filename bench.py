@@ -96,20 +96,45 @@ class ClockSampler:
 
 
 def build_bytes_per_cell(n, n_nodes, sort_passes):
-    """Algorithmic HBM bytes of bh_build per cell."""
+    """ALGORITHMIC HBM bytes of bh_build per cell, exactly SURVEY.md §8(d)'s table: a1 keys 36; a2 sort 8 (one
+    histogram read) + 24 per executed 8-bit pass; a3 permute 84; a4 topology 8 + 24 n_nodes/n; a5 moments
+    32 + 72 n_nodes/n.  What the implementation moves beyond that (its leaf_slot and c(s) arrays) is reported
+    separately as IMPL_EXTRA_BYTES_PER_CELL and is not part of the roofline numerator."""
     keys = 36.0
-    sort = (8.0 + 24.0 * sort_passes) if sort_passes else 0.0   # one histogram read + read/write of 12 B per pass
-    permute = 84.0 + 4.0
-    topo = 8.0 + 5.0 + (n_nodes / n) * 24.0
+    sort = (8.0 + 24.0 * sort_passes) if sort_passes else 0.0
+    permute = 84.0
+    topo = 8.0 + (n_nodes / n) * 24.0
     mom = 32.0 + (n_nodes / n) * 72.0
     return keys + sort + permute + topo + mom
 
 
-def oracle_step(w, orc, n_sample_groups, phi_buf):
-    """One pass of the oracle as it stands: full build, then the group walk on `n_sample_groups`
-    groups taken as 16 evenly spaced contiguous runs; walk time is extrapolated linearly to all
-    groups (groups are independent).  Returns (t_build, t_walk_extrapolated, interactions_sampled,
-    targets_sampled)."""
+IMPL_EXTRA_BYTES_PER_CELL = 9.0     # leaf_slot: 4 B written; c(s): 1 B written + 1 B read; leaf_slot read by the refit: not per build
+
+
+def make_config(w, world):
+    """The `config` object, identical for both arms (--impl ours / reference) so that the driver can match them."""
+    return {"workload": w.name, "n_cells": w.n, "theta": w.theta, "group": 32, "mac": "eq3", "G": w.G,
+            "l2": "inputs_exceed_l2 (4 x %.0f MB fp64 arrays re-read every step)" % (w.n * 8 / 1e6),
+            "parallelism": "replicas x%d" % world}
+
+
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for ln in f:
+                if ln.lower().startswith("model name"):
+                    return ln.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def oracle_step(w, orc, n_sample_groups, phi_buf, sample=None):
+    """One pass of the oracle as it stands (fp64, the criterion evaluated in fp64 as the paper writes it): full
+    build, then the group walk on `n_sample_groups` groups taken as 16 evenly spaced contiguous runs; walk time
+    is extrapolated linearly to all groups (groups are independent).  Returns (t_build, t_walk_extrapolated,
+    interactions_sampled, targets_sampled, groups walked).  `sample` (a dict) receives what the parity key needs:
+    the runs, the per-group counters and the sorted permutation; phi_buf holds Phi of the walked targets."""
     import numpy as np
     t0 = time.perf_counter()
     ot = orc.OracleTree(w.x, w.y, w.z, w.m, w.cube)
@@ -121,6 +146,7 @@ def oracle_step(w, orc, n_sample_groups, phi_buf):
     inter = 0
     targets = 0
     t_walk = 0.0
+    spans, counts = [], []
     for r in range(runs):
         g0 = min((ng // runs) * r + (ng // runs - per) // 2, ng - per)
         t1 = time.perf_counter()
@@ -129,9 +155,43 @@ def oracle_step(w, orc, n_sample_groups, phi_buf):
         members = np.minimum(32, w.n - 32 * np.arange(g0, g0 + per))
         inter += int(((cnt[:, 0] + cnt[:, 1]) * members).sum())
         targets += int(members.sum())
+        spans.append((g0, g0 + per))
+        counts.append(cnt)
     walked = runs * per
+    if sample is not None:
+        sample["runs"], sample["counts"] = spans, counts
+        sample["perm"] = ot.sorted_keys_perm()[1].astype(np.int64)
     del ot
     return t_build, t_walk * (ng / walked), inter, targets, walked
+
+
+def parity_key(w, phi_gpu, cnt_gpu, ev_gpu, phi_orc, sample):
+    """The GPU's Phi of the timed configuration against the oracle's on the groups the cpu_baseline leg walked
+    (tests/parity.py's primary comparison): groups whose (accepted, leaf, opened) differ from the fp64-decision
+    oracle's are flips (fp32-vs-fp64 opening decisions), counted; relative errors over the targets of the
+    other groups, and separately over the flipped ones."""
+    import numpy as np
+    keep, flp = [], []
+    flips = ng = 0
+    own = True
+    for (g0, g1), c64 in zip(sample["runs"], sample["counts"]):
+        flipped = np.any(cnt_gpu[g0:g1] != c64, axis=1)
+        own = own and bool(np.array_equal(ev_gpu[g0:g1], cnt_gpu[g0:g1, 0] + cnt_gpu[g0:g1, 1]))
+        flips += int(flipped.sum())
+        ng += g1 - g0
+        for g in range(g0, g1):
+            tg = sample["perm"][32 * g:min(32 * (g + 1), w.n)]
+            ref = phi_orc[tg]
+            rel = np.abs(phi_gpu[tg] - ref) / np.abs(ref)
+            (flp if flipped[g - g0] else keep).append(rel)
+    keep = np.concatenate(keep) if keep else np.zeros(1)
+    out = {"groups": ng, "targets": int(keep.size + sum(a.size for a in flp)), "max_rel": float(keep.max()),
+           "median_rel": float(np.median(keep)), "flips_fp32_vs_fp64": flips,
+           "max_rel_flipped_groups": float(np.concatenate(flp).max()) if flp else None,
+           "kernel_entry_counts_equal_counters": own,
+           "oracle": "fp64 decisions (Eq. 3 as written); tolerance 1e-4 max / 1e-6 median on non-flipped groups",
+           "pass": bool(keep.max() <= 1e-4 and np.median(keep) <= 1e-6 and own)}
+    return out
 
 
 def run_reference(args):
@@ -162,9 +222,10 @@ def run_reference(args):
         "impl": "reference", "metric": "cells_per_s_build_plus_walk", "value": value, "unit": "cells/s",
         "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": (tb + tw) * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": w.name, "n_cells": w.n, "theta": w.theta, "group": 32, "mac": "eq3"},
+        "config": make_config(w, max(args.gpus, 1)), "timing": "host wall clock, single thread",
         "walk_interactions_per_s": (inter / tg) * w.n / tw,
-        "cpu_baseline": {"value": value, "unit": "cells/s", "cores": 1, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": "cells/s", "cores": 1, "kind": "oracle", "sample": sample,
+                         "host_cpus": os.cpu_count(), "host_cpu_model": cpu_model()},
         "e2e": {"value": value, "unit": "cells/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -235,9 +296,48 @@ def run_ours(args):
     step_median, step_best = per_step[len(per_step) // 2], per_step[0]
     dev_total, elapsed, t_build, t_walk = ranks.max_over_ranks([dev_total, elapsed, t_build, t_walk], dev)
     st = ctx.get_stats()
+    phi_timed = phi.cpu().numpy() if rank == 0 else None             # the result of the timed configuration (parity key)
+    cnt_timed = ctx.last_group_counts().cpu().numpy() if rank == 0 else None
+    ev_timed = ctx.last_group_evaluated().cpu().numpy().astype("int64") if rank == 0 else None
 
-    # ---- measured FP32 denominator: register-resident FMA chains, packed (FFMA2) and scalar ----
-    fma_packed_tflops, fma_scalar_tflops = ctx.measure_fma_peak()
+    # ---- measured FP32 denominator: register-resident FMA chains, packed (FFMA2) and scalar (own small library) ----
+    from paper_1509_07370_b200 import fma_peak
+    fma_packed_tflops, fma_scalar_tflops = fma_peak.measure(local)
+
+    # ---- per-pass table of the build (BH_OPT_PASS_TIMING: one event per kernel; medians over 5 builds) ----
+    ctx.set_option(bh.binding.BH_OPT_PASS_TIMING, 1)
+    runs_p = []
+    for _ in range(5):
+        ctx.build(d[0], d[1], d[2], d[3], w.cube)
+        runs_p.append(ctx.build_passes())
+    ctx.set_option(bh.binding.BH_OPT_PASS_TIMING, 0)
+    passes = []
+    for k, (name, _, nbytes) in enumerate(runs_p[0]):
+        ms = statistics.median(r[k][1] for r in runs_p)
+        passes.append({"pass": name, "ms": round(ms, 5), "alg_bytes": nbytes,
+                       "frac": (nbytes / (ms * 1e-3) / 1e9 / hbm_gbs) if (nbytes > 0 and ms > 0) else None})
+
+    # ---- cold and plan-miss builds (the timed steps always hit the sort plan speculated from the previous build) ----
+    def timed_build(c, arrs):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        t_0 = time.perf_counter()
+        a.record()
+        c.build(*arrs, w.cube)
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b), (time.perf_counter() - t_0) * 1e3
+    other = wl.uniform_sphere(64)                      # a different mesh: other key bits vary, the speculated plan misses
+    od = [torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in (other.x, other.y, other.z, other.m)]
+    miss = []
+    for _ in range(3):
+        ctx.build(*od, other.cube)
+        miss.append(timed_build(ctx, d))
+    ms_build_miss = statistics.median(m_[0] for m_ in miss)
+    cold_ctx = bh.Context(local)                       # fresh context: every buffer allocated, no plan to speculate on
+    ms_build_cold, ms_build_cold_wall = timed_build(cold_ctx, d)
+    ms_build_second = timed_build(cold_ctx, d)[0]
+    cold_ctx.close()
 
     # ---- mass-only refit (bh_update_masses): same cells, new masses; keys / sort / topology reused ----
     ra, rb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -313,6 +413,16 @@ def run_ours(args):
     torch.cuda.synchronize()
     e2e_t = time.perf_counter() - t1
     e2e_t = ranks.max_over_ranks([e2e_t], dev)[0]
+    e2e_split = ctx.host_breakdown()
+    # the same call with pageable (ordinary numpy) buffers: staged through pinned chunks inside the library
+    px = [np.array(a) for a in (w.x, w.y, w.z, w.m)]
+    pphi = np.empty(n)
+    ctx.solve_host(*px, w.cube, w.theta, w.G, out=pphi)
+    torch.cuda.synchronize()
+    t1 = time.perf_counter()
+    ctx.solve_host(*px, w.cube, w.theta, w.G, out=pphi)
+    torch.cuda.synchronize()
+    e2e_pageable_t = time.perf_counter() - t1
 
     if rank != 0:
         if dist:
@@ -327,14 +437,18 @@ def run_ours(args):
         "metric": "cells_per_s_build_plus_walk", "value": ranks.whole_job_rate(n, args.steps, dev_total, world), "unit": "cells/s",
         "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": dev_total / args.steps * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": w.name, "n_cells": n, "theta": w.theta, "group": 32, "mac": "eq3", "G": w.G,
-                   "l2": "inputs_exceed_l2 (4 x %.0f MB fp64 arrays re-read every step)" % (n * 8 / 1e6),
-                   "parallelism": "replicas x%d" % world, "timing": "cuda events, max over ranks",
-                   "wall_ms_per_step": elapsed / args.steps * 1e3},
+        "config": make_config(w, world), "timing": "cuda events, max over ranks",
+        "wall_ms_per_step": elapsed / args.steps * 1e3,
         "walk_interactions_per_s": world * inter / t_walk,
         "interactions_per_target": inter / n,
         "ms_build": t_build * 1e3, "ms_walk": t_walk * 1e3, "ms_update_masses": t_refit * 1e3,
         "ms_step_median": step_median, "ms_step_best": step_best,
+        "ms_build_cold": ms_build_cold, "ms_build_cold_wall": ms_build_cold_wall, "ms_build_second": ms_build_second,
+        "ms_build_miss": ms_build_miss,
+        "build_notes": "ms_build: the timed steps (same mesh every step: the sort plan speculated from the previous build "
+                       "hits, one host round trip); ms_build_miss: previous build on another mesh (plan miss: keys, sort and "
+                       "count run twice, two round trips); ms_build_cold: first build of a fresh context (allocations inside)",
+        "build_passes": passes,
         "field": {"ms_walk": t_field * 1e3, "interactions_per_s": world * st.interactions / t_field,
                   "flops_per_interaction": 22, "frac_fp32": st.interactions * 22 / t_field / 1e12 / (
                       st_sms(local) * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12)},
@@ -354,10 +468,19 @@ def run_ours(args):
                                     "13 flops/interaction" % (st_sms(local), sm_max_mhz, peak_src),
                      "build_hbm": {"achieved": bpc * n / t_build / 1e9, "peak": hbm_gbs, "unit": "GB/s",
                                    "frac": bpc * n / t_build / 1e9 / hbm_gbs, "bytes_per_cell": bpc,
+                                   "bytes_per_cell_source": "SURVEY.md 8(d): 36 + 8 + 24 x %d passes + 84 + (8 + 24 nn/n) + (32 + 72 nn/n)" % st.sort_passes,
+                                   "impl_extra_bytes_per_cell": IMPL_EXTRA_BYTES_PER_CELL,
+                                   "frac_incl_impl_extra": (bpc + IMPL_EXTRA_BYTES_PER_CELL) * n / t_build / 1e9 / hbm_gbs,
+                                   "dram_bytes_measured": build_traffic(w.name),
+                                   "frac_of_measured_dram_bytes": (build_traffic(w.name) / t_build / 1e9 / hbm_gbs)
+                                   if build_traffic(w.name) else None,
                                    "peak_source": peak_src}},
         "clocks": clocks,
         "e2e": {"value": ranks.whole_job_rate(n, e2e_steps, e2e_t, world), "unit": "cells/s", "h2d_bytes_per_step": 4 * 8 * n,
-                "d2h_bytes_per_step": 8 * n, "steps": e2e_steps, "api": "bh_solve_host (pinned host buffers)"},
+                "d2h_bytes_per_step": 8 * n, "steps": e2e_steps, "api": "bh_solve_host (pinned host buffers)",
+                "ms_per_step": e2e_t / e2e_steps * 1e3, "split_last_call": e2e_split,
+                "pageable_buffers": {"value": n / e2e_pageable_t, "ms_per_step": e2e_pageable_t * 1e3,
+                                     "note": "ordinary numpy arrays, staged through two pinned 16 MB chunks inside bh_solve_host"}},
         "gpu_launches": launches_per_step * args.steps,
     }
     if let_info is not None:
@@ -366,17 +489,34 @@ def run_ours(args):
         import oracle as orc
         orc.build_library()
         phi_buf = np.full(n, np.nan)
-        tb, tw, oi, otg, walked = oracle_step(w, orc, args.ref_groups, phi_buf)
+        sample = {}
+        tb, tw, oi, otg, walked = oracle_step(w, orc, args.ref_groups, phi_buf, sample)
         ng = (n + 31) // 32
         line["cpu_baseline"] = {
             "value": n / (tb + tw), "unit": "cells/s", "cores": 1, "kind": "oracle",
             "sample": f"full fp64 build ({tb:.1f} s) + group walk of {walked} of {ng} groups "
                       f"(16 evenly spaced runs), walk time scaled by {ng / walked:.1f} to {tw:.1f} s",
-            "walk_interactions_per_s": (oi / otg) * n / tw, "host_cpus": os.cpu_count()}
+            "walk_interactions_per_s": (oi / otg) * n / tw, "host_cpus": os.cpu_count(), "host_cpu_model": cpu_model()}
+        # the groups the oracle just walked, against the Phi of the timed steps
+        line["parity"] = parity_key(w, phi_timed, cnt_timed, ev_timed, phi_buf, sample)
     print(json.dumps(line))
     if dist:
         dist.destroy_process_group()
     return 0
+
+
+def build_traffic(workload):
+    """Sum over the build kernels of dram__bytes_read.sum + dram__bytes_write.sum per build, from the committed ncu
+    capture (profiles/build_traffic.csv), if one was taken on this workload; else None."""
+    import csv
+    try:
+        with open(os.path.join(ROOT, "profiles", "build_traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == workload:
+                    return float(row["dram_bytes_per_build"])
+    except Exception:
+        pass
+    return None
 
 
 def walk_traffic(workload, theta):

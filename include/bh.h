@@ -40,7 +40,9 @@ typedef struct bh_ctx bh_ctx;
 #define BH_ERR_NOT_BUILT   -2   /* bh_potential / export / direct before a successful bh_build */
 #define BH_ERR_CUDA        -3   /* a CUDA runtime call failed; see bh_last_cuda_error() */
 #define BH_ERR_OOM         -4   /* device or host allocation failed */
-#define BH_ERR_TOO_LARGE   -5   /* bh_potential_direct over all n with n above BH_DIRECT_ALL_MAX; n + nodes >= 2^32; n >= 2^30 */
+#define BH_ERR_TOO_LARGE   -5   /* bh_build with 2^30 <= n < 2^31 or n + n_nodes >= 2^32 (32-bit slots; checked in 64 bits
+                                   before any node or slot array is sized); bh_potential_direct over all n with n above
+                                   BH_DIRECT_ALL_MAX; an output buffer smaller than the result (bh_essential_nodes) */
 
 /* ---- options (bh_set_option) ---------------------------------------------------------------- */
 #define BH_OPT_MAC    1   /* opening criterion */
@@ -48,6 +50,8 @@ typedef struct bh_ctx bh_ctx;
 #define BH_MAC_BARNES94 1 /*   Eq. 4:  accept iff d > l/theta + delta              */
 #define BH_OPT_GROUP  2   /* how many consecutive Morton-sorted targets share one walk and one vote */
                           /*   32 (default): the paper's warp vote; 1: per-target lists  */
+#define BH_OPT_PASS_TIMING 3 /* 1: bh_build records a CUDA event after every kernel (bh_get_build_passes); a
+                                reporting mode -- the events cost a little, 0 (default) records none          */
 
 #define BH_MAX_LEVEL 21               /* 21 key bits per dimension -> 63-bit keys */
 #define BH_DIRECT_ALL_MAX (1 << 18)   /* largest n for bh_potential_direct with targets == NULL */
@@ -65,7 +69,8 @@ typedef struct bh_stats {
     int64_t n_leaf;            /* last walk: sum over groups of leaf cells summed directly            */
     int64_t n_opened;          /* last walk: sum over groups of internal nodes opened                 */
     int64_t n_exact_tests;     /* last walk: nodes whose vote needed the per-target test (diagnostic)  */
-    double  interactions;      /* last walk: sum over TARGETS of (accepted + leaf) of their group     */
+    double  interactions;      /* last walk: sum over TARGETS of the list entries evaluated for their group,
+                                  counted by the Phi kernel itself at every list flush (the roofline numerator) */
     /* device time in ms of the passes of the last bh_build / bh_potential (CUDA events) */
     /* device ms of the last build: keys (a1), sort (a2), count = c(s) + level histograms + scan (a4),
      * assign = entity numbering + cells moved into their slots (a4 + a3), moments (a5), whole build */
@@ -73,6 +78,9 @@ typedef struct bh_stats {
     float ms_walk;
     int32_t launches_build;    /* kernels the last bh_build launched                                   */
     int32_t launches_walk;     /* kernels the last bh_potential launched                               */
+    int32_t walk_group;        /* BH_OPT_GROUP of the last walk (32 or 1): rows of the per-group outputs = ceil(n / it) */
+    double  interactions_counted; /* the same sum as `interactions`, from the count-only repeat of the traversal
+                                  ((accepted + leaf) of W6); equal to it unless the Phi kernel lost or doubled an entry */
 } bh_stats;
 
 /* ---- life cycle ----------------------------------------------------------------------------- */
@@ -96,7 +104,8 @@ int bh_set_option(bh_ctx* ctx, int key, int value);
  *   x, y, z, m : DEVICE, const double[n] each (SoA, "arrays with a one-dimensional layout",
  *                PAPER.md:96): cell centres and cell masses, caller's ("original") order.
  *                Borrowed until the stream has passed this call; the context keeps sorted copies.
- *   n          : 1 <= n < 2^31.
+ *   n          : 1 <= n < 2^30 (n in [2^30, 2^31) returns BH_ERR_TOO_LARGE: 30-bit tile counters of the sort,
+ *                and n + n_nodes must stay below 2^32; larger or non-positive n is BH_ERR_INVALID_ARG).
  *   cube       : HOST, const double[4] = {x0, y0, z0, L}: the root cube [x0,x0+L) x ....
  *                L > 0.  A coordinate outside the cube is clamped into the edge cell and counted
  *                (bh_stats.n_clamped); NaN coordinates quantise to 0.
@@ -147,20 +156,21 @@ int bh_essential_nodes(bh_ctx* ctx, const double box_lo[3], const double box_hi[
  * are skipped, and phi needs only ntargets entries. */
 int bh_set_num_targets(bh_ctx* ctx, int64_t ntargets);
 
-/* bh_measure_fma_peak: a MEASURED denominator for the walk's roofline (the walk is bound by the plain FP32
- * pipe; SURVEY.md §8(d) asks for the nominal peak and a measured FMA-chain peak side by side).  Runs, on the
- * context's stream, a kernel in which every thread advances 8 independent chains of fp32 FMAs from registers
- * -- packed (FFMA2, what the walk's evaluation issues) and scalar -- and returns the best of three timed
- * repetitions each, in TFLOP/s (2 flops per FMA).  Measurement aid, not part of the path; synchronises. */
-int bh_measure_fma_peak(bh_ctx* ctx, double* tflops_packed, double* tflops_scalar);
-
 /* bh_potential: Phi_i = -G sum_j m_j/|r_i - r_j| over the nodes and leaf cells the group walk of
  * PAPER.md:176-178 selects (DESIGN.md W-rules).
  *   theta : >= 0; theta = 0 opens every node (the result is then the direct sum in fp32 terms).
  *   G     : gravitational constant.
  *   phi   : DEVICE, double[n], ORIGINAL cell order; every element is written.
  * fp32 arithmetic for distances and m/d, accumulated in short fp32 blocks that are flushed into
- * fp64 sums.  The opening decision of a node is taken in fp32 exactly as DESIGN.md W8 states. */
+ * fp64 sums.  Precision contract (W8, W9):
+ *  - the opening decision d^2 > r_c^2 of a node is taken in fp32 on fp32-rounded operands, so a node whose
+ *    d^2 lies within ~1e-7 relative of r_c^2 for the deciding group member can fall on the other side than
+ *    in an fp64 evaluation of Eq. 3 / Eq. 4 ("flip": the group then sums the node's children instead of
+ *    the node, or the reverse -- both are valid Barnes-Hut lists; the difference is within the method's
+ *    own error).  Tests and bench.py count such groups against the fp64 oracle and report the count.
+ *  - positions are held in fp32: a pair at distance d carries a relative distance error up to
+ *    ~2^-23 L/d.  Cell centres of grids and AMR meshes (dyadic rationals) are exact; for arbitrary
+ *    points the 1e-4 bar on Phi holds while the closest pairs are farther apart than ~1e-3 L. */
 int bh_potential(bh_ctx* ctx, double theta, double G, double* phi);
 
 /* bh_field: bh_potential plus the acceleration g_i = -grad Phi_i in the same walk (
@@ -183,11 +193,36 @@ int bh_field(bh_ctx* ctx, double theta, double G, double* phi, double* acc);
 int bh_potential_direct(bh_ctx* ctx, double G, const int64_t* targets, int64_t nt, double* phi);
 
 /* One call with HOST buffers: copies x, y, z, m (double[n] each, pageable or pinned) to the
- * device, runs bh_build and bh_potential, copies phi (double[n]) back, synchronises. */
+ * device, runs bh_build and bh_potential, copies phi (double[n]) back, synchronises ("Only position and
+ * mass data is copied to the device ... just results are copied back").
+ * The copies run on a stream of their own, positions first: keys, sort and the entity counting start when
+ * x, y, z have landed and run beside the copy of m; the first kernel that reads a mass waits for it.
+ * Pinned (page-locked) buffers are copied in one asynchronous transfer each; pageable ones are staged through
+ * two pinned 16 MB chunks so that the CPU's copy of one chunk runs beside the DMA of the other. */
 int bh_solve_host(bh_ctx* ctx, const double* x, const double* y, const double* z, const double* m,
                   int64_t n, const double cube[4], double theta, double G, double* phi);
 
+/* Device-side time split of the last bh_solve_host (HOST output, milliseconds, CUDA events):
+ * ms[0] host->device copies (all four arrays), ms[1] build + walk (from the arrival of x, y, z to the end of
+ * the walk; includes any wait for m), ms[2] device->host copy of phi, ms[3] the whole call.
+ * ms[0] + ms[1] + ms[2] - ms[3] is the time the copies and the kernels overlapped. */
+int bh_host_breakdown(bh_ctx* ctx, float ms[4]);
+
 /* ---- parity / reporting --------------------------------------------------------------------- */
+
+/* One kernel (or small group of kernels) of the last bh_build, in launch order, when BH_OPT_PASS_TIMING was on:
+ * its device time and its ALGORITHMIC bytes by SURVEY.md §8(d) -- keys 36 B/cell; sort_hist 8 B/cell; each
+ * sort_pass 24 B/cell; topo_count 8 B/cell; topo_scan 0 (bookkeeping on the chunk histograms); assign_permute
+ * 84 B/cell + 24 B/node; moments_L<level> 32 B per leaf-cell child + 72 B per node of that level. */
+typedef struct bh_pass {
+    char   name[24];
+    float  ms;
+    double alg_bytes;
+} bh_pass;
+
+/* Fills out[0 .. min(cap, *count)) (HOST) with the passes of the last bh_build; *count = number recorded.
+ * Synchronises the stream.  BH_ERR_TOO_LARGE when cap is too small (the first cap entries are written). */
+int bh_get_build_passes(bh_ctx* ctx, bh_pass* out, int cap, int* count);
 
 /* Sizes of the last build (HOST outputs, any may be NULL). */
 int bh_tree_sizes(const bh_ctx* ctx, int64_t* n, int64_t* n_nodes, int64_t* n_slots);
@@ -207,6 +242,14 @@ int bh_export_tree(bh_ctx* ctx, uint64_t* keys, uint32_t* perm, int32_t* level, 
  * ceil(n / group), group g at [3g..3g+2] = {internal nodes accepted, leaf cells summed, internal
  * nodes opened}; same definition as the oracle's counters (W6). */
 int bh_last_group_counts(bh_ctx* ctx, int64_t* counts);
+
+/* The number of interaction-list entries the Phi kernel of the last bh_potential / bh_field itself
+ * evaluated for each group (counted at every list flush of the timed kernel, not by the count-only
+ * repeat that serves bh_last_group_counts): DEVICE uint32[ngroups].  Equals accepted + leaf of W6. */
+int bh_last_group_evaluated(bh_ctx* ctx, uint32_t* per_group);
+
+/* BH_OPT_GROUP of the last walk (32 or 1), or a negative BH_ERR_*: sizes the per-group outputs. */
+int bh_last_walk_group(const bh_ctx* ctx);
 
 /* Interactions evaluated for each target in the last bh_potential (accepted + leaf of its group;
  * the target's own cell is counted as evaluated-and-masked): DEVICE uint32[n], original order. */

@@ -190,14 +190,14 @@ class OracleTree:
         rec = rec[:k].copy()
         return (rec, lev[:k].copy(), lo[:k].copy(), hi[:k].copy()) if want_ranges else rec
 
-    def field(self, theta, G=1.0, mac=MAC_BH86, group=32, mac_fp32=False, groups=None):
+    def field(self, theta, G=1.0, mac=MAC_BH86, group=32, mac_fp32=False, groups=None, out=None):
         """NEXT-4: the group walk returning (phi[n], acc[n, 3]) in ORIGINAL order; acc = -grad phi evaluated
         on the same interaction lists (monopole gradient of every accepted node and leaf cell).
-        `groups` = (begin, end) restricts the walk; cells not walked stay NaN."""
+        `groups` = (begin, end) restricts the walk; cells not walked stay NaN.
+        `out`: reuse a (float64[n], float64[n, 3]) pair of buffers (marshalling only)."""
         ng = (self.n + group - 1) // group
         gb, ge = (0, ng) if groups is None else groups
-        phi = np.full(self.n, np.nan)
-        acc = np.full((self.n, 3), np.nan)
+        phi, acc = (np.full(self.n, np.nan), np.full((self.n, 3), np.nan)) if out is None else out
         rc = _L().orc_field(self._h, float(theta), float(G), int(mac), int(group), int(bool(mac_fp32)),
                             gb, ge, _p(phi, C.c_double), _p(acc, C.c_double), None)
         if rc != 0:

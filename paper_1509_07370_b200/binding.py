@@ -10,12 +10,14 @@ BH_MAC_BH86 = 0       # Eq. 3
 BH_MAC_BARNES94 = 1   # Eq. 4
 BH_OPT_MAC = 1
 BH_OPT_GROUP = 2
+BH_OPT_PASS_TIMING = 3
 BH_DIRECT_ALL_MAX = 1 << 18
 
 EXPORTED_SYMBOLS = (
     "bh_create", "bh_destroy", "bh_strerror", "bh_last_cuda_error", "bh_set_option", "bh_build", "bh_potential",
     "bh_potential_direct", "bh_solve_host", "bh_tree_sizes", "bh_export_tree", "bh_last_group_counts",
-    "bh_last_interactions", "bh_get_stats", "bh_update_masses", "bh_essential_nodes", "bh_set_num_targets", "bh_field", "bh_measure_fma_peak",
+    "bh_last_interactions", "bh_get_stats", "bh_update_masses", "bh_essential_nodes", "bh_set_num_targets", "bh_field",
+    "bh_last_group_evaluated", "bh_last_walk_group", "bh_get_build_passes", "bh_host_breakdown",
 )
 
 
@@ -26,10 +28,15 @@ class Stats(C.Structure):
                 ("n_exact_tests", C.c_int64), ("interactions", C.c_double),
                 ("ms_keys", C.c_float), ("ms_sort", C.c_float), ("ms_count", C.c_float),
                 ("ms_assign", C.c_float), ("ms_moments", C.c_float), ("ms_build_total", C.c_float),
-                ("ms_walk", C.c_float), ("launches_build", C.c_int32), ("launches_walk", C.c_int32)]
+                ("ms_walk", C.c_float), ("launches_build", C.c_int32), ("launches_walk", C.c_int32),
+                ("walk_group", C.c_int32), ("interactions_counted", C.c_double)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+class Pass(C.Structure):
+    _fields_ = [("name", C.c_char * 24), ("ms", C.c_float), ("alg_bytes", C.c_double)]
 
 
 class BHError(RuntimeError):
@@ -64,7 +71,6 @@ def lib():
         L.bh_essential_nodes.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_double, dp, i64,
                                          C.POINTER(i64)]
         L.bh_set_num_targets.argtypes = [vp, i64]
-        L.bh_measure_fma_peak.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.bh_potential.argtypes = [vp, C.c_double, C.c_double, dp]
         L.bh_field.argtypes = [vp, C.c_double, C.c_double, dp, dp]
         L.bh_potential_direct.argtypes = [vp, C.c_double, dp, i64, dp]
@@ -73,6 +79,10 @@ def lib():
         L.bh_export_tree.argtypes = [vp] + [dp] * 12
         L.bh_last_group_counts.argtypes = [vp, dp]
         L.bh_last_interactions.argtypes = [vp, dp]
+        L.bh_last_group_evaluated.argtypes = [vp, dp]
+        L.bh_last_walk_group.argtypes = [vp]
+        L.bh_get_build_passes.argtypes = [vp, C.POINTER(Pass), i32, C.POINTER(i32)]
+        L.bh_host_breakdown.argtypes = [vp, C.POINTER(C.c_float)]
         L.bh_get_stats.argtypes = [vp, C.POINTER(Stats)]
         for name in EXPORTED_SYMBOLS:
             if name not in ("bh_strerror", "bh_last_cuda_error"):
@@ -86,7 +96,12 @@ def _cube(c):
 
 
 class Context:
-    """One tree on one CUDA stream (bh_create ... bh_destroy).  Tensors are torch CUDA tensors."""
+    """One tree on one CUDA stream (bh_create ... bh_destroy).  Tensors are torch CUDA tensors.
+
+    Stream contract: every call enqueues its kernels on the stream given here (default: the torch stream
+    current at construction).  Tensors handed to a call while ANOTHER torch stream is current are marked
+    with `record_stream`, so the caching allocator does not reuse them while libbh kernels are in flight;
+    ordering between the two streams stays the caller's business (wait_stream / events)."""
 
     def __init__(self, device: int = 0, stream=None):
         import torch
@@ -114,6 +129,8 @@ class Context:
         torch = self._torch
         if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()):
             raise TypeError(f"expected a contiguous CUDA tensor of dtype {dtype}")
+        if torch.cuda.current_stream(self.device) != self.stream:
+            t.record_stream(self.stream)        # the tensor is used on the context's stream, not the current one
         return C.c_void_p(t.data_ptr())
 
     def close(self):
@@ -177,12 +194,6 @@ class Context:
             res = out[: cnt.value]
             return res.clone() if cap > cnt.value + (cnt.value >> 2) + 4096 else res     # do not pin a much larger buffer
 
-    def measure_fma_peak(self):
-        """bh_measure_fma_peak: (packed FFMA2, scalar FFMA) register-resident FMA-chain rates in TFLOP/s."""
-        a, b = C.c_double(0.0), C.c_double(0.0)
-        self._check(self._L.bh_measure_fma_peak(self._h, C.byref(a), C.byref(b)))
-        return a.value, b.value
-
     def set_num_targets(self, ntargets: int):
         """bh_set_num_targets: cells with original index < ntargets are targets, the rest sources only (-1: all)."""
         self._check(self._L.bh_set_num_targets(self._h, int(ntargets)))
@@ -234,6 +245,21 @@ class Context:
         self.n = n
         return out
 
+    def host_breakdown(self):
+        """bh_host_breakdown: dict of the last solve_host's device-side time split in ms."""
+        ms = (C.c_float * 4)()
+        self._check(self._L.bh_host_breakdown(self._h, ms))
+        return {"h2d_ms": ms[0], "device_ms": ms[1], "d2h_ms": ms[2], "total_ms": ms[3],
+                "overlap_ms": ms[0] + ms[1] + ms[2] - ms[3]}
+
+    def build_passes(self):
+        """bh_get_build_passes: [(name, ms, algorithmic bytes)] of the last build (BH_OPT_PASS_TIMING on)."""
+        cap = 96
+        arr = (Pass * cap)()
+        cnt = C.c_int(0)
+        self._check(self._L.bh_get_build_passes(self._h, arr, cap, C.byref(cnt)))
+        return [(arr[k].name.decode(), float(arr[k].ms), float(arr[k].alg_bytes)) for k in range(cnt.value)]
+
     def tree_sizes(self):
         n, nn, ns = C.c_int64(), C.c_int64(), C.c_int64()
         self._check(self._L.bh_tree_sizes(self._h, C.byref(n), C.byref(nn), C.byref(ns)))
@@ -252,20 +278,39 @@ class Context:
             Rx=torch.empty(nn, dtype=torch.float64, device=dev), Ry=torch.empty(nn, dtype=torch.float64, device=dev),
             Rz=torch.empty(nn, dtype=torch.float64, device=dev), delta=torch.empty(nn, dtype=torch.float64, device=dev))
         order = ("keys", "perm", "level", "prefix", "lo", "hi", "nchild", "M", "Rx", "Ry", "Rz", "delta")
-        self._check(self._L.bh_export_tree(self._h, *[C.c_void_p(out[k].data_ptr()) for k in order]))
+        self._check(self._L.bh_export_tree(self._h, *[self._dev(out[k], out[k].dtype) for k in order]))
         return out
 
-    def last_group_counts(self, group: int = 32):
+    def last_walk_group(self) -> int:
+        """BH_OPT_GROUP of the last walk (32 or 1)."""
+        g = self._L.bh_last_walk_group(self._h)
+        if g < 0:
+            self._check(g)
+        return g
+
+    def last_group_counts(self):
+        """[ngroups, 3] int64 = (accepted, leaf, opened) per group of the last walk; ngroups follows the
+        group size of that walk (bh_last_walk_group), not an argument of this call."""
         torch = self._torch
+        group = self.last_walk_group()
         ng = (self.n + group - 1) // group
         out = torch.empty((ng, 3), dtype=torch.int64, device=f"cuda:{self.device}")
-        self._check(self._L.bh_last_group_counts(self._h, C.c_void_p(out.data_ptr())))
+        self._check(self._L.bh_last_group_counts(self._h, self._dev(out, torch.int64)))
+        return out
+
+    def last_group_evaluated(self):
+        """[ngroups] int32: list entries the Phi kernel itself evaluated for each group of the last walk."""
+        torch = self._torch
+        group = self.last_walk_group()
+        ng = (self.n + group - 1) // group
+        out = torch.empty(ng, dtype=torch.int32, device=f"cuda:{self.device}")
+        self._check(self._L.bh_last_group_evaluated(self._h, self._dev(out, torch.int32)))
         return out
 
     def last_interactions(self):
         torch = self._torch
         out = torch.empty(self.n, dtype=torch.int32, device=f"cuda:{self.device}")
-        self._check(self._L.bh_last_interactions(self._h, C.c_void_p(out.data_ptr())))
+        self._check(self._L.bh_last_interactions(self._h, self._dev(out, torch.int32)))
         return out
 
     def get_stats(self) -> Stats:

@@ -10,6 +10,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libbh.so")
+PEAK_LIB = os.path.join(HERE, "libbh_fma_peak.so")      # bench.py's measured FP32 denominator; not part of libbh
+PEAK_SRC = os.path.join(CSRC, "fma_peak.cu")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
 
@@ -22,8 +24,8 @@ def _nvcc() -> str:
 
 
 def sources():
-    return sorted(glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cuh")) +
-                  [os.path.join(os.path.dirname(HERE), "include", "bh.h")])
+    return sorted([s for s in glob.glob(os.path.join(CSRC, "*.cu")) if s != PEAK_SRC] +
+                  glob.glob(os.path.join(CSRC, "*.cuh")) + [os.path.join(os.path.dirname(HERE), "include", "bh.h")])
 
 
 def needs_build() -> bool:
@@ -42,5 +44,13 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_fma_peak(force: bool = False) -> str:
+    """The FMA-chain peak measurement bench.py reports beside the nominal FP32 peak (its own small library)."""
+    if force or not os.path.exists(PEAK_LIB) or os.path.getmtime(PEAK_LIB) < os.path.getmtime(PEAK_SRC):
+        subprocess.check_call([_nvcc()] + NVCC_FLAGS + ["-o", PEAK_LIB, PEAK_SRC])
+    return PEAK_LIB
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build_fma_peak(force="--force" in sys.argv))

@@ -12,7 +12,6 @@
 #include "direct.cuh"
 #include "keys.cuh"
 #include "let.cuh"
-#include "peak.cuh"
 #include "scan.cuh"
 #include "sort.cuh"
 #include "tree.cuh"
@@ -44,10 +43,13 @@ struct DeviceScalars {          // small device-resident results read back by th
     u32 topo_rows[kTopoDigits + 1];   // row starts of the scanned level histogram + grand total
     u32 scan_total;
     u32 max_bucket;
-    unsigned long long totals[5];
+    unsigned long long totals[6];     // sums of the four twin counters, twin interactions, the Phi kernel's own interactions
 };
 
-enum { EV_B0, EV_KEYS, EV_SORT, EV_PERM, EV_TOPO, EV_MOM, EV_W0, EV_W1, EV_COUNT };
+enum { EV_B0, EV_KEYS, EV_SORT, EV_PERM, EV_TOPO, EV_MOM, EV_W0, EV_W1,
+       EV_H0, EV_HC0, EV_HXYZ, EV_HM, EV_HD0, EV_HD1, EV_HEND, EV_COUNT };   // EV_H*: bh_solve_host
+
+constexpr size_t kStageChunk = 16u << 20;      // pinned staging chunk of bh_solve_host for pageable callers
 
 }  // namespace
 
@@ -89,15 +91,30 @@ struct bh_ctx {
     // walk
     i64 ntargets = -1;                    // bh_set_num_targets: cells [0, ntargets) are targets; -1 = all
     DevBuf ess_state, ess_emit;           // bh_essential_nodes: per-slot flags
-    DevBuf gcount;
+    DevBuf gcount;                        // W6 counters of the count-only twin (lazy)
+    DevBuf geval;                         // list entries the Phi kernel itself evaluated, per group
     DevBuf scalars;                       // DeviceScalars
     DeviceScalars* h_scalars = nullptr;   // pinned host mirror
     DevBuf stage[4];                      // bh_solve_host staging (x, y, z, m) and phi
     DevBuf stage_phi;
+    cudaStream_t copy_stream = nullptr;   // bh_solve_host: the host->device copies run beside the build
+    cudaEvent_t assign_wait = nullptr;    // set by bh_solve_host: the masses land after the positions; the first kernel
+                                          // that reads m (the assigning kernel) waits for this event
+    void* pinned[2] = {nullptr, nullptr}; // two staging chunks for pageable host buffers
+    cudaEvent_t pinned_ev[2] = {nullptr, nullptr};
+    bool host_timed = false;
 
     cudaEvent_t ev[EV_COUNT] = {nullptr};
     bool ev_build = false, ev_walk = false;
     int launches_build = 0, launches_walk = 0;
+
+    // BH_OPT_PASS_TIMING: one event after every kernel of bh_build (a reporting mode: the events add gaps)
+    bool pass_timing = false;
+    static constexpr int kMaxPasses = 96;
+    cudaEvent_t pev[kMaxPasses] = {nullptr};
+    char pname[kMaxPasses][24];
+    double pbytes[kMaxPasses];
+    int npass = 0;
 };
 
 namespace {
@@ -114,6 +131,18 @@ int cuda_fail(bh_ctx* c, cudaError_t e, const char* where)
         cudaError_t e__ = (call);                                        \
         if (e__ != cudaSuccess) return cuda_fail(ctx, e__, #call);       \
     } while (0)
+
+// per-pass timing: closes the pass `name` (everything enqueued since the previous mark) with an event
+void pass_mark(bh_ctx* ctx, const char* name, double alg_bytes)
+{
+    if (!ctx->pass_timing || ctx->npass >= bh_ctx::kMaxPasses) return;
+    const int k = ctx->npass;
+    if (!ctx->pev[k] && cudaEventCreate(&ctx->pev[k]) != cudaSuccess) { cudaGetLastError(); return; }
+    snprintf(ctx->pname[k], sizeof(ctx->pname[k]), "%s", name);
+    ctx->pbytes[k] = alg_bytes;
+    cudaEventRecord(ctx->pev[k], ctx->stream);
+    ctx->npass = k + 1;
+}
 
 inline unsigned blocks_for(i64 n, int threads) { return (unsigned)((n + threads - 1) / threads); }
 
@@ -140,13 +169,26 @@ int launch_moments(bh_ctx* ctx)
     MA.x0 = ctx->cube[0]; MA.y0 = ctx->cube[1]; MA.z0 = ctx->cube[2]; MA.L = ctx->cube[3];
     SmallLevels sl;
     sl.nlev = 0;
+    double small_bytes = 0.0;
     for (int l = ctx->maxlevel; l >= -1; --l) {
         const i64 b0 = l >= 0 ? ctx->lv.node_base[l] : 0, b1 = l >= 0 ? ctx->lv.node_base[l + 1] : 0;
         const bool small = l >= 0 && b1 - b0 <= kSmallLevelNodes;
+        // 32 B per leaf cell read + 72 B per node (fp64 moments + packed record); the children
+        // of level l are the level-(l+1) entities, of which the level-(l+1) nodes are not leaf cells
+        double lvl_bytes = 0.0;
+        if (l >= 0) {
+            const double kids = (double)ctx->lv.slot_base[l + 2] - (double)ctx->lv.slot_base[l + 1];
+            const double inner = l + 1 < kNumLevels ? (double)ctx->lv.node_base[l + 2] - (double)ctx->lv.node_base[l + 1] : 0.0;
+            lvl_bytes = 32.0 * (kids - inner) + 72.0 * (double)(b1 - b0);
+        }
         if ((!small || l < 0) && sl.nlev > 0) {          // flush the pending run of small levels
             moments_small_kernel<<<1, kMomSmallThreads, 0, st>>>(sl, MA);
             BH_CUDA(cudaGetLastError());
             ctx->launches_build += 1;
+            char nm[24];
+            snprintf(nm, sizeof(nm), "moments_L%d-%d", sl.level[sl.nlev - 1], sl.level[0]);
+            pass_mark(ctx, nm, small_bytes);
+            small_bytes = 0.0;
             sl.nlev = 0;
         }
         if (l < 0 || b1 == b0) continue;
@@ -154,10 +196,14 @@ int launch_moments(bh_ctx* ctx)
             sl.level[sl.nlev] = l; sl.b0[sl.nlev] = (u32)b0; sl.b1[sl.nlev] = (u32)b1;
             sl.slot_end[sl.nlev] = ctx->lv.slot_base[l + 2];
             ++sl.nlev;
+            small_bytes += lvl_bytes;
         } else {
             moments_kernel<<<blocks_for(b1 - b0, 128), 128, 0, st>>>(b0, b1, l, ctx->lv.slot_base[l + 2], MA);
             BH_CUDA(cudaGetLastError());
             ctx->launches_build += 1;
+            char nm[24];
+            snprintf(nm, sizeof(nm), "moments_L%d", l);
+            pass_mark(ctx, nm, lvl_bytes);
         }
     }
     return BH_OK;
@@ -208,6 +254,7 @@ int bh_create(bh_ctx** out, int device, void* cuda_stream)
         for (int i = 0; i < EV_COUNT; ++i)
             if ((e = cudaEventCreate(&ctx->ev[i])) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaEventCreate"); break; }
         if (rc) break;
+        if ((e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking)) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaStreamCreate"); break; }
         if ((e = ctx->scalars.ensure(sizeof(DeviceScalars))) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaMalloc"); break; }
         if ((e = cudaMallocHost(&ctx->h_scalars, sizeof(DeviceScalars))) != cudaSuccess) { rc = cuda_fail(ctx, e, "cudaMallocHost"); break; }
         // kernels whose dynamic shared memory exceeds the 48 KB default
@@ -243,11 +290,17 @@ int bh_destroy(bh_ctx* ctx)
     cudaStreamSynchronize(ctx->stream);
     DevBuf* all[] = {&ctx->keysA, &ctx->keysB, &ctx->idxA, &ctx->idxB, &ctx->clev, &ctx->leaf_slot, &ctx->leaf64,
                      &ctx->slot_of, &ctx->hist, &ctx->scan_scratch, &ctx->nlo, &ctx->nfirst, &ctx->node_slot,
-                     &ctx->delta64, &ctx->rec64, &ctx->rec, &ctx->aux, &ctx->gcount, &ctx->scalars, &ctx->stage[0],
+                     &ctx->delta64, &ctx->rec64, &ctx->rec, &ctx->aux, &ctx->gcount, &ctx->geval, &ctx->scalars, &ctx->stage[0],
                      &ctx->stage[1], &ctx->stage[2], &ctx->stage[3], &ctx->stage_phi, &ctx->ess_state, &ctx->ess_emit};
     for (DevBuf* b : all) b->release();
     if (ctx->h_scalars) cudaFreeHost(ctx->h_scalars);
+    if (ctx->copy_stream) { cudaStreamSynchronize(ctx->copy_stream); cudaStreamDestroy(ctx->copy_stream); }
+    for (int i = 0; i < 2; ++i) {
+        if (ctx->pinned[i]) cudaFreeHost(ctx->pinned[i]);
+        if (ctx->pinned_ev[i]) cudaEventDestroy(ctx->pinned_ev[i]);
+    }
     for (int i = 0; i < EV_COUNT; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+    for (int i = 0; i < bh_ctx::kMaxPasses; ++i) if (ctx->pev[i]) cudaEventDestroy(ctx->pev[i]);
     delete ctx;
     return BH_OK;
 }
@@ -257,6 +310,7 @@ int bh_set_option(bh_ctx* ctx, int key, int value)
     if (!ctx) return BH_ERR_INVALID_ARG;
     if (key == BH_OPT_MAC && (value == BH_MAC_BH86 || value == BH_MAC_BARNES94)) { ctx->mac = value; return BH_OK; }
     if (key == BH_OPT_GROUP && (value == 32 || value == 1)) { ctx->group = value; return BH_OK; }
+    if (key == BH_OPT_PASS_TIMING && (value == 0 || value == 1)) { ctx->pass_timing = value != 0; ctx->npass = 0; return BH_OK; }
     return BH_ERR_INVALID_ARG;
 }
 
@@ -301,6 +355,7 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
     for (int attempt = 0;; ++attempt) {
         const bool speculate = attempt == 0 && ctx->plan_hint_valid;
         ctx->launches_build = 0;
+        ctx->npass = 0;
         BH_CUDA(cudaMemsetAsync(ds, 0, sizeof(DeviceScalars), st));
         {   // key_and starts as all ones
             const u64 ones = ~0ULL;
@@ -320,6 +375,7 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
             BH_CUDA(cudaGetLastError());
         }
         ctx->launches_build += 1;
+        pass_mark(ctx, "keys", 36.0 * (double)n);
         BH_CUDA(cudaEventRecord(ctx->ev[EV_KEYS], st));
 
         // read-back 1: which key bits vary (decides the radix passes) and the clamp count
@@ -338,7 +394,8 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
             BH_CUDA(ctx->idxB.ensure(sizeof(u32) * n));
         }
         BH_CUDA(radix_sort_pairs(ctx->keysA.as<u64>(), ctx->idxA.as<u32>(), ctx->keysB.as<u64>(), ctx->idxB.as<u32>(), n,
-                                 plan, ctx->hist.as<u32>(), persistent_grid(ctx, 8), st));
+                                 plan, ctx->hist.as<u32>(), persistent_grid(ctx, 8), st,
+                                 [ctx](const char* nm, double b) { pass_mark(ctx, nm, b); }));
         ctx->launches_build += plan.npasses ? 1 + plan.npasses : 0;   // histogram + one kernel per pass
         {
             const bool odd = plan.npasses & 1;
@@ -366,10 +423,12 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
             u32* hist = ctx->hist.as<u32>();
             topo_count_kernel<<<tgrid, kTopoThreads, 0, st>>>(ctx->sv, n, ctx->clev.as<signed char>(), hist, nchunks);
             BH_CUDA(cudaGetLastError());
+            pass_mark(ctx, "topo_count", 8.0 * (double)n);
             BH_CUDA(exclusive_scan_u32(hist, hist, (i64)kTopoDigits * nchunks, ctx->scan_scratch.as<u32>(),
                                        &ds->scan_total, st));
             topo_totals_kernel<<<1, 64, 0, st>>>(hist, nchunks, &ds->scan_total, ds->topo_rows);
             BH_CUDA(cudaGetLastError());
+            pass_mark(ctx, "topo_scan", 0.0);
             // read-back 2: entities and nodes per level (sizes every node / slot array)
             BH_CUDA(cudaMemcpyAsync(ctx->h_scalars->topo_rows, ds->topo_rows, sizeof(u32) * (kTopoDigits + 1),
                                     cudaMemcpyDeviceToHost, st));
@@ -397,8 +456,18 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
     if (n >= 2) {
         u32* hist = ctx->hist.as<u32>();
         const u32* rows = ctx->h_scalars->topo_rows;
-        const i64 nslots = rows[kSlotLevels];                 // entities of all levels = n + n_nodes
-        const i64 nn = (i64)rows[kTopoDigits] - nslots;
+        // The device scan runs in u32.  Every histogram row sums to at most n < 2^30, so consecutive row
+        // starts differ by less than 2^30 and the true 64-bit starts follow from the differences mod 2^32.
+        unsigned long long true_rows[kTopoDigits + 1];
+        true_rows[0] = rows[0];
+        for (int d = 1; d <= kTopoDigits; ++d) true_rows[d] = true_rows[d - 1] + (u32)(rows[d] - rows[d - 1]);
+        if (true_rows[kSlotLevels] >= (1ULL << 32)) {          // slots are u32: n + n_nodes must stay below 2^32
+            snprintf(ctx->cuda_msg, sizeof(ctx->cuda_msg), "n + n_nodes = %llu needs more than 32-bit slots",
+                     true_rows[kSlotLevels]);
+            return BH_ERR_TOO_LARGE;
+        }
+        const i64 nslots = (i64)true_rows[kSlotLevels];       // entities of all levels = n + n_nodes
+        const i64 nn = (i64)(true_rows[kTopoDigits] - true_rows[kSlotLevels]);
         for (int l = 0; l <= kSlotLevels; ++l) ctx->lv.slot_base[l] = rows[l];
         for (int l = 0; l <= kNumLevels; ++l) ctx->lv.node_base[l] = (u32)(rows[kSlotLevels + l] - nslots);
         for (int l = 0; l < kNumLevels; ++l)
@@ -425,11 +494,14 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
         BH_CUDA(ctx->rec64.ensure(sizeof(double4) * nslots));
         BH_CUDA(ctx->rec.ensure(sizeof(float4) * nslots));
 
+        pass_mark(ctx, "aux_clear+readback", 0.0);      // node-slot aux clearing and the idle wait for the level totals
+        if (ctx->assign_wait) BH_CUDA(cudaStreamWaitEvent(st, ctx->assign_wait, 0));   // bh_solve_host: m is still landing
         topo_assign_kernel<<<tgrid, kTopoThreads, 0, st>>>(
             ctx->clev.as<signed char>(), n, ctx->sv, x, y, z, m, hist, nchunks, (u32)nslots,
             ctx->leaf_slot.as<u32>(), ctx->node_slot.as<u32>(), ctx->nfirst.as<u32>(), ctx->nlo.as<u32>(),
             ctx->rec64.as<double4>(), ctx->rec.as<float4>());
         BH_CUDA(cudaGetLastError());
+        pass_mark(ctx, "assign_permute", 84.0 * (double)n + 24.0 * (double)nn);   // a3 84 B/cell + a4 24 B/node
         ctx->launches_build += 1 + 3 + 1 + 1;   // count, scan, totals, assign
         BH_CUDA(cudaEventRecord(ctx->ev[EV_TOPO], st));
 
@@ -438,6 +510,7 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
         ctx->aux_dirty_nn = nn;
     } else {
         // n = 1: no tree (T-rule 1); the lone cell's record is kept for bh_essential_nodes
+        if (ctx->assign_wait) BH_CUDA(cudaStreamWaitEvent(st, ctx->assign_wait, 0));
         BH_CUDA(ctx->rec64.ensure(sizeof(double4)));
         const double* src[4] = {x, y, z, m};
         for (int a = 0; a < 4; ++a)
@@ -470,37 +543,6 @@ int bh_update_masses(bh_ctx* ctx, const double* m)
         { int rc = launch_moments(ctx); if (rc != BH_OK) return rc; }
     }
     BH_CUDA(cudaEventRecord(ctx->ev[EV_MOM], st));
-    return BH_OK;
-}
-
-int bh_measure_fma_peak(bh_ctx* ctx, double* tflops_packed, double* tflops_scalar)
-{
-    if (!ctx || !tflops_packed || !tflops_scalar) return BH_ERR_INVALID_ARG;
-    BH_CUDA(cudaSetDevice(ctx->device));
-    cudaStream_t st = ctx->stream;
-    const int grid = persistent_grid(ctx, 8), iters = 1 << 15;
-    BH_CUDA(ctx->gcount.ensure(sizeof(float) * (size_t)grid * 256));
-    float* out = ctx->gcount.as<float>();
-    ctx->counts_valid = false;                       // gcount doubles as the sink of the chains
-    cudaEvent_t e0 = ctx->ev[EV_W0], e1 = ctx->ev[EV_W1];
-    ctx->ev_walk = false;
-    const double flops = (double)grid * 256.0 * iters * kPeakChains * 2.0 * 2.0;   // 2 lanes x (mul + add)
-    double* res[2] = {tflops_packed, tflops_scalar};
-    for (int v = 0; v < 2; ++v) {
-        float best = 1e30f;
-        for (int rep = 0; rep < 4; ++rep) {          // first repetition warms up
-            BH_CUDA(cudaEventRecord(e0, st));
-            if (v == 0) fp32_fma_chain_kernel<true><<<grid, 256, 0, st>>>(out, iters, 0.999f, 1e-3f);
-            else fp32_fma_chain_kernel<false><<<grid, 256, 0, st>>>(out, iters, 0.999f, 1e-3f);
-            BH_CUDA(cudaGetLastError());
-            BH_CUDA(cudaEventRecord(e1, st));
-            BH_CUDA(cudaStreamSynchronize(st));
-            float ms = 0.f;
-            BH_CUDA(cudaEventElapsedTime(&ms, e0, e1));
-            if (rep > 0 && ms < best) best = ms;
-        }
-        *res[v] = flops / (best * 1e-3) / 1e12;
-    }
     return BH_OK;
 }
 
@@ -591,10 +633,12 @@ int launch_walk(bh_ctx* ctx, double theta, double G, double* phi, int group, int
     const i64 n = ctx->n;
     const i64 ngroups = (n + group - 1) / group;
     BH_CUDA(ctx->gcount.ensure(sizeof(uint4) * ngroups));
+    BH_CUDA(ctx->geval.ensure(sizeof(u32) * ngroups));
     if (n == 1) {   // T-rule 1: a lone cell has no tree; Phi = 0
         if (!count_only) BH_CUDA(cudaMemsetAsync(phi, 0, sizeof(double), st));
         if (!count_only && acc) BH_CUDA(cudaMemsetAsync(acc, 0, 3 * sizeof(double), st));
         BH_CUDA(cudaMemsetAsync(ctx->gcount.p, 0, sizeof(uint4), st));
+        if (!count_only) BH_CUDA(cudaMemsetAsync(ctx->geval.p, 0, sizeof(u32), st));
         return BH_OK;
     }
     WalkParams P;
@@ -605,6 +649,7 @@ int launch_walk(bh_ctx* ctx, double theta, double G, double* phi, int group, int
     P.phi = phi;
     P.acc = acc;
     P.gcount = ctx->gcount.as<uint4>();
+    P.geval = ctx->geval.as<u32>();
     P.n = n;
     P.ngroups = ngroups;
     P.inv_theta = (float)(1.0 / theta);
@@ -717,25 +762,134 @@ int bh_potential_direct(bh_ctx* ctx, double G, const int64_t* targets, int64_t n
     return BH_OK;
 }
 
+}  // extern "C" (reopened below)
+
+namespace {
+
+bool is_pinned(const void* p)
+{
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeHost || a.type == cudaMemoryTypeManaged;
+}
+
+int ensure_pinned_chunks(bh_ctx* ctx)
+{
+    for (int i = 0; i < 2; ++i) {
+        if (!ctx->pinned[i]) BH_CUDA(cudaMallocHost(&ctx->pinned[i], kStageChunk));
+        if (!ctx->pinned_ev[i]) BH_CUDA(cudaEventCreateWithFlags(&ctx->pinned_ev[i], cudaEventDisableTiming));
+    }
+    return BH_OK;
+}
+
+// host -> device on `st`.  Pinned sources go in one asynchronous copy; pageable ones are staged through two
+// pinned chunks so that the CPU's memcpy of chunk k+1 runs beside the DMA of chunk k.
+int h2d(bh_ctx* ctx, void* dst, const void* src, size_t bytes, cudaStream_t st)
+{
+    if (is_pinned(src)) { BH_CUDA(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, st)); return BH_OK; }
+    { int rc = ensure_pinned_chunks(ctx); if (rc != BH_OK) return rc; }
+    int k = 0;
+    for (size_t off = 0; off < bytes; off += kStageChunk, k ^= 1) {
+        const size_t len = bytes - off < kStageChunk ? bytes - off : kStageChunk;
+        BH_CUDA(cudaEventSynchronize(ctx->pinned_ev[k]));            // the chunk's previous DMA is done
+        memcpy(ctx->pinned[k], static_cast<const char*>(src) + off, len);
+        BH_CUDA(cudaMemcpyAsync(static_cast<char*>(dst) + off, ctx->pinned[k], len, cudaMemcpyHostToDevice, st));
+        BH_CUDA(cudaEventRecord(ctx->pinned_ev[k], st));
+    }
+    return BH_OK;
+}
+
+// device -> host on `st`, complete on return for pageable destinations (staged the same way)
+int d2h(bh_ctx* ctx, void* dst, const void* src, size_t bytes, cudaStream_t st)
+{
+    if (is_pinned(dst)) { BH_CUDA(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, st)); return BH_OK; }
+    { int rc = ensure_pinned_chunks(ctx); if (rc != BH_OK) return rc; }
+    const size_t nchunk = (bytes + kStageChunk - 1) / kStageChunk;
+    for (size_t c = 0; c <= nchunk; ++c) {           // DMA of chunk c runs beside the CPU's memcpy of chunk c - 1
+        if (c < nchunk) {
+            const size_t off = c * kStageChunk, len = bytes - off < kStageChunk ? bytes - off : kStageChunk;
+            BH_CUDA(cudaMemcpyAsync(ctx->pinned[c & 1], static_cast<const char*>(src) + off, len, cudaMemcpyDeviceToHost, st));
+            BH_CUDA(cudaEventRecord(ctx->pinned_ev[c & 1], st));
+        }
+        if (c > 0) {
+            const size_t off = (c - 1) * kStageChunk, len = bytes - off < kStageChunk ? bytes - off : kStageChunk;
+            BH_CUDA(cudaEventSynchronize(ctx->pinned_ev[(c - 1) & 1]));
+            memcpy(static_cast<char*>(dst) + off, ctx->pinned[(c - 1) & 1], len);
+        }
+    }
+    return BH_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
 int bh_solve_host(bh_ctx* ctx, const double* x, const double* y, const double* z, const double* m, int64_t n,
                   const double cube[4], double theta, double G, double* phi)
 {
     if (!ctx || !x || !y || !z || !m || !cube || !phi || n <= 0 || n >= 2147483648LL) return BH_ERR_INVALID_ARG;
     BH_CUDA(cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream, cs = ctx->copy_stream;
+    for (int k = 0; k < 4; ++k) BH_CUDA(ctx->stage[k].ensure(sizeof(double) * n));
+    BH_CUDA(ctx->stage_phi.ensure(sizeof(double) * n));
+    ctx->host_timed = false;
+    // The copies run on their own stream, positions first: the build (keys, sort, counting -- none of which
+    // reads a mass) starts as soon as x, y, z have landed, the assigning kernel waits for m.
+    BH_CUDA(cudaEventRecord(ctx->ev[EV_H0], st));
+    BH_CUDA(cudaStreamWaitEvent(cs, ctx->ev[EV_H0], 0));           // the staging buffers may still be in use on `st`
+    BH_CUDA(cudaEventRecord(ctx->ev[EV_HC0], cs));
     const double* src[4] = {x, y, z, m};
     for (int k = 0; k < 4; ++k) {
-        BH_CUDA(ctx->stage[k].ensure(sizeof(double) * n));
-        BH_CUDA(cudaMemcpyAsync(ctx->stage[k].p, src[k], sizeof(double) * n, cudaMemcpyHostToDevice, ctx->stream));
+        int rc = h2d(ctx, ctx->stage[k].p, src[k], sizeof(double) * n, cs);
+        if (rc != BH_OK) return rc;
+        if (k == 2) BH_CUDA(cudaEventRecord(ctx->ev[EV_HXYZ], cs));
     }
-    BH_CUDA(ctx->stage_phi.ensure(sizeof(double) * n));
+    BH_CUDA(cudaEventRecord(ctx->ev[EV_HM], cs));
+    BH_CUDA(cudaStreamWaitEvent(st, ctx->ev[EV_HXYZ], 0));
+    BH_CUDA(cudaEventRecord(ctx->ev[EV_HD0], st));
+    ctx->assign_wait = ctx->ev[EV_HM];
     int rc = bh_build(ctx, ctx->stage[0].as<double>(), ctx->stage[1].as<double>(), ctx->stage[2].as<double>(),
                       ctx->stage[3].as<double>(), n, cube);
-    if (rc != BH_OK) return rc;
+    ctx->assign_wait = nullptr;
+    if (rc != BH_OK) { cudaStreamSynchronize(cs); return rc; }
     rc = bh_potential(ctx, theta, G, ctx->stage_phi.as<double>());
+    if (rc != BH_OK) { cudaStreamSynchronize(cs); return rc; }
+    BH_CUDA(cudaEventRecord(ctx->ev[EV_HD1], st));
+    rc = d2h(ctx, phi, ctx->stage_phi.p, sizeof(double) * n, st);
     if (rc != BH_OK) return rc;
-    BH_CUDA(cudaMemcpyAsync(phi, ctx->stage_phi.p, sizeof(double) * n, cudaMemcpyDeviceToHost, ctx->stream));
-    BH_CUDA(cudaStreamSynchronize(ctx->stream));
+    BH_CUDA(cudaEventRecord(ctx->ev[EV_HEND], st));
+    BH_CUDA(cudaStreamSynchronize(st));
+    ctx->host_timed = true;
     return BH_OK;
+}
+
+int bh_host_breakdown(bh_ctx* ctx, float ms[4])
+{
+    if (!ctx || !ms) return BH_ERR_INVALID_ARG;
+    if (!ctx->host_timed) return BH_ERR_NOT_BUILT;
+    BH_CUDA(cudaSetDevice(ctx->device));
+    BH_CUDA(cudaEventElapsedTime(&ms[0], ctx->ev[EV_HC0], ctx->ev[EV_HM]));     // host -> device, all four arrays
+    BH_CUDA(cudaEventElapsedTime(&ms[1], ctx->ev[EV_HD0], ctx->ev[EV_HD1]));    // build + walk, from the arrival of x, y, z
+    BH_CUDA(cudaEventElapsedTime(&ms[2], ctx->ev[EV_HD1], ctx->ev[EV_HEND]));   // device -> host
+    BH_CUDA(cudaEventElapsedTime(&ms[3], ctx->ev[EV_H0], ctx->ev[EV_HEND]));    // whole call on the device
+    return BH_OK;
+}
+
+int bh_get_build_passes(bh_ctx* ctx, bh_pass* out, int cap, int* count)
+{
+    if (!ctx || !count || cap < 0 || (cap > 0 && !out)) return BH_ERR_INVALID_ARG;
+    if (!ctx->built) return BH_ERR_NOT_BUILT;
+    BH_CUDA(cudaSetDevice(ctx->device));
+    BH_CUDA(cudaStreamSynchronize(ctx->stream));
+    *count = ctx->npass;
+    for (int k = 0; k < ctx->npass && k < cap; ++k) {
+        memset(&out[k], 0, sizeof(out[k]));
+        snprintf(out[k].name, sizeof(out[k].name), "%s", ctx->pname[k]);
+        out[k].alg_bytes = ctx->pbytes[k];
+        cudaEventElapsedTime(&out[k].ms, k == 0 ? ctx->ev[EV_B0] : ctx->pev[k - 1], ctx->pev[k]);
+    }
+    cudaGetLastError();
+    return ctx->npass > cap ? BH_ERR_TOO_LARGE : BH_OK;
 }
 
 int bh_tree_sizes(const bh_ctx* ctx, int64_t* n, int64_t* n_nodes, int64_t* n_slots)
@@ -782,6 +936,24 @@ int bh_last_group_counts(bh_ctx* ctx, int64_t* counts)
     return BH_OK;
 }
 
+int bh_last_group_evaluated(bh_ctx* ctx, uint32_t* per_group)
+{
+    if (!ctx || !per_group) return BH_ERR_INVALID_ARG;
+    if (!ctx->walked) return BH_ERR_NOT_BUILT;
+    BH_CUDA(cudaSetDevice(ctx->device));
+    const i64 ng = (ctx->n + ctx->walk_group - 1) / ctx->walk_group;
+    group_eval_export_kernel<<<blocks_for(ng, 256), 256, 0, ctx->stream>>>(ctx->geval.as<u32>(), ng, per_group);
+    BH_CUDA(cudaGetLastError());
+    return BH_OK;
+}
+
+int bh_last_walk_group(const bh_ctx* ctx)
+{
+    if (!ctx) return BH_ERR_INVALID_ARG;
+    if (!ctx->walked) return BH_ERR_NOT_BUILT;
+    return ctx->walk_group;
+}
+
 int bh_last_interactions(bh_ctx* ctx, uint32_t* per_target)
 {
     if (!ctx || !per_target) return BH_ERR_INVALID_ARG;
@@ -806,8 +978,8 @@ int bh_get_stats(bh_ctx* ctx, bh_stats* out)
         { int rc = ensure_counts(ctx); if (rc != BH_OK) return rc; }
         const i64 ng = (ctx->n + ctx->walk_group - 1) / ctx->walk_group;
         BH_CUDA(cudaMemsetAsync(ds->totals, 0, sizeof(ds->totals), st));
-        group_counts_total_kernel<<<persistent_grid(ctx, 2), 256, 0, st>>>(ctx->gcount.as<uint4>(), ng, ctx->n,
-                                                                          ctx->walk_group, ds->totals);
+        group_counts_total_kernel<<<persistent_grid(ctx, 2), 256, 0, st>>>(ctx->gcount.as<uint4>(), ctx->geval.as<u32>(),
+                                                                          ng, ctx->n, ctx->walk_group, ds->totals);
         BH_CUDA(cudaGetLastError());
         BH_CUDA(cudaMemcpyAsync(ctx->h_scalars->totals, ds->totals, sizeof(ds->totals), cudaMemcpyDeviceToHost, st));
     }
@@ -826,7 +998,9 @@ int bh_get_stats(bh_ctx* ctx, bh_stats* out)
         out->n_leaf = (i64)ctx->h_scalars->totals[1];
         out->n_opened = (i64)ctx->h_scalars->totals[2];
         out->n_exact_tests = (i64)ctx->h_scalars->totals[3];
-        out->interactions = (double)ctx->h_scalars->totals[4];
+        out->interactions = (double)ctx->h_scalars->totals[5];          // counted by the Phi kernel itself
+        out->interactions_counted = (double)ctx->h_scalars->totals[4];  // counted by the count-only twin
+        out->walk_group = ctx->walk_group;
     }
     if (ctx->ev_build) {
         cudaEventElapsedTime(&out->ms_keys, ctx->ev[EV_B0], ctx->ev[EV_KEYS]);

@@ -298,8 +298,10 @@ inline size_t sort_smem_bytes(bool packed) { return sizeof(SortSmem) + (packed ?
 // between (k0, v0) and (k1, v1); pass p writes to buffer 1 if p is even, else to buffer 0, so the result
 // is in buffer (npasses & 1).  Packed plans never touch v0 / v1 (may be null).
 // scratch holds plan.npasses * sort_pass_words(n) u32.
+// `mark(name, algorithmic bytes)` is called after every launch (bh_build's optional per-pass timing).
+template <class Mark>
 inline cudaError_t radix_sort_pairs(u64* k0, u32* v0, u64* k1, u32* v1, i64 n, const SortPlan& plan, u32* scratch,
-                                    int hist_grid, cudaStream_t st)
+                                    int hist_grid, cudaStream_t st, Mark&& mark)
 {
     if (plan.npasses == 0) return cudaSuccess;
     const size_t pw = sort_pass_words(n);
@@ -308,6 +310,7 @@ inline cudaError_t radix_sort_pairs(u64* k0, u32* v0, u64* k1, u32* v1, i64 n, c
     if (e != cudaSuccess) return e;
     // all histograms in one read; each pass's 256 counters sit at the head of its scratch block
     radix_hist_strided_kernel<<<hist_grid, kSortThreads, 0, st>>>(k0, n, plan, scratch, (u32)pw);
+    mark("sort_hist", 8.0 * (double)n);
     const size_t smem = sort_smem_bytes(plan.packed);
     for (int p = 0; p < plan.npasses; ++p) {
         u32* blk = scratch + pw * p;
@@ -328,6 +331,7 @@ inline cudaError_t radix_sort_pairs(u64* k0, u32* v0, u64* k1, u32* v1, i64 n, c
                 radix_onesweep_kernel<kGeneric><<<ntiles, kSortThreads, smem, st>>>(
                     k0, v0, k1, v1, blk, status, ticket, n, plan.shift[p], plan.mask[p], plan.lo);
         }
+        mark("sort_pass", 24.0 * (double)n);          // 12 B read + 12 B written per pair and pass
         u64* tk = k0; k0 = k1; k1 = tk;
         u32* tv = v0; v0 = v1; v1 = tv;
     }

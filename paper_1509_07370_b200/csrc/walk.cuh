@@ -53,6 +53,7 @@ struct WalkParams {
     double* phi;              // [n] original order
     double* acc;              // bh_field only: [3n] (gx, gy, gz) per cell, original order
     uint4* gcount;            // [ngroups] {accepted, leaf, opened, exact-tested}
+    u32* geval;               // [ngroups] list entries the Phi kernel itself evaluated for the group
     i64 n;
     i64 ngroups;
     float inv_theta;          // (float)(1/theta); +inf for theta = 0
@@ -140,12 +141,13 @@ __device__ __forceinline__ void eval_soa2(const float* __restrict__ L, int cnt, 
 // ---- C: leaf cells inside a group's bounding box; zero-distance pairs are skipped (W3) ----------
 __device__ __forceinline__ void eval_c(const float4* __restrict__ L, const u32* __restrict__ Lm, int cnt,
                                        const float2 npx, const float2 npy, const float2 npz, double& accA,
-                                       double& accB)
+                                       double& accB, u32& evA, u32& evB)
 {
     float2 s = splat2(0.f);
     for (int e = 0; e < cnt; ++e) {
         const float4 v = L[e];
         const u32 mk = Lm[e];
+        evA += mk & 1u; evB += mk >> 1;               // every lane sees every entry: warp-uniform
         const float2 dx = __fadd2_rn(splat2(v.x), npx);
         const float2 dy = __fadd2_rn(splat2(v.y), npy);
         const float2 dz = __fadd2_rn(splat2(v.z), npz);
@@ -240,12 +242,13 @@ __device__ __forceinline__ void eval_soa2_g(const float* __restrict__ L, int cnt
 
 __device__ __forceinline__ void eval_c_g(const float4* __restrict__ L, const u32* __restrict__ Lm, int cnt,
                                          const float2 npx, const float2 npy, const float2 npz, double& accA,
-                                         double& accB, double* gA, double* gB)
+                                         double& accB, double* gA, double* gB, u32& evA, u32& evB)
 {
     float2 s = splat2(0.f), gx = splat2(0.f), gy = splat2(0.f), gz = splat2(0.f);
     for (int e = 0; e < cnt; ++e) {
         const float4 v = L[e];
         const u32 mk = Lm[e];
+        evA += mk & 1u; evB += mk >> 1;
         const float2 dx = __fadd2_rn(splat2(v.x), npx);
         const float2 dy = __fadd2_rn(splat2(v.y), npy);
         const float2 dz = __fadd2_rn(splat2(v.z), npz);
@@ -350,9 +353,14 @@ walk_pair_kernel(const WalkParams P)
         // of the sorted order: a pair of groups without a single target has nothing to compute
         const bool want = (liveA && sv_idx(P.sv, sA) < P.ntargets) || (liveB && sv_idx(P.sv, sB) < P.ntargets);
         if (!__any_sync(0xffffffffu, want)) {
-            if (COUNT && lane == 0) {
-                P.gcount[gA] = make_uint4(0u, 0u, 0u, 0u);
-                if (hasB) P.gcount[gB] = make_uint4(0u, 0u, 0u, 0u);
+            if (lane == 0) {
+                if (COUNT) {
+                    P.gcount[gA] = make_uint4(0u, 0u, 0u, 0u);
+                    if (hasB) P.gcount[gB] = make_uint4(0u, 0u, 0u, 0u);
+                } else {
+                    P.geval[gA] = 0u;
+                    if (hasB) P.geval[gB] = 0u;
+                }
             }
             return;
         }
@@ -371,6 +379,7 @@ walk_pair_kernel(const WalkParams P)
     double accA = 0.0, accB = 0.0;
     double grA[3] = {0.0, 0.0, 0.0}, grB[3] = {0.0, 0.0, 0.0};   // ACC: sums of w (r_j - r_t)
     int nU2 = 0, nUA = 0, nUB = 0, nC = 0;          // list fill (warp-uniform)
+    u32 evA = 0, evB = 0;                           // list entries evaluated so far for A / B (unpadded, warp-uniform)
     u32 cAccA = 0, cLeafA = 0, cOpenA = 0, cExA = 0;  // COUNT: per-lane partial counters
     u32 cAccB = 0, cLeafB = 0, cOpenB = 0, cExB = 0;
     int sp = 0;
@@ -488,23 +497,26 @@ walk_pair_kernel(const WalkParams P)
                 __syncwarp();
                 if (ACC) eval_soa2_g<kU2Cap>(U2, nU2, TA, TB, accA, accB, grA, grB);
                 else eval_soa2<kU2Cap>(U2, nU2, TA, TB, accA, accB);
+                evA += (u32)nU2; evB += (u32)nU2;
                 nU2 = 0;
             }
             if (nUA >= kU1Cap - kStepMax) {
                 soa_pad<kU1Cap>(UA, nUA);
                 __syncwarp();
                 accA += ACC ? eval_soa_g<kU1Cap>(UA, nUA, TA, grA) : eval_soa<kU1Cap>(UA, nUA, TA);
+                evA += (u32)nUA;
                 nUA = 0;
             }
             if (nUB >= kU1Cap - kStepMax) {
                 soa_pad<kU1Cap>(UB, nUB);
                 __syncwarp();
                 accB += ACC ? eval_soa_g<kU1Cap>(UB, nUB, TB, grB) : eval_soa<kU1Cap>(UB, nUB, TB);
+                evB += (u32)nUB;
                 nUB = 0;
             }
             if (nC >= kCCap - kStepMax) {
-                if (ACC) eval_c_g(C, Cm, nC, npx, npy, npz, accA, accB, grA, grB);
-                else eval_c(C, Cm, nC, npx, npy, npz, accA, accB);
+                if (ACC) eval_c_g(C, Cm, nC, npx, npy, npz, accA, accB, grA, grB, evA, evB);
+                else eval_c(C, Cm, nC, npx, npy, npz, accA, accB, evA, evB);
                 nC = 0;
             }
             __syncwarp();
@@ -538,8 +550,13 @@ walk_pair_kernel(const WalkParams P)
         accB += ACC ? eval_soa_g<kU1Cap>(UB, nUB, TB, grB) : eval_soa<kU1Cap>(UB, nUB, TB);
     }
     if (nC > 0) {
-        if (ACC) eval_c_g(C, Cm, nC, npx, npy, npz, accA, accB, grA, grB);
-        else eval_c(C, Cm, nC, npx, npy, npz, accA, accB);
+        if (ACC) eval_c_g(C, Cm, nC, npx, npy, npz, accA, accB, grA, grB, evA, evB);
+        else eval_c(C, Cm, nC, npx, npy, npz, accA, accB, evA, evB);
+    }
+    // the kernel answers for its own lists: entries it evaluated for each group (= accepted + leaf of W6)
+    if (lane == 0) {
+        P.geval[gA] = evA + (u32)(nU2 + nUA);
+        if (hasB) P.geval[gB] = evB + (u32)(nU2 + nUB);
     }
     // ---- a7: Phi_t = -G * sum, written in the original cell order (W-rule 4) ----
     // bh_field: g_t = -grad Phi_t = G * sum w (r_j - r_t)
@@ -570,7 +587,7 @@ walk_single_kernel(const WalkParams P)
 {
     const i64 s = (i64)blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= P.n) return;
-    if (sv_idx(P.sv, s) >= P.ntargets) { P.gcount[s] = make_uint4(0u, 0u, 0u, 0u); return; }
+    if (sv_idx(P.sv, s) >= P.ntargets) { P.gcount[s] = make_uint4(0u, 0u, 0u, 0u); P.geval[s] = 0u; return; }
     const float4 tp = __ldg(P.rec + __ldg(P.leaf_slot + s));
     u32 st_first[kSingleStack], st_count[kSingleStack];
     int sp = 0;
@@ -620,10 +637,19 @@ walk_single_kernel(const WalkParams P)
     }
     acc += (double)part;
     const u32 o = sv_idx(P.sv, s);
-    P.phi[o] = P.negG * acc;
+    if (P.phi) P.phi[o] = P.negG * acc;
     if (P.acc)
         for (int k = 0; k < 3; ++k) P.acc[3 * (size_t)o + k] = -P.negG * (g[k] + (double)gp[k]);
     P.gcount[s] = make_uint4(c_acc, c_leaf, c_open, 0u);
+    P.geval[s] = c_acc + c_leaf;
+}
+
+// the Phi kernel's own per-group entry counts as plain u32 (bh_last_group_evaluated)
+__global__ void __launch_bounds__(256)
+group_eval_export_kernel(const u32* __restrict__ geval, i64 ngroups, u32* __restrict__ out)
+{
+    const i64 g = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g < ngroups) out[g] = geval[g];
 }
 
 // per-target interaction counts / int64 group counts from the uint4 group counters
@@ -646,20 +672,22 @@ per_target_counts_kernel(const uint4* __restrict__ gcount, const SortedView sv, 
     out[sv_idx(sv, s)] = c.x + c.y;
 }
 
-// totals[0..3] = sum of the four group counters; totals[4] = sum over targets of (acc + leaf)
+// totals[0..3] = sum of the four group counters of the count-only twin; totals[4] = sum over targets of their
+// (acc + leaf); totals[5] = the same sum taken from the Phi kernel's own per-group entry counts (geval)
 __global__ void __launch_bounds__(256)
-group_counts_total_kernel(const uint4* __restrict__ gcount, i64 ngroups, i64 n, int group,
-                          unsigned long long* __restrict__ totals)
+group_counts_total_kernel(const uint4* __restrict__ gcount, const u32* __restrict__ geval, i64 ngroups, i64 n,
+                          int group, unsigned long long* __restrict__ totals)
 {
-    unsigned long long t[5] = {0, 0, 0, 0, 0};
+    unsigned long long t[6] = {0, 0, 0, 0, 0, 0};
     for (i64 g = (i64)blockIdx.x * blockDim.x + threadIdx.x; g < ngroups; g += (i64)gridDim.x * blockDim.x) {
         const uint4 c = gcount[g];
         const i64 members = min((i64)group, n - g * group);
         t[0] += c.x; t[1] += c.y; t[2] += c.z; t[3] += c.w;
         t[4] += (unsigned long long)(c.x + c.y) * (unsigned long long)members;
+        t[5] += (unsigned long long)geval[g] * (unsigned long long)members;
     }
     #pragma unroll
-    for (int k = 0; k < 5; ++k) {
+    for (int k = 0; k < 6; ++k) {
         #pragma unroll
         for (int o = 16; o > 0; o >>= 1) t[k] += __shfl_xor_sync(0xffffffffu, t[k], o);
         if (lane_id() == 0 && t[k]) atomicAdd(&totals[k], t[k]);

@@ -28,15 +28,24 @@ def domain_box(x, y, z):
     return lo, hi
 
 
-def gather_boxes(box, group=None):
+def _comm_device(group, data_device):
+    """Where the tensors handed to torch.distributed must live: NCCL moves device buffers (the records go from
+    device buffer to device buffer over NVLink); any other backend (gloo: the CPU tests, and GPU data exchanged
+    between processes that have no NCCL group) is served through host tensors."""
+    import torch
+    import torch.distributed as dist
+    if dist.get_backend(group) == "nccl":
+        return data_device if data_device.type == "cuda" else torch.device("cuda", torch.cuda.current_device())
+    return torch.device("cpu")
+
+
+def gather_boxes(box, group=None, device=None):
     """Step 2: every rank's (lo, hi); ranks without cells send an inverted box and are skipped by senders."""
     import torch
     import torch.distributed as dist
     world = dist.get_world_size(group)
-    mine = torch.tensor(list(box[0]) + list(box[1]), dtype=torch.float64)
-    backend = dist.get_backend(group)
-    if backend == "nccl":
-        mine = mine.cuda()
+    cdev = _comm_device(group, device if device is not None else torch.device("cpu"))
+    mine = torch.tensor(list(box[0]) + list(box[1]), dtype=torch.float64, device=cdev)
     out = [torch.empty_like(mine) for _ in range(world)]
     dist.all_gather(out, mine, group=group)
     return [(tuple(t[:3].tolist()), tuple(t[3:].tolist())) for t in out]
@@ -49,24 +58,25 @@ def exchange_records(send: Sequence, group=None):
     import torch
     import torch.distributed as dist
     world, rank = dist.get_world_size(group), dist.get_rank(group)
-    dev = send[(rank + 1) % world].device if world > 1 else send[0].device
-    counts = torch.tensor([0 if r == rank else int(send[r].shape[0]) for r in range(world)], dtype=torch.int64, device=dev)
+    dev = send[(rank + 1) % world].device if world > 1 else send[0].device      # where the records live
+    cdev = _comm_device(group, dev)                                               # where the backend wants them
+    counts = torch.tensor([0 if r == rank else int(send[r].shape[0]) for r in range(world)], dtype=torch.int64, device=cdev)
     allc = [torch.empty_like(counts) for _ in range(world)]
     dist.all_gather(allc, counts, group=group)
     allc = torch.stack(allc).cpu()                                   # allc[s, r] = entries s sends to r
-    recv = [torch.empty((int(allc[s, rank]), 4), dtype=torch.float64, device=dev) for s in range(world)]
+    recv = [torch.empty((int(allc[s, rank]), 4), dtype=torch.float64, device=cdev) for s in range(world)]
     ops = []
     for r in range(world):
         if r == rank:
             continue
         if send[r].shape[0] > 0:
-            ops.append(dist.P2POp(dist.isend, send[r].contiguous(), r, group))
+            ops.append(dist.P2POp(dist.isend, send[r].contiguous().to(cdev), r, group))   # no copy when cdev == dev
         if recv[r].shape[0] > 0:
             ops.append(dist.P2POp(dist.irecv, recv[r], r, group))
     if ops:
         for w in dist.batch_isend_irecv(ops):
             w.wait()
-    return recv
+    return [t.to(dev) for t in recv]
 
 
 def let_potential(x, y, z, m, cube, theta: float, G: float = 1.0, group=None, mac: int = 1,
@@ -106,7 +116,7 @@ def let_potential(x, y, z, m, cube, theta: float, G: float = 1.0, group=None, ma
     info = {"rank": rank, "world": world, "n_own": n_own, "sent": [0] * world, "received": [0] * world}
     if world == 1:
         return solve(x, y, z, m, cube, n_own, theta, G, mac), info
-    boxes = gather_boxes(domain_box(x, y, z) if n_own else ((1.0, 1.0, 1.0), (0.0, 0.0, 0.0)), group)
+    boxes = gather_boxes(domain_box(x, y, z) if n_own else ((1.0, 1.0, 1.0), (0.0, 0.0, 0.0)), group, x.device)
     want = [None if (r == rank or boxes[r][0][0] > boxes[r][1][0]) else boxes[r] for r in range(world)]
     if n_own:
         send = select(x, y, z, m, cube, want, theta, mac)

@@ -33,8 +33,10 @@ def test_strerror_and_stats_layout():
     L = pkg.lib()
     assert L.bh_strerror(0) == b"ok"
     assert b"invalid" in L.bh_strerror(-1)
-    # struct bh_stats: 3*8 + 2*4 + 6*8 + 8 + 7*4 + 2*4 (+4 pad) bytes
-    assert C.sizeof(pkg.Stats) == 128
+    # struct bh_stats: 3*8 + 2*4 + 6*8 + 8 + 7*4 + 3*4 + 8 bytes; struct bh_pass: 24 + 4 (+4 pad) + 8
+    assert C.sizeof(pkg.Stats) == 136
+    from paper_1509_07370_b200.binding import Pass
+    assert C.sizeof(Pass) == 40
 
 
 def test_no_cpu_fallback_without_device():

@@ -11,7 +11,7 @@ import numpy as np
 import pytest
 
 import bh_workloads as wl
-from tests import analytic
+from tests import analytic, parity
 
 pytestmark = pytest.mark.gpu
 
@@ -36,36 +36,12 @@ def _build(bh, w):
     return ctx
 
 
-def _sample_runs(ngroups, nruns, per):
-    """`nruns` evenly spaced runs of `per` consecutive groups, first and last group included."""
-    per = min(per, ngroups)
-    starts = np.unique(np.linspace(0, ngroups - per, nruns).astype(np.int64))
-    return [(int(s), int(s) + per) for s in starts]
-
-
-def _check_sampled(ctx, ot, w, theta, mac=0, nruns=12, per=24, max_tol=1e-4, med_tol=1e-6):
-    """Phi and the (accepted, leaf, opened) counters of sampled groups against the oracle."""
-    ctx.set_mac(mac)
-    phi = ctx.potential(theta, w.G).cpu().numpy()
-    cnt = ctx.last_group_counts().cpu().numpy()
-    perm = ot.sorted_keys_perm()[1].astype(np.int64)
+def _check_sampled(ctx, ot, w, theta, mac=0, nruns=12, per=24):
+    """Phi and the per-group counters of sampled runs of groups under the protocol of tests/parity.py (fp64
+    oracle with flips counted and reported; fp32-decision oracle flip-free)."""
     ngroups = (w.n + 31) // 32
-    rels, flips, ngr = [], 0, 0
-    buf = np.full(w.n, np.nan)
-    for g0, g1 in _sample_runs(ngroups, nruns, per):
-        _, ocnt = ot.potential(theta, w.G, mac=mac, group=32, mac_fp32=True, groups=(g0, g1), want_counts=True,
-                               out=buf)
-        flips += int(np.sum(np.any(cnt[g0:g1] != ocnt, axis=1)))
-        ngr += g1 - g0
-        tg = perm[32 * g0:min(32 * g1, w.n)]
-        ref = buf[tg]
-        ok = ref != 0
-        rels.append(np.abs(phi[tg][ok] - ref[ok]) / np.abs(ref[ok]))
-    rel = np.concatenate(rels)
-    assert flips == 0, f"{flips} of {ngr} sampled groups differ in (accepted, leaf, opened)"
-    assert rel.max() <= max_tol, f"max rel {rel.max():.3e}"
-    assert np.median(rel) <= med_tol, f"median rel {np.median(rel):.3e}"
-    return phi, cnt
+    rep = parity.check_walk(ctx, ot, w, theta, mac=mac, runs=parity.sample_runs(ngroups, nruns, per))
+    return rep["phi"], rep["counts"]
 
 
 def _check_essential(ctx, ot, w, theta=0.5):
@@ -122,7 +98,7 @@ def test_config1_maclaurin(bh, oracle):
     ctx = _build(bh, w)
     ot = oracle.OracleTree(w.x, w.y, w.z, w.m, w.cube)
     _check_tree(ctx, ot, w)
-    phi, _ = _check_sampled(ctx, ot, w, 0.5)
+    phi, _ = _check_sampled(ctx, ot, w, 0.5, nruns=32, per=32)
     a1, e = 0.4, 0.9
     a3 = a1 * np.sqrt(1 - e * e)
     X, Y, Z = w.x - 0.5, w.y - 0.5, w.z - 0.5
@@ -148,7 +124,7 @@ def test_config2_amr_core_and_config4_theta_sweep(bh, oracle):
     assert np.max(np.abs(direct[sub] - ref) / np.abs(ref)) <= 1e-12
     errs, inter = [], []
     for theta in (0.3, 0.5, 0.7, 1.0):
-        phi, cnt = _check_sampled(ctx, ot, w, theta, nruns=6, per=8)
+        phi, cnt = _check_sampled(ctx, ot, w, theta, nruns=32, per=32)      # 1024 of ~122 k groups per theta
         errs.append(np.max(np.abs(phi[tg] - direct) / np.abs(direct)))
         inter.append(ctx.get_stats().interactions / w.n)
     assert all(a < b for a, b in zip(errs, errs[1:])), errs               # error grows with theta
@@ -165,8 +141,8 @@ def test_config3_turb256_bench_configuration(bh, oracle):
     st = ctx.get_stats()
     assert st.n_nodes == (w.n - 1) // 7 and st.depth == 7 and st.sort_passes == 3
     _check_essential(ctx, ot, w)
-    _check_sampled(ctx, ot, w, 0.5, nruns=16, per=16)
-    _check_sampled(ctx, ot, w, 0.5, mac=1, nruns=4, per=8)
+    _check_sampled(ctx, ot, w, 0.5, nruns=64, per=64)           # 4096 of 524,288 groups, like bench.py's parity key
+    _check_sampled(ctx, ot, w, 0.5, mac=1, nruns=16, per=16)
     # properties that hold at any size: every potential is finite and negative (all masses are positive)
     phi = ctx.potential(0.5, w.G).cpu().numpy()
     assert np.all(np.isfinite(phi)) and np.all(phi < 0)

@@ -147,6 +147,99 @@ def test_mac_fp32_decisions_match_on_dyadic_grid(oracle):
     assert (c64 != c32).any(axis=1).mean() < 0.05  # flips are rare
 
 
+# ---- pin of the oracle's mac_fp32 branch (W8) against tests/fp32_decision.py --------------------
+@pytest.mark.parametrize("w", [W.random_points(1500, seed=41), W.clustered_points(1200, seed=42, ),
+                               W.with_duplicates(W.random_points(300, seed=43), 25, near=2e-3)], ids=lambda w: w.name)
+@pytest.mark.parametrize("theta,mac,group", [(0.7, 0, 32), (0.3, 1, 32), (0.45, 1, 1), (0.9, 0, 32)])
+def test_mac_fp32_branch_equals_numpy_float32_restatement(oracle, w, theta, mac, group):
+    """Non-dyadic inputs, 1/theta inexact in fp32: the per-group (accepted, leaf, opened) counters of the oracle's
+    fp32-decision mode equal those of an independent numpy-float32 walk written from reading W8."""
+    from tests import fp32_decision as F
+    if group == 1 and w.n > 400:
+        w = W.Workload(w.name + "_head", w.x[:400], w.y[:400], w.z[:400], w.m[:400], cube=w.cube)
+    t = oracle.OracleTree(w.x, w.y, w.z, w.m, w.cube)
+    _, perm = t.sorted_keys_perm()
+    _, c32 = t.potential(theta, mac=mac, group=group, mac_fp32=True, want_counts=True)
+    ref = F.walk_counts_fp32(w.x[perm], w.y[perm], w.z[perm], t.nodes(), float(w.cube[3]), theta, mac, group)
+    assert np.array_equal(c32, ref)
+
+
+def _threshold_scan(oracle, theta, mac, yz, accept_fn, level=2, steps=160):
+    """A tight pair (a chain of nodes with one centre of mass R) and a lone target whose x runs through
+    consecutive fp32 values across the distance at which the level-`level` node of the chain switches from
+    opened to accepted.  Returns (oracle decisions, decisions of `accept_fn`) per step, True = accepted."""
+    px = np.array([0.13, 0.17]); py = np.array([0.11, 0.12]); pz = np.array([0.09, 0.10]); pm = np.array([1.0, 2.3])
+    R = np.array([(px * pm).sum(), (py * pm).sum(), (pz * pm).sum()]) / pm.sum()
+    size = 2.0 ** -level
+    rc = size / theta + (np.linalg.norm(R - (np.floor(R / size) + 0.5) * size) if mac == 1 else 0.0)
+    ty, tz = yz
+    x0 = np.float32(R[0] + np.sqrt(rc * rc - (ty - R[1]) ** 2 - (tz - R[2]) ** 2))
+    xs = [x0]
+    for _ in range(steps // 2):
+        xs.insert(0, np.nextafter(xs[0], np.float32(-1))); xs.append(np.nextafter(xs[-1], np.float32(2)))
+    got, ref = [], []
+    for xt in xs:
+        x = np.append(px, float(xt)); y = np.append(py, ty); z = np.append(pz, tz); m = np.append(pm, 0.7)
+        t = oracle.OracleTree(x, y, z, m, [0, 0, 0, 1.0])
+        _, perm = t.sorted_keys_perm()
+        s = int(np.where(perm == 2)[0][0])
+        _, c = t.potential(theta, mac=mac, group=1, mac_fp32=True, want_counts=True)
+        nd = t.nodes()
+        k = int(np.where(nd["level"] == level)[0][0])
+        # root .. level-1 are opened for this target (d < their r_c); the chain node at `level` decides
+        assert c[s, 2] in (level, level + 1) and c[s, 0] == 1
+        got.append(c[s, 2] == level)
+        ref.append(accept_fn(np.float32(xt), np.float32(ty), np.float32(tz), (nd["Rx"][k], nd["Ry"][k], nd["Rz"][k]),
+                             size, nd["delta"][k], theta, mac))
+    return np.array(got), np.array(ref)
+
+
+def test_mac_fp32_branch_at_the_threshold(oracle):
+    """One-ulp steps of a target across r_c: the oracle's fp32 decision equals the restatement at EVERY step, and
+    the plausible mistakes -- l/theta instead of l*(1/theta), the fma chain nested the other way round, unfused
+    multiply-adds, the decision taken in fp64 -- each disagree with the oracle at some step, so this pin would
+    catch them."""
+    from tests import fp32_decision as F
+    f32 = np.float32
+
+    def w8(tx, ty, tz, R, size, delta, theta, mac):
+        return F.group_accepts_fp32([tx], [ty], [tz], R, size, delta, theta, mac)
+
+    def div_theta(tx, ty, tz, R, size, delta, theta, mac):
+        rc = f32(f32(size) / f32(theta))
+        rc = f32(rc + f32(delta)) if mac == 1 else rc
+        return bool(F.d2_fp32([tx], [ty], [tz], R)[0] > f32(rc * rc))
+
+    def nest_x_last(tx, ty, tz, R, size, delta, theta, mac):
+        dx, dy, dz = (f32(f32(a) - f32(b)) for a, b in zip((tx, ty, tz), R))
+        d2 = F.fma32(dx, dx, F.fma32(dy, dy, f32(dz * dz)))
+        return bool(d2 > F.rc2_fp32(size, delta, theta, mac))
+
+    def unfused(tx, ty, tz, R, size, delta, theta, mac):
+        dx, dy, dz = (f32(f32(a) - f32(b)) for a, b in zip((tx, ty, tz), R))
+        d2 = f32(f32(f32(dx * dx) + f32(dy * dy)) + f32(dz * dz))
+        return bool(d2 > F.rc2_fp32(size, delta, theta, mac))
+
+    def in_fp64(tx, ty, tz, R, size, delta, theta, mac):
+        rc = size / theta + (delta if mac == 1 else 0.0)
+        d2 = sum((float(a) - float(b)) ** 2 for a, b in zip((tx, ty, tz), R))
+        return d2 > rc * rc
+
+    variants = {"div_theta": div_theta, "nest_x_last": nest_x_last, "unfused": unfused, "in_fp64": in_fp64}
+    caught = {k: 0 for k in variants}
+    for theta, mac, yz in ((0.7, 0, (0.3141, 0.2718)), (0.3, 1, (0.4567, 0.3789)), (0.9, 1, (0.2222, 0.3333)),
+                           (0.55, 0, (0.19, 0.41)), (0.35, 0, (0.6180339, 0.5772156)), (0.77, 1, (0.33, 0.07)),
+                           (0.62, 0, (0.2468, 0.1357)), (0.41, 1, (0.52, 0.23)), (0.83, 0, (0.05, 0.31)),
+                           (0.48, 0, (0.3775, 0.4425)), (0.66, 1, (0.1414, 0.1732)), (0.37, 1, (0.29, 0.61))):
+        got, ref = _threshold_scan(oracle, theta, mac, yz, w8)
+        assert got[0] != got[-1]                               # the scan does cross the threshold
+        assert np.array_equal(got, ref), (theta, mac)
+        for name, fn in variants.items():
+            _, alt = _threshold_scan(oracle, theta, mac, yz, fn)
+            caught[name] += int(np.sum(alt != got))
+    assert all(v > 0 for v in caught.values()), caught
+
+
 def test_uniform_sphere_closed_form(oracle):
     # configs[0] at 32^3: direct sum vs -2 pi G rho (R^2 - r^2/3) inside, -GM/r outside
     w = W.uniform_sphere(32)
