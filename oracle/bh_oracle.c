@@ -619,3 +619,214 @@ int orc_direct_acc(const double *x, const double *y, const double *z, const doub
     }
     return 0;
 }
+
+/* ==== periodic boundaries (Appendix A) =====================
+ * "In case of periodic boundary conditions, a node's or data cell's contribution to the gravitational
+ * potential of a data cell changes to phi = G M f_EF(r)" (Eq. A.1), f_EF the Ewald field:
+ * Eq. A.2 splits 1/r = erf(alpha r)/r + erfc(alpha r)/r and Eq. A.3 sums a short-range part A_S over the
+ * periodic images and a long-range part A_L obtained with the Poisson summation formula.  The paper prints
+ * neither A_S nor A_L nor alpha; reading (P1), the standard Ewald sum of 1/r in a cubic box of
+ * edge L with a neutralising uniform background, in box units u = r/L, a = alpha L:
+ *   psi1(u) = sum_n erfc(a |u - n|)/|u - n|                               (A_S, images n in Z^3)
+ *           + (1/pi) sum_{h != 0} exp(-pi^2 |h|^2 / a^2)/|h|^2 cos(2 pi h.u) (A_L, wave vectors h in Z^3)
+ *           - pi / a^2                                                      (background: zero mean over the box)
+ * f_EF(r) = psi1(r/L)/L, and a source of mass M at displacement r contributes -G M f_EF(r) to Phi (sign as in
+ * reading R1).  Both index ranges are the cube |n_i|, |h_i| <= nser ("gpuEwaldSeriesN ... controls the range
+ * of the indices i1, i2, i3").  psi1 does not depend on a once the sums have converged. */
+double orc_ewald_psi(const double *u, double a, int nser)
+{
+    const double pi = 3.14159265358979323846;
+    double s = 0.0;
+    for (int i = -nser; i <= nser; ++i)
+        for (int j = -nser; j <= nser; ++j)
+            for (int k = -nser; k <= nser; ++k) {
+                double dx = u[0] - i, dy = u[1] - j, dz = u[2] - k;
+                double d = sqrt(dx * dx + dy * dy + dz * dz);
+                s += erfc(a * d) / d;                                        /* A_S */
+                int h2 = i * i + j * j + k * k;
+                if (h2 > 0)                                                  /* A_L */
+                    s += exp(-pi * pi * h2 / (a * a)) / (pi * h2) * cos(2.0 * pi * (i * u[0] + j * u[1] + k * u[2]));
+            }
+    return s - pi / (a * a);
+}
+
+/* The smooth part that is tabulated: corr1(u) = psi1(u) - 1/|u| for u inside the box, and its limit at
+ * u = 0 (erfc(a d)/d - 1/d -> -2a/sqrt(pi)).  The singular 1/|u| is the isolated-boundary term the walk
+ * evaluates directly; reading P2: the field array holds f_EF with that term taken out. */
+double orc_ewald_corr(const double *u, double a, int nser)
+{
+    const double pi = 3.14159265358979323846;
+    double d0 = sqrt(u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);
+    if (d0 > 0.0) return orc_ewald_psi(u, a, nser) - 1.0 / d0;
+    double s = 0.0;
+    for (int i = -nser; i <= nser; ++i)
+        for (int j = -nser; j <= nser; ++j)
+            for (int k = -nser; k <= nser; ++k) {
+                int h2 = i * i + j * j + k * k;
+                if (h2 == 0) continue;
+                double d = sqrt((double)h2);
+                s += erfc(a * d) / d + exp(-pi * pi * h2 / (a * a)) / (pi * h2);
+            }
+    return s - pi / (a * a) - 2.0 * a / sqrt(pi);
+}
+
+/* "The Ewald field is calculated once on startup and stored in a large array representing a hierarchy of
+ * nested grids".  Reading P3: corr1 is even in every coordinate, so the array covers the
+ * octant u_a >= 0; grid `lev` (0 .. nref-1, "gpuEwaldSeriesNref ... the number of nested grids") has N
+ * points per axis ("gpuEwaldFieldNx/y/z"; one N here, the box is a cube) at u = i * h_lev,
+ * h_lev = (1/2) / (N - 1) / 2^lev, i.e. it spans [0, 1/2^(lev+1)] per axis: every grid refines the corner
+ * of the previous one around u = 0.  table[((lev * N + k) * N + j) * N + i] = corr1(i h, j h, k h). */
+int orc_ewald_table(int N, int nref, double a, int nser, double *table)
+{
+    if (N < 4 || nref < 1 || !(a > 0.0) || nser < 1 || !table) return -1;
+    for (int lev = 0; lev < nref; ++lev) {
+        double h = 0.5 / (N - 1) / (double)(1 << lev);
+        double *t = table + (size_t)lev * N * N * N;
+        for (int k = 0; k < N; ++k)
+            for (int j = 0; j <= k; ++j)
+                for (int i = 0; i <= j; ++i) { /* corr1 is symmetric under permutations of the axes */
+                    double u[3] = {i * h, j * h, k * h};
+                    double v = orc_ewald_corr(u, a, nser);
+                    int p[3] = {i, j, k};
+                    static const int perm[6][3] = {{0, 1, 2}, {0, 2, 1}, {1, 0, 2}, {1, 2, 0}, {2, 0, 1}, {2, 1, 0}};
+                    for (int q = 0; q < 6; ++q)
+                        t[((size_t)p[perm[q][2]] * N + p[perm[q][1]]) * N + p[perm[q][0]]] = v;
+                }
+    }
+    return 0;
+}
+
+/* "... carried out during the respective tree walk using quadratic interpolation".
+ * Reading P4 (the stencil is not given): on the finest grid that holds the point with its stencil, take the
+ * NEAREST grid point i0 per axis and the quadratic through the 3 points per axis around it,
+ *   corr(u) ~ C0 + sum_a Da d_a + 1/2 sum_a Daa d_a^2 + sum_{a<b} Dab d_a d_b,   d_a = |u_a|/h - i0_a in [-1/2, 1/2],
+ *   Da = (C[+a] - C[-a])/2,  Daa = C[+a] - 2 C0 + C[-a],  Dab = (C[+a+b] - C[+a-b] - C[-a+b] + C[-a-b])/4.
+ * Index -1 mirrors to +1 (corr1 is even); on grid 0, index N mirrors to N - 2 (corr1(1/2 + t) = corr1(1/2 - t):
+ * periodic and even).  u must be a minimum-image displacement in box units, |u_a| <= 1/2. */
+static double tab_at(const double *t, int N, int i, int j, int k)
+{
+    int v[3] = {i, j, k};
+    for (int c = 0; c < 3; ++c) {
+        if (v[c] < 0) v[c] = -v[c];
+        if (v[c] >= N) v[c] = 2 * (N - 1) - v[c];
+    }
+    i = v[0]; j = v[1]; k = v[2];
+    return t[((size_t)k * N + j) * N + i];
+}
+
+double orc_ewald_interp(const double *table, int N, int nref, const double *u)
+{
+    double ax = fabs(u[0]), ay = fabs(u[1]), az = fabs(u[2]);
+    double mx = ax > ay ? (ax > az ? ax : az) : (ay > az ? ay : az);
+    int lev = 0; /* finest grid whose interior (nearest point <= N - 2) holds the point */
+    for (int l = nref - 1; l > 0; --l) {
+        double h = 0.5 / (N - 1) / (double)(1 << l);
+        if (mx <= (N - 2) * h) { lev = l; break; }
+    }
+    double h = 0.5 / (N - 1) / (double)(1 << lev);
+    const double *t = table + (size_t)lev * N * N * N;
+    double p[3] = {ax / h, ay / h, az / h};
+    int i0[3]; double d[3];
+    for (int c = 0; c < 3; ++c) {
+        i0[c] = (int)floor(p[c] + 0.5);
+        if (i0[c] > N - 1) i0[c] = N - 1;
+        d[c] = p[c] - i0[c];
+    }
+    int i = i0[0], j = i0[1], k = i0[2];
+    double C0 = tab_at(t, N, i, j, k);
+    double xp = tab_at(t, N, i + 1, j, k), xm = tab_at(t, N, i - 1, j, k);
+    double yp = tab_at(t, N, i, j + 1, k), ym = tab_at(t, N, i, j - 1, k);
+    double zp = tab_at(t, N, i, j, k + 1), zm = tab_at(t, N, i, j, k - 1);
+    double Dx = 0.5 * (xp - xm), Dy = 0.5 * (yp - ym), Dz = 0.5 * (zp - zm);
+    double Dxx = xp - 2.0 * C0 + xm, Dyy = yp - 2.0 * C0 + ym, Dzz = zp - 2.0 * C0 + zm;
+    double Dxy = 0.25 * (tab_at(t, N, i + 1, j + 1, k) - tab_at(t, N, i + 1, j - 1, k) - tab_at(t, N, i - 1, j + 1, k) + tab_at(t, N, i - 1, j - 1, k));
+    double Dxz = 0.25 * (tab_at(t, N, i + 1, j, k + 1) - tab_at(t, N, i + 1, j, k - 1) - tab_at(t, N, i - 1, j, k + 1) + tab_at(t, N, i - 1, j, k - 1));
+    double Dyz = 0.25 * (tab_at(t, N, i, j + 1, k + 1) - tab_at(t, N, i, j + 1, k - 1) - tab_at(t, N, i, j - 1, k + 1) + tab_at(t, N, i, j - 1, k - 1));
+    return C0 + Dx * d[0] + Dy * d[1] + Dz * d[2] + 0.5 * (Dxx * d[0] * d[0] + Dyy * d[1] * d[1] + Dzz * d[2] * d[2]) +
+           Dxy * d[0] * d[1] + Dxz * d[0] * d[2] + Dyz * d[1] * d[2];
+}
+
+/* The group walk under periodic boundaries (W-rules unchanged except, reading P5):
+ *  - every displacement is the MINIMUM IMAGE one, d_a -> d_a - L nearbyint(d_a / L), in the opening test
+ *    (Eq. 3 / Eq. 4 with that distance) and in the sums;
+ *  - an accepted node or a leaf cell contributes M (1/d + corr1(d_vec/L)/L) = M f_EF (Eq. A.1), corr1 taken
+ *    from the table by quadratic interpolation;
+ *  - the target's own cell, and a distinct cell at zero distance, contribute their images and background
+ *    only: m corr1(0)/L (the 1/d term is dropped as in W-rule 3).
+ * table: orc_ewald_table(N, nref, ...).  The cube of the tree is the periodic box. */
+static double wrap_mi(double d, double L) { return d - L * nearbyint(d / L); }
+
+int orc_potential_periodic(const orc_tree *t, double theta, double G, int mac, int group, const double *table,
+                           int N, int nref, int64_t group_begin, int64_t group_end, double *phi_orig, int64_t *counts)
+{
+    if (!t || !phi_orig || !table || !(theta >= 0.0) || group < 1) return -1;
+    int64_t n = t->n;
+    double L = t->cube[3];
+    int64_t ngroups = (n + group - 1) / group;
+    if (group_end < 0 || group_end > ngroups) group_end = ngroups;
+    if (group_begin < 0) group_begin = 0;
+    int64_t stack[8 * (ORC_MAXLEVEL + 2)];
+    double *acc = (double *)malloc(sizeof(double) * (size_t)group);
+    if (!acc) return -2;
+    const double zero[3] = {0.0, 0.0, 0.0};
+    double c0 = orc_ewald_interp(table, N, nref, zero) / L;
+    for (int64_t g = group_begin; g < group_end; ++g) {
+        int64_t t0 = g * group, t1 = t0 + group;
+        if (t1 > n) t1 = n;
+        int nt = (int)(t1 - t0);
+        for (int a = 0; a < nt; ++a) acc[a] = 0.0;
+        int64_t n_acc = 0, n_leaf = 0, n_open = 0;
+        int sp = 0;
+        if (n >= 2) stack[sp++] = 0;
+        else acc[0] = t->m[0] * c0; /* a lone cell still feels its own images */
+        while (sp > 0) {
+            int64_t e = stack[--sp];
+            const orc_node *nd = e >= 0 ? &t->node[e] : NULL;
+            if (e <= -2 || nd->level == ORC_MAXLEVEL) { /* leaf cell, or every cell of a bucket */
+                int64_t j0 = e <= -2 ? -(e + 2) : nd->lo, j1 = e <= -2 ? j0 + 1 : nd->hi;
+                for (int64_t j = j0; j < j1; ++j) {
+                    for (int a = 0; a < nt; ++a) {
+                        int64_t s = t0 + a;
+                        double r[3] = {wrap_mi(t->x[s] - t->x[j], L), wrap_mi(t->y[s] - t->y[j], L), wrap_mi(t->z[s] - t->z[j], L)};
+                        double d2 = r[0] * r[0] + r[1] * r[1] + r[2] * r[2];
+                        if (s == j || d2 == 0.0) { acc[a] += t->m[j] * c0; continue; }
+                        double u[3] = {r[0] / L, r[1] / L, r[2] / L};
+                        acc[a] += t->m[j] * (1.0 / sqrt(d2) + orc_ewald_interp(table, N, nref, u) / L);
+                    }
+                    ++n_leaf;
+                }
+                continue;
+            }
+            int accept = theta > 0.0;
+            if (accept) {
+                double rc = nd->size / theta;
+                if (mac == ORC_MAC_BARNES94) rc += nd->delta;
+                for (int a = 0; a < nt && accept; ++a) {
+                    int64_t s = t0 + a;
+                    double dx = wrap_mi(t->x[s] - nd->R[0], L), dy = wrap_mi(t->y[s] - nd->R[1], L), dz = wrap_mi(t->z[s] - nd->R[2], L);
+                    if (!(dx * dx + dy * dy + dz * dz > rc * rc)) accept = 0;
+                }
+            }
+            if (accept) {
+                for (int a = 0; a < nt; ++a) {
+                    int64_t s = t0 + a;
+                    double r[3] = {wrap_mi(t->x[s] - nd->R[0], L), wrap_mi(t->y[s] - nd->R[1], L), wrap_mi(t->z[s] - nd->R[2], L)};
+                    double u[3] = {r[0] / L, r[1] / L, r[2] / L};
+                    acc[a] += nd->M * (1.0 / sqrt(r[0] * r[0] + r[1] * r[1] + r[2] * r[2]) + orc_ewald_interp(table, N, nref, u) / L);
+                }
+                ++n_acc;
+                continue;
+            }
+            ++n_open;
+            for (int c = 7; c >= 0; --c)
+                if (nd->child[c] != -1) stack[sp++] = nd->child[c];
+        }
+        for (int a = 0; a < nt; ++a) phi_orig[t->perm[t0 + a]] = -G * acc[a];
+        if (counts) {
+            int64_t *c = counts + 3 * (g - group_begin);
+            c[0] = n_acc; c[1] = n_leaf; c[2] = n_open;
+        }
+    }
+    free(acc);
+    return 0;
+}

@@ -37,8 +37,11 @@
 namespace bh {
 
 constexpr int kWalkWarps = 4;                 // warps (= group pairs) per CTA
-constexpr int kU2Cap = 128;                   // entries of the both-groups list (float4 each)
-constexpr int kU1Cap = 64;                    // entries of each one-group list (SoA x,y,z,m)
+constexpr int kU2Cap = 128;                   // entries of the both-groups list
+constexpr int kU1Cap = 64;                    // entries of each one-group list
+constexpr int kSoaCap = kU2Cap + 2 * kU1Cap;  // the three unchecked lists share ONE SoA block x[256] y[256] z[256] m[256]:
+constexpr int kOffUA = kU2Cap;                //   U2 at [0, 128), UA at [128, 192), UB at [192, 256) of every component,
+constexpr int kOffUB = kU2Cap + kU1Cap;       //   so an append is four stores at one computed index whatever the list
 constexpr int kCCap = 64;                     // entries of the checked list (float4 + group mask)
 constexpr int kStepMax = 32;                  // a traversal step appends <= 32 entries to any list
 constexpr int kStackPerLevel = 36;            // stack entries a level can leave behind (<= 3 + 32)
@@ -65,7 +68,7 @@ struct WalkParams {
 
 __host__ __device__ inline size_t walk_smem_per_warp(int stack_cap)
 {
-    return (size_t)kU2Cap * 16 + 2 * (size_t)kU1Cap * 16 + (size_t)kCCap * 16 + (size_t)kCCap * 4 + 32 * 16 +
+    return (size_t)kSoaCap * 16 + (size_t)kCCap * 16 + (size_t)kCCap * 4 + 32 * 16 +
            (size_t)stack_cap * sizeof(uint2);
 }
 
@@ -334,10 +337,10 @@ walk_pair_kernel(const WalkParams P)
     if (gA >= P.ngroups) return;                      // whole warp leaves; no block-level sync below
 
     unsigned char* my = smem_raw + (size_t)warp * walk_smem_per_warp(P.stack_cap);
-    float* U2 = reinterpret_cast<float*>(my);                           // both groups (SoA)
-    float* UA = U2 + 4 * kU2Cap;                                        // group A only (SoA)
-    float* UB = UA + 4 * kU1Cap;                                        // group B only (SoA)
-    float4* C = reinterpret_cast<float4*>(UB + 4 * kU1Cap);             // checked leaf cells
+    float* U2 = reinterpret_cast<float*>(my);                           // both groups (SoA block, component stride kSoaCap)
+    float* UA = U2 + kOffUA;                                            // group A only (same block)
+    float* UB = U2 + kOffUB;                                            // group B only (same block)
+    float4* C = reinterpret_cast<float4*>(U2 + 4 * kSoaCap);            // checked leaf cells
     u32* Cm = reinterpret_cast<u32*>(C + kCCap);                        //   and the groups they serve
     float4* amb = reinterpret_cast<float4*>(Cm + kCCap);                // nodes awaiting the member vote
     uint2* stack = reinterpret_cast<uint2*>(amb + 32);                  // (first child slot, count | groups << 30)
@@ -439,11 +442,13 @@ walk_pair_kernel(const WalkParams P)
         const u32 bAmb = __ballot_sync(0xffffffffu, ambm != 0u);
         if (bAmb) {
             const int myr = __popc(bAmb & lt);
-            if (ambm) amb[myr] = make_float4(r.x, r.y, r.z, rc2);
+            // .w = ~bits(r_c^2): for non-negative floats d^2 <= r_c^2 iff bits(d^2) + ~bits(r_c^2) < 0 as integers
+            if (ambm) amb[myr] = make_float4(r.x, r.y, r.z, __uint_as_float(~__float_as_uint(rc2)));
             __syncwarp();
             const int na = __popc(bAmb);
-            // bit i of failA / failB: this lane's member of A / B does NOT pass node i; one OR-reduction
-            // per group then replaces a vote per node
+            // failA / failB collect, one bit per undecided node (node i at bit na - 1 - i), whether this lane's
+            // member of A / B does NOT pass it (the sign bit of the integer difference is shifted in); one
+            // OR-reduction per group then replaces a vote per node
             u32 failA = 0u, failB = 0u;
             #pragma unroll 4
             for (int i = 0; i < na; ++i) {
@@ -451,12 +456,13 @@ walk_pair_kernel(const WalkParams P)
                 const float2 dx = __fadd2_rn(splat2(q.x), npx), dy = __fadd2_rn(splat2(q.y), npy),
                              dz = __fadd2_rn(splat2(q.z), npz);
                 const float2 d2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
-                failA |= (d2.x > q.w ? 0u : 1u) << i;
-                failB |= (d2.y > q.w ? 0u : 1u) << i;
+                failA = __funnelshift_l(__float_as_uint(d2.x) + __float_as_uint(q.w), failA, 1);
+                failB = __funnelshift_l(__float_as_uint(d2.y) + __float_as_uint(q.w), failB, 1);
             }
             const u32 resA = ~__reduce_or_sync(0xffffffffu, liveA ? failA : 0u);
             const u32 resB = ~__reduce_or_sync(0xffffffffu, liveB ? failB : 0u);
-            accm |= ambm & (((resA >> myr) & 1u) | (((resB >> myr) & 1u) << 1));
+            const int bit = na - 1 - myr;
+            accm |= ambm & (((resA >> bit) & 1u) | (((resB >> bit) & 1u) << 1));
             if (COUNT) { cExA += ambm & 1u; cExB += ambm >> 1; }
             __syncwarp();
         }
@@ -476,41 +482,43 @@ walk_pair_kernel(const WalkParams P)
         // ---- append accepted nodes and leaf cells to the lists ----
         // leaf cells inside a group's box may be a target's own cell or coincide with one
         const bool danger = leaf && (((msk & 1u) && !(d2min.x > 0.f)) || ((msk & 2u) && !(d2min.y > 0.f)));
-        const u32 um = internal ? accm : (danger ? 0u : msk);
-        const bool toU2 = um == 3u, toUA = um == 1u, toUB = um == 2u;
-        const u32 bU2 = __ballot_sync(0xffffffffu, toU2);
-        const u32 bUA = __ballot_sync(0xffffffffu, toUA);
-        const u32 bUB = __ballot_sync(0xffffffffu, toUB);
+        const u32 um = internal ? accm : (danger ? 0u : msk);           // 3: both groups, 1: A only, 2: B only
+        const u32 b1 = __ballot_sync(0xffffffffu, um & 1u);
+        const u32 b2 = __ballot_sync(0xffffffffu, um & 2u);
+        const u32 same = ((um & 1u) ? b1 : ~b1) & ((um & 2u) ? b2 : ~b2);   // lanes that append to the same list
+        const int cU2 = __popc(b1 & b2), cUA = __popc(b1 & ~b2), cUB = __popc(b2 & ~b1);
+        if (um) {
+            const int at = (um == 3u ? nU2 : (um == 1u ? kOffUA + nUA : kOffUB + nUB)) + __popc(same & lt);
+            soa_store<kSoaCap>(U2, at, r);
+        }
+        nU2 += cU2; nUA += cUA; nUB += cUB;
         const u32 bC = __ballot_sync(0xffffffffu, danger);
-        const u32 bsel = toU2 ? bU2 : (toUA ? bUA : (toUB ? bUB : bC));
-        const int rank = __popc(bsel & lt);
-        if (toU2) soa_store<kU2Cap>(U2, nU2 + rank, r);
-        if (toUA) soa_store<kU1Cap>(UA, nUA + rank, r);
-        if (toUB) soa_store<kU1Cap>(UB, nUB + rank, r);
-        if (danger) { C[nC + rank] = r; Cm[nC + rank] = msk; }
-        nU2 += __popc(bU2); nUA += __popc(bUA); nUB += __popc(bUB); nC += __popc(bC);
+        if (bC) {                                                       // rare: only next to the groups' own cells
+            if (danger) { const int at = nC + __popc(bC & lt); C[at] = r; Cm[at] = msk; }
+            nC += __popc(bC);
+        }
         __syncwarp();
         // ---- evaluate a list before the next step could overflow it ----
         if ((((nUA | nUB | nC) >> 5) != 0) || nU2 >= kU2Cap - kStepMax) {
             if (nU2 >= kU2Cap - kStepMax) {
-                soa_pad<kU2Cap>(U2, nU2);
+                soa_pad<kSoaCap>(U2, nU2);
                 __syncwarp();
-                if (ACC) eval_soa2_g<kU2Cap>(U2, nU2, TA, TB, accA, accB, grA, grB);
-                else eval_soa2<kU2Cap>(U2, nU2, TA, TB, accA, accB);
+                if (ACC) eval_soa2_g<kSoaCap>(U2, nU2, TA, TB, accA, accB, grA, grB);
+                else eval_soa2<kSoaCap>(U2, nU2, TA, TB, accA, accB);
                 evA += (u32)nU2; evB += (u32)nU2;
                 nU2 = 0;
             }
             if (nUA >= kU1Cap - kStepMax) {
-                soa_pad<kU1Cap>(UA, nUA);
+                soa_pad<kSoaCap>(UA, nUA);
                 __syncwarp();
-                accA += ACC ? eval_soa_g<kU1Cap>(UA, nUA, TA, grA) : eval_soa<kU1Cap>(UA, nUA, TA);
+                accA += ACC ? eval_soa_g<kSoaCap>(UA, nUA, TA, grA) : eval_soa<kSoaCap>(UA, nUA, TA);
                 evA += (u32)nUA;
                 nUA = 0;
             }
             if (nUB >= kU1Cap - kStepMax) {
-                soa_pad<kU1Cap>(UB, nUB);
+                soa_pad<kSoaCap>(UB, nUB);
                 __syncwarp();
-                accB += ACC ? eval_soa_g<kU1Cap>(UB, nUB, TB, grB) : eval_soa<kU1Cap>(UB, nUB, TB);
+                accB += ACC ? eval_soa_g<kSoaCap>(UB, nUB, TB, grB) : eval_soa<kSoaCap>(UB, nUB, TB);
                 evB += (u32)nUB;
                 nUB = 0;
             }
@@ -534,20 +542,20 @@ walk_pair_kernel(const WalkParams P)
         return;
     }
     if (nU2 > 0) {
-        soa_pad<kU2Cap>(U2, nU2);
+        soa_pad<kSoaCap>(U2, nU2);
         __syncwarp();
-        if (ACC) eval_soa2_g<kU2Cap>(U2, nU2, TA, TB, accA, accB, grA, grB);
-        else eval_soa2<kU2Cap>(U2, nU2, TA, TB, accA, accB);
+        if (ACC) eval_soa2_g<kSoaCap>(U2, nU2, TA, TB, accA, accB, grA, grB);
+        else eval_soa2<kSoaCap>(U2, nU2, TA, TB, accA, accB);
     }
     if (nUA > 0) {
-        soa_pad<kU1Cap>(UA, nUA);
+        soa_pad<kSoaCap>(UA, nUA);
         __syncwarp();
-        accA += ACC ? eval_soa_g<kU1Cap>(UA, nUA, TA, grA) : eval_soa<kU1Cap>(UA, nUA, TA);
+        accA += ACC ? eval_soa_g<kSoaCap>(UA, nUA, TA, grA) : eval_soa<kSoaCap>(UA, nUA, TA);
     }
     if (nUB > 0) {
-        soa_pad<kU1Cap>(UB, nUB);
+        soa_pad<kSoaCap>(UB, nUB);
         __syncwarp();
-        accB += ACC ? eval_soa_g<kU1Cap>(UB, nUB, TB, grB) : eval_soa<kU1Cap>(UB, nUB, TB);
+        accB += ACC ? eval_soa_g<kSoaCap>(UB, nUB, TB, grB) : eval_soa<kSoaCap>(UB, nUB, TB);
     }
     if (nC > 0) {
         if (ACC) eval_c_g(C, Cm, nC, npx, npy, npz, accA, accB, grA, grB, evA, evB);
