@@ -25,6 +25,10 @@
  *                 domain box with the minimum-distance form of the opening test (E1-E4).
  *   orc_field / orc_direct_acc  the acceleration g = -grad Phi on the walk's own interaction lists and by
  *                 direct summation (the Phi arithmetic of orc_potential is untouched).
+ *   orc_ewald_psi / orc_ewald_corr / orc_ewald_table / orc_ewald_interp / orc_potential_periodic
+ *                 periodic boundaries (App. A, Eq. A.1-A.3): the Ewald
+ *                 field of 1/r in a cubic box, its nested-grid table, quadratic interpolation, and the group
+ *                 walk with minimum-image displacements (readings P1-P5).
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): keys vs closed form on 2^k grids and a per-bit
  * interleave; tree vs a recursive brute-force partition in numpy; node counts (n-1)/7 on grids;
@@ -33,7 +37,13 @@
  * coordinates, the 1..n limits of PAPER.md:106, mass conservation and the potential inside the box
  * (tests/test_oracle_essential.py); accelerations vs a numpy brute force, the numerical gradient of the
  * direct-sum potential, Newton's third law and the two-body / uniform-sphere closed forms
- * (tests/test_oracle_field.py).  No function here is "parity unpinned".
+ * (tests/test_oracle_field.py); the Ewald field vs its independence of alpha over a decade, a brute-force
+ * shell-summed lattice sum, the simple-cubic Madelung constant 2.8372974795, zero mean against the cube
+ * constant 2.3800774, the Laplacian 4 pi, cubic symmetry and periodicity; the table and its interpolation vs
+ * the exact field; the periodic walk vs the exact Ewald direct sum, translation invariance and the closed
+ * form of a uniform periodic lattice (tests/test_oracle_ewald.py); the mac_fp32 branch of group_accepts vs
+ * an independent numpy-float32 restatement incl. one-ulp threshold scans (tests/test_oracle_walk.py,
+ * tests/fp32_decision.py).  No function here is "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>
@@ -674,13 +684,15 @@ double orc_ewald_corr(const double *u, double a, int nser)
  * nested grids".  Reading P3: corr1 is even in every coordinate, so the array covers the
  * octant u_a >= 0; grid `lev` (0 .. nref-1, "gpuEwaldSeriesNref ... the number of nested grids") has N
  * points per axis ("gpuEwaldFieldNx/y/z"; one N here, the box is a cube) at u = i * h_lev,
- * h_lev = (1/2) / (N - 1) / 2^lev, i.e. it spans [0, 1/2^(lev+1)] per axis: every grid refines the corner
- * of the previous one around u = 0.  table[((lev * N + k) * N + j) * N + i] = corr1(i h, j h, k h). */
+ * h_lev = (1/2) / (N - 2) / 2^lev: grid 0 reaches ONE point past the face of the minimum-image cell
+ * (u = 1/2 is its point N - 2; corr1 is smooth there but not mirror symmetric, because 1/|u| is not), so the
+ * 3-point stencil of any |u_a| <= 1/2 lies inside it; every further grid refines the corner of the previous one
+ * around u = 0 by a factor of two.  table[((lev * N + k) * N + j) * N + i] = corr1(i h, j h, k h). */
 int orc_ewald_table(int N, int nref, double a, int nser, double *table)
 {
     if (N < 4 || nref < 1 || !(a > 0.0) || nser < 1 || !table) return -1;
     for (int lev = 0; lev < nref; ++lev) {
-        double h = 0.5 / (N - 1) / (double)(1 << lev);
+        double h = 0.5 / (N - 2) / (double)(1 << lev);
         double *t = table + (size_t)lev * N * N * N;
         for (int k = 0; k < N; ++k)
             for (int j = 0; j <= k; ++j)
@@ -701,15 +713,13 @@ int orc_ewald_table(int N, int nref, double a, int nser, double *table)
  * NEAREST grid point i0 per axis and the quadratic through the 3 points per axis around it,
  *   corr(u) ~ C0 + sum_a Da d_a + 1/2 sum_a Daa d_a^2 + sum_{a<b} Dab d_a d_b,   d_a = |u_a|/h - i0_a in [-1/2, 1/2],
  *   Da = (C[+a] - C[-a])/2,  Daa = C[+a] - 2 C0 + C[-a],  Dab = (C[+a+b] - C[+a-b] - C[-a+b] + C[-a-b])/4.
- * Index -1 mirrors to +1 (corr1 is even); on grid 0, index N mirrors to N - 2 (corr1(1/2 + t) = corr1(1/2 - t):
- * periodic and even).  u must be a minimum-image displacement in box units, |u_a| <= 1/2. */
+ * Index -1 mirrors to +1 (corr1 is even); the nearest point never exceeds N - 2, so index N - 1 is the last one
+ * read.  u must be a minimum-image displacement in box units, |u_a| <= 1/2. */
 static double tab_at(const double *t, int N, int i, int j, int k)
 {
     int v[3] = {i, j, k};
-    for (int c = 0; c < 3; ++c) {
+    for (int c = 0; c < 3; ++c)
         if (v[c] < 0) v[c] = -v[c];
-        if (v[c] >= N) v[c] = 2 * (N - 1) - v[c];
-    }
     i = v[0]; j = v[1]; k = v[2];
     return t[((size_t)k * N + j) * N + i];
 }
@@ -718,18 +728,18 @@ double orc_ewald_interp(const double *table, int N, int nref, const double *u)
 {
     double ax = fabs(u[0]), ay = fabs(u[1]), az = fabs(u[2]);
     double mx = ax > ay ? (ax > az ? ax : az) : (ay > az ? ay : az);
-    int lev = 0; /* finest grid whose interior (nearest point <= N - 2) holds the point */
+    int lev = 0; /* finest grid whose interior (nearest point <= N - 2) holds the point: mx <= 1/2^(l+1) */
     for (int l = nref - 1; l > 0; --l) {
-        double h = 0.5 / (N - 1) / (double)(1 << l);
+        double h = 0.5 / (N - 2) / (double)(1 << l);
         if (mx <= (N - 2) * h) { lev = l; break; }
     }
-    double h = 0.5 / (N - 1) / (double)(1 << lev);
+    double h = 0.5 / (N - 2) / (double)(1 << lev);
     const double *t = table + (size_t)lev * N * N * N;
     double p[3] = {ax / h, ay / h, az / h};
     int i0[3]; double d[3];
     for (int c = 0; c < 3; ++c) {
         i0[c] = (int)floor(p[c] + 0.5);
-        if (i0[c] > N - 1) i0[c] = N - 1;
+        if (i0[c] > N - 2) i0[c] = N - 2;
         d[c] = p[c] - i0[c];
     }
     int i = i0[0], j = i0[1], k = i0[2];

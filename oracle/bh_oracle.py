@@ -56,6 +56,15 @@ def _L():
         lib.orc_direct_acc.argtypes = [dp, dp, dp, dp, C.c_int64, C.c_double, i64p, C.c_int64, dp]
         lib.orc_essential_nodes.argtypes = [C.c_void_p, dp, dp, C.c_double, C.c_int, dp, i32p, i64p, i64p]
         lib.orc_essential_nodes.restype = C.c_int64
+        lib.orc_ewald_psi.argtypes = [dp, C.c_double, C.c_int]
+        lib.orc_ewald_psi.restype = C.c_double
+        lib.orc_ewald_corr.argtypes = [dp, C.c_double, C.c_int]
+        lib.orc_ewald_corr.restype = C.c_double
+        lib.orc_ewald_table.argtypes = [C.c_int, C.c_int, C.c_double, C.c_int, dp]
+        lib.orc_ewald_interp.argtypes = [dp, C.c_int, C.c_int, dp]
+        lib.orc_ewald_interp.restype = C.c_double
+        lib.orc_potential_periodic.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_int, dp, C.c_int, C.c_int,
+                                               C.c_int64, C.c_int64, dp, i64p]
         _lib = lib
     return _lib
 
@@ -121,6 +130,37 @@ def direct_acc(x, y, z, m, G=1.0, targets=None):
     return acc
 
 
+def ewald_psi(u, a=2.0, nser=5):
+    """psi1(u): the Ewald sum of 1/r in the unit cube with neutralising background (PAPER.md:551-567, Eq. A.1-A.3;
+    DESIGN.md reading P1), u = r/L; a = alpha L; sums over |n_i|, |h_i| <= nser."""
+    u = _f64(u)
+    return float(_L().orc_ewald_psi(_p(u, C.c_double), float(a), int(nser)))
+
+
+def ewald_corr(u, a=2.0, nser=5):
+    """corr1(u) = psi1(u) - 1/|u| (its finite limit at u = 0): what the field array tabulates (reading P2)."""
+    u = _f64(u)
+    return float(_L().orc_ewald_corr(_p(u, C.c_double), float(a), int(nser)))
+
+
+class EwaldTable:
+    """The nested-grid Ewald field array (readings P3, P4): `nref` grids of N^3 points of corr1
+    on the octant u_a >= 0, spacing (1/2)/(N-2)/2^k (u = 1/2^(k+1) is point N-2 of grid k); quadratic interpolation."""
+
+    def __init__(self, N=32, nref=1, a=2.0, nser=5):
+        self.N, self.nref, self.a, self.nser = int(N), int(nref), float(a), int(nser)
+        self.data = np.empty(self.nref * self.N ** 3, dtype=np.float64)
+        if _L().orc_ewald_table(self.N, self.nref, self.a, self.nser, _p(self.data, C.c_double)) != 0:
+            raise ValueError("orc_ewald_table: invalid argument")
+
+    def grid(self, lev=0):
+        return self.data[lev * self.N ** 3:(lev + 1) * self.N ** 3].reshape(self.N, self.N, self.N)   # [k][j][i]
+
+    def interp(self, u):
+        u = _f64(u)
+        return float(_L().orc_ewald_interp(_p(self.data, C.c_double), self.N, self.nref, _p(u, C.c_double)))
+
+
 class OracleTree:
     """keys -> sort -> octree -> monopoles for one set of cells (orc_build)."""
 
@@ -172,6 +212,21 @@ class OracleTree:
                                 gb, ge, _p(phi, C.c_double), _p(counts, C.c_int64))
         if rc != 0:
             raise ValueError("orc_potential: invalid argument")
+        return (phi, counts) if want_counts else phi
+
+    def potential_periodic(self, theta, table, G=1.0, mac=MAC_BH86, group=32, groups=None, want_counts=False, out=None):
+        """The group walk under periodic boundaries (App. A; reading P5): minimum-image displacements in the opening
+        test and the sums, every entry contributing M (1/d + corr1(d/L)/L) with corr1 interpolated in `table`
+        (an EwaldTable); the tree's cube is the periodic box.  Decisions in fp64."""
+        ng = (self.n + group - 1) // group
+        gb, ge = (0, ng) if groups is None else groups
+        phi = np.full(self.n, np.nan) if out is None else out
+        counts = np.zeros((max(ge - gb, 0), 3), dtype=np.int64)
+        rc = _L().orc_potential_periodic(self._h, float(theta), float(G), int(mac), int(group),
+                                         _p(table.data, C.c_double), table.N, table.nref, gb, ge,
+                                         _p(phi, C.c_double), _p(counts, C.c_int64))
+        if rc != 0:
+            raise ValueError("orc_potential_periodic: invalid argument")
         return (phi, counts) if want_counts else phi
 
     def essential_nodes(self, box_lo, box_hi, theta, mac=MAC_BARNES94, want_ranges=False):
