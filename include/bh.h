@@ -50,6 +50,11 @@ typedef struct bh_ctx bh_ctx;
 #define BH_MAC_BARNES94 1 /*   Eq. 4:  accept iff d > l/theta + delta              */
 #define BH_OPT_GROUP  2   /* how many consecutive Morton-sorted targets share one walk and one vote */
                           /*   32 (default): the paper's warp vote; 1: per-target lists  */
+#define BH_OPT_PERIODIC 4    /* 1: the cube of bh_build is a PERIODIC box (App. A): bh_potential uses
+                                minimum-image displacements and adds the Ewald field; 0 (default): isolated        */
+#define BH_OPT_EWALD_N    5  /* points per axis of each grid of the Ewald field array (6..258, default 66;
+                                "gpuEwaldFieldNx/y/z"; one number: the box is a cube)                */
+#define BH_OPT_EWALD_NREF 6  /* number of nested grids (1..8, default 1; "gpuEwaldSeriesNref")      */
 #define BH_OPT_PASS_TIMING 3 /* 1: bh_build records a CUDA event after every kernel (bh_get_build_passes); a
                                 reporting mode -- the events cost a little, 0 (default) records none          */
 
@@ -172,6 +177,21 @@ int bh_set_num_targets(bh_ctx* ctx, int64_t ntargets);
  *    ~2^-23 L/d.  Cell centres of grids and AMR meshes (dyadic rationals) are exact; for arbitrary
  *    points the 1e-4 bar on Phi holds while the closest pairs are farther apart than ~1e-3 L. */
 int bh_potential(bh_ctx* ctx, double theta, double G, double* phi);
+
+/* Periodic boundaries (BH_OPT_PERIODIC = 1; Appendix A, readings P1-P5).
+ * A node or cell of mass M at minimum-image displacement r contributes -G M f_EF(r) (Eq. A.1),
+ * f_EF(r) = 1/|r| + corr1(r/L)/L, corr1 = the Ewald sum of 1/r in the unit cube with a neutralising background
+ * (Eq. A.2-A.3) minus 1/|u|.  corr1 is tabulated once per context on `nref` nested grids of N^3 points covering
+ * the octant u >= 0 (grid k: spacing (1/2)/(N-2)/2^k) and evaluated in the walk by quadratic interpolation
+ * around the nearest grid point.  The opening test uses the minimum-image distance.  A target's own
+ * cell and distinct cells at zero distance contribute their images and background only, m corr1(0)/L.
+ * Restrictions: group walk of all cells only -- BH_OPT_GROUP = 1, bh_field and bh_set_num_targets return
+ * BH_ERR_INVALID_ARG while BH_OPT_PERIODIC is on; cells must lie inside the cube.
+ *
+ * bh_ewald_table: the grid values of corr1 (fp64) as the context computed them, for checking:
+ *   out : DEVICE, double[nref * N^3], out[((k_grid * N + k) * N + j) * N + i] = corr1(i h, j h, k h); NULL with cap 0
+ *         queries *N and *nref (HOST, may be NULL) and returns BH_ERR_TOO_LARGE. */
+int bh_ewald_table(bh_ctx* ctx, double* out, int64_t cap, int* N, int* nref);
 
 /* bh_field: bh_potential plus the acceleration g_i = -grad Phi_i in the same walk (
  * the paper returns Phi only and lets the host code difference it).  The interaction lists,

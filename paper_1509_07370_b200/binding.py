@@ -11,13 +11,16 @@ BH_MAC_BARNES94 = 1   # Eq. 4
 BH_OPT_MAC = 1
 BH_OPT_GROUP = 2
 BH_OPT_PASS_TIMING = 3
+BH_OPT_PERIODIC = 4
+BH_OPT_EWALD_N = 5
+BH_OPT_EWALD_NREF = 6
 BH_DIRECT_ALL_MAX = 1 << 18
 
 EXPORTED_SYMBOLS = (
     "bh_create", "bh_destroy", "bh_strerror", "bh_last_cuda_error", "bh_set_option", "bh_build", "bh_potential",
     "bh_potential_direct", "bh_solve_host", "bh_tree_sizes", "bh_export_tree", "bh_last_group_counts",
     "bh_last_interactions", "bh_get_stats", "bh_update_masses", "bh_essential_nodes", "bh_set_num_targets", "bh_field",
-    "bh_last_group_evaluated", "bh_last_walk_group", "bh_get_build_passes", "bh_host_breakdown",
+    "bh_last_group_evaluated", "bh_last_walk_group", "bh_get_build_passes", "bh_host_breakdown", "bh_ewald_table",
 )
 
 
@@ -83,6 +86,7 @@ def lib():
         L.bh_last_walk_group.argtypes = [vp]
         L.bh_get_build_passes.argtypes = [vp, C.POINTER(Pass), i32, C.POINTER(i32)]
         L.bh_host_breakdown.argtypes = [vp, C.POINTER(C.c_float)]
+        L.bh_ewald_table.argtypes = [vp, dp, i64, C.POINTER(i32), C.POINTER(i32)]
         L.bh_get_stats.argtypes = [vp, C.POINTER(Stats)]
         for name in EXPORTED_SYMBOLS:
             if name not in ("bh_strerror", "bh_last_cuda_error"):
@@ -153,6 +157,23 @@ class Context:
 
     def set_group(self, group: int):
         self.set_option(BH_OPT_GROUP, group)
+
+    def set_periodic(self, on: bool, N: int = None, nref: int = None):
+        """BH_OPT_PERIODIC (+ the size of the Ewald field array): the cube of the build is a periodic box."""
+        if N is not None:
+            self.set_option(BH_OPT_EWALD_N, int(N))
+        if nref is not None:
+            self.set_option(BH_OPT_EWALD_NREF, int(nref))
+        self.set_option(BH_OPT_PERIODIC, 1 if on else 0)
+
+    def ewald_table(self):
+        """bh_ewald_table: CUDA float64 tensor [nref, N, N, N] (k, j, i order) of corr1 on the nested grids."""
+        torch = self._torch
+        N, nref = C.c_int(0), C.c_int(0)
+        self._L.bh_ewald_table(self._h, None, 0, C.byref(N), C.byref(nref))
+        out = torch.empty((nref.value, N.value, N.value, N.value), dtype=torch.float64, device=f"cuda:{self.device}")
+        self._check(self._L.bh_ewald_table(self._h, self._dev(out, torch.float64), out.numel(), C.byref(N), C.byref(nref)))
+        return out
 
     def build(self, x, y, z, m, cube):
         f64 = self._torch.float64

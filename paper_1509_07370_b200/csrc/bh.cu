@@ -10,6 +10,7 @@
 
 #include "common.cuh"
 #include "direct.cuh"
+#include "ewald.cuh"
 #include "keys.cuh"
 #include "let.cuh"
 #include "scan.cuh"
@@ -61,6 +62,11 @@ struct bh_ctx {
     bool built = false;
     bool walked = false;
     int walk_group = 32;
+    bool periodic = false;                // BH_OPT_PERIODIC: the cube of the build is a periodic box (App. A)
+    bool walk_periodic = false;           // ... of the last walk (the count pass repeats it)
+    int ew_N = 66, ew_nref = 1;           // BH_OPT_EWALD_N / _NREF: points per axis and nested grids of the field array
+    int ew_ready_N = 0, ew_ready_nref = 0;
+    DevBuf ew_table, ew_coef;             // grid values (fp64) and per-point quadratic coefficients (fp32)
     bool counts_valid = false;            // gcount holds the counters of the last walk
     double walk_theta = 0.0;              // arguments of the last bh_potential (the count pass repeats its walk)
     int walk_mac = BH_MAC_BH86;
@@ -270,6 +276,8 @@ int bh_create(bh_ctx** out, int device, void* cuda_stream)
             {(const void*)walk_pair_kernel<true, true>, walk_smem, "walk subset count"},
             {(const void*)walk_pair_kernel<false, false, true>, walk_smem, "walk field"},
             {(const void*)walk_pair_kernel<false, true, true>, walk_smem, "walk field subset"},
+            {(const void*)walk_pair_kernel<false, false, false, true>, walk_smem, "walk periodic"},
+            {(const void*)walk_pair_kernel<true, false, false, true>, walk_smem, "walk periodic count"},
         };
         for (const auto& k : big_smem) {
             if ((e = cudaFuncSetAttribute(k.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, k.bytes)) != cudaSuccess) {
@@ -291,7 +299,8 @@ int bh_destroy(bh_ctx* ctx)
     DevBuf* all[] = {&ctx->keysA, &ctx->keysB, &ctx->idxA, &ctx->idxB, &ctx->clev, &ctx->leaf_slot, &ctx->leaf64,
                      &ctx->slot_of, &ctx->hist, &ctx->scan_scratch, &ctx->nlo, &ctx->nfirst, &ctx->node_slot,
                      &ctx->delta64, &ctx->rec64, &ctx->rec, &ctx->aux, &ctx->gcount, &ctx->geval, &ctx->scalars, &ctx->stage[0],
-                     &ctx->stage[1], &ctx->stage[2], &ctx->stage[3], &ctx->stage_phi, &ctx->ess_state, &ctx->ess_emit};
+                     &ctx->stage[1], &ctx->stage[2], &ctx->stage[3], &ctx->stage_phi, &ctx->ess_state, &ctx->ess_emit,
+                     &ctx->ew_table, &ctx->ew_coef};
     for (DevBuf* b : all) b->release();
     if (ctx->h_scalars) cudaFreeHost(ctx->h_scalars);
     if (ctx->copy_stream) { cudaStreamSynchronize(ctx->copy_stream); cudaStreamDestroy(ctx->copy_stream); }
@@ -310,6 +319,9 @@ int bh_set_option(bh_ctx* ctx, int key, int value)
     if (!ctx) return BH_ERR_INVALID_ARG;
     if (key == BH_OPT_MAC && (value == BH_MAC_BH86 || value == BH_MAC_BARNES94)) { ctx->mac = value; return BH_OK; }
     if (key == BH_OPT_GROUP && (value == 32 || value == 1)) { ctx->group = value; return BH_OK; }
+    if (key == BH_OPT_PERIODIC && (value == 0 || value == 1)) { ctx->periodic = value != 0; return BH_OK; }
+    if (key == BH_OPT_EWALD_N && value >= 6 && value <= 258) { ctx->ew_N = value; return BH_OK; }
+    if (key == BH_OPT_EWALD_NREF && value >= 1 && value <= 8) { ctx->ew_nref = value; return BH_OK; }
     if (key == BH_OPT_PASS_TIMING && (value == 0 || value == 1)) { ctx->pass_timing = value != 0; ctx->npass = 0; return BH_OK; }
     return BH_ERR_INVALID_ARG;
 }
@@ -385,11 +397,11 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
             BH_CUDA(cudaStreamSynchronize(st));
             kr = ctx->h_scalars->keyred;
         }
-        const SortPlan plan = make_sort_plan(kr.key_or ^ kr.key_and);
+        const SortPlan plan = make_sort_plan(kr.key_or ^ kr.key_and, n);
         ctx->sort_passes = plan.npasses;
 
         // ---- a2: radix sort of (key, index) ----
-        if (plan.npasses > 0 && !plan.packed) {      // the permutation is stored only when a key window of 32 bits is too narrow
+        if (plan.npasses > 0 && !plan.packed) {      // the permutation is stored only when the key window left beside the index is too narrow
             BH_CUDA(ctx->idxA.ensure(sizeof(u32) * n));
             BH_CUDA(ctx->idxB.ensure(sizeof(u32) * n));
         }
@@ -401,12 +413,12 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
             const bool odd = plan.npasses & 1;
             const u64* kres = odd ? ctx->keysB.as<u64>() : ctx->keysA.as<u64>();
             SortedView& sv = ctx->sv;
-            sv.packed = nullptr; sv.keys = nullptr; sv.idx = nullptr; sv.cbits = 0; sv.lo = 0;
+            sv.packed = nullptr; sv.keys = nullptr; sv.idx = nullptr; sv.cbits = 0; sv.lo = 0; sv.ib = plan.ib;
             if (plan.npasses == 0) sv.keys = kres;                      // identity: all keys equal
             else if (plan.packed) {
                 sv.packed = kres;
                 sv.lo = plan.lo;
-                sv.cbits = kr.key_and & ~(0xffffffffULL << plan.lo);
+                sv.cbits = kr.key_and & ~(((~0ULL) >> plan.ib) << plan.lo);
             } else {
                 sv.keys = kres;
                 sv.idx = odd ? ctx->idxB.as<u32>() : ctx->idxA.as<u32>();
@@ -624,18 +636,46 @@ int bh_essential_nodes(bh_ctx* ctx, const double box_lo[3], const double box_hi[
 
 namespace {
 
+// The Ewald field array of the context's (N, nref): built on first use and whenever the options changed
+// ("calculated once on startup").  Box units, so it does not depend on the cube.
+int ensure_ewald(bh_ctx* ctx)
+{
+    if (ctx->ew_ready_N == ctx->ew_N && ctx->ew_ready_nref == ctx->ew_nref) return BH_OK;
+    const int N = ctx->ew_N, nref = ctx->ew_nref, M = N - 1;
+    const i64 npts = (i64)nref * N * N * N, ncoef = (i64)nref * M * M * M;
+    BH_CUDA(ctx->ew_table.ensure(sizeof(double) * npts));
+    BH_CUDA(ctx->ew_coef.ensure(sizeof(float4) * 3 * ncoef));
+    ewald_table_kernel<<<blocks_for(npts, 128), 128, 0, ctx->stream>>>(N, nref, ctx->ew_table.as<double>());
+    BH_CUDA(cudaGetLastError());
+    ewald_coef_kernel<<<blocks_for(ncoef, 128), 128, 0, ctx->stream>>>(N, nref, ctx->ew_table.as<double>(), ctx->ew_coef.as<float4>());
+    BH_CUDA(cudaGetLastError());
+    ctx->ew_ready_N = N;
+    ctx->ew_ready_nref = nref;
+    return BH_OK;
+}
+
 // Launches the walk of the last build on the context's stream.  count_only: the traversal of
 // walk_pair_kernel<true> (same decisions, no arithmetic on masses), filling ctx->gcount.
 int launch_walk(bh_ctx* ctx, double theta, double G, double* phi, int group, int mac, bool count_only,
-                double* acc = nullptr)
+                double* acc = nullptr, bool periodic = false)
 {
     cudaStream_t st = ctx->stream;
     const i64 n = ctx->n;
+    if (periodic) {
+        // the periodic walk is the group walk for Phi over all cells (no per-target mode, no field, no source-only cells)
+        if (group != 32 || acc || (ctx->ntargets >= 0 && ctx->ntargets < n)) return BH_ERR_INVALID_ARG;
+        int rc = ensure_ewald(ctx);
+        if (rc != BH_OK) return rc;
+    }
     const i64 ngroups = (n + group - 1) / group;
     BH_CUDA(ctx->gcount.ensure(sizeof(uint4) * ngroups));
     BH_CUDA(ctx->geval.ensure(sizeof(u32) * ngroups));
     if (n == 1) {   // T-rule 1: a lone cell has no tree; Phi = 0
-        if (!count_only) BH_CUDA(cudaMemsetAsync(phi, 0, sizeof(double), st));
+        if (!count_only && !periodic) BH_CUDA(cudaMemsetAsync(phi, 0, sizeof(double), st));
+        if (!count_only && periodic) {      // the lone cell still feels its own images (reading P5)
+            periodic_single_kernel<<<1, 1, 0, st>>>(ctx->rec64.as<double4>(), ctx->ew_table.as<double>(), ctx->cube[3], -G, phi);
+            BH_CUDA(cudaGetLastError());
+        }
         if (!count_only && acc) BH_CUDA(cudaMemsetAsync(acc, 0, 3 * sizeof(double), st));
         BH_CUDA(cudaMemsetAsync(ctx->gcount.p, 0, sizeof(uint4), st));
         if (!count_only) BH_CUDA(cudaMemsetAsync(ctx->geval.p, 0, sizeof(u32), st));
@@ -657,6 +697,16 @@ int launch_walk(bh_ctx* ctx, double theta, double G, double* phi, int group, int
     P.negG = -G;
     P.stack_cap = 0;
     P.ntargets = ctx->ntargets < 0 ? 0xffffffffu : (u32)(ctx->ntargets < n ? ctx->ntargets : n);
+    memset(&P.ew, 0, sizeof(P.ew));
+    if (periodic) {
+        P.ew.coef = ctx->ew_coef.as<float4>();
+        P.ew.L = (float)ctx->cube[3];
+        P.ew.invL = (float)(1.0 / ctx->cube[3]);
+        P.ew.s0 = (float)(2.0 * (ctx->ew_N - 2) / ctx->cube[3]);
+        P.ew.top = (float)(ctx->ew_N - 2);
+        P.ew.M = ctx->ew_N - 1;
+        P.ew.nref = ctx->ew_nref;
+    }
     if (group == 32) {
         i64 cap = (i64)kStackPerLevel * (ctx->maxlevel + 2) + 32;
         cap = (cap + 1) & ~1LL;
@@ -665,7 +715,11 @@ int launch_walk(bh_ctx* ctx, double theta, double G, double* phi, int group, int
         P.stack_cap = (int)cap;
         const i64 npairs = (ngroups + 1) / 2;
         const bool subset = P.ntargets != 0xffffffffu;
-        if (count_only && subset)
+        if (periodic && count_only)
+            walk_pair_kernel<true, false, false, true><<<blocks_for(npairs, kWalkWarps), kWalkWarps * 32, smem, st>>>(P);
+        else if (periodic)
+            walk_pair_kernel<false, false, false, true><<<blocks_for(npairs, kWalkWarps), kWalkWarps * 32, smem, st>>>(P);
+        else if (count_only && subset)
             walk_pair_kernel<true, true><<<blocks_for(npairs, kWalkWarps), kWalkWarps * 32, smem, st>>>(P);
         else if (count_only)
             walk_pair_kernel<true><<<blocks_for(npairs, kWalkWarps), kWalkWarps * 32, smem, st>>>(P);
@@ -689,7 +743,7 @@ int launch_walk(bh_ctx* ctx, double theta, double G, double* phi, int group, int
 int ensure_counts(bh_ctx* ctx)
 {
     if (ctx->counts_valid) return BH_OK;
-    int rc = launch_walk(ctx, ctx->walk_theta, 0.0, nullptr, ctx->walk_group, ctx->walk_mac, true);
+    int rc = launch_walk(ctx, ctx->walk_theta, 0.0, nullptr, ctx->walk_group, ctx->walk_mac, true, nullptr, ctx->walk_periodic);
     if (rc == BH_OK) ctx->counts_valid = true;
     return rc;
 }
@@ -708,8 +762,9 @@ static int potential_impl(bh_ctx* ctx, double theta, double G, double* phi, doub
     ctx->launches_walk = 0;
     ctx->walked = false;
     BH_CUDA(cudaEventRecord(ctx->ev[EV_W0], st));
-    int rc = launch_walk(ctx, theta, G, phi, group, ctx->mac, false, acc);
+    int rc = launch_walk(ctx, theta, G, phi, group, ctx->mac, false, acc, ctx->periodic);
     if (rc != BH_OK) return rc;
+    ctx->walk_periodic = ctx->periodic;
     ctx->launches_walk = ctx->n > 1 ? 1 : 0;
     BH_CUDA(cudaEventRecord(ctx->ev[EV_W1], st));
     ctx->ev_walk = true;
@@ -890,6 +945,19 @@ int bh_get_build_passes(bh_ctx* ctx, bh_pass* out, int cap, int* count)
     }
     cudaGetLastError();
     return ctx->npass > cap ? BH_ERR_TOO_LARGE : BH_OK;
+}
+
+int bh_ewald_table(bh_ctx* ctx, double* out, int64_t cap, int* N, int* nref)
+{
+    if (!ctx || cap < 0 || (cap > 0 && !out)) return BH_ERR_INVALID_ARG;
+    BH_CUDA(cudaSetDevice(ctx->device));
+    { int rc = ensure_ewald(ctx); if (rc != BH_OK) return rc; }
+    if (N) *N = ctx->ew_N;
+    if (nref) *nref = ctx->ew_nref;
+    const i64 npts = (i64)ctx->ew_nref * ctx->ew_N * ctx->ew_N * ctx->ew_N;
+    if (cap < npts) return BH_ERR_TOO_LARGE;
+    BH_CUDA(cudaMemcpyAsync(out, ctx->ew_table.p, sizeof(double) * npts, cudaMemcpyDeviceToDevice, ctx->stream));
+    return BH_OK;
 }
 
 int bh_tree_sizes(const bh_ctx* ctx, int64_t* n, int64_t* n_nodes, int64_t* n_slots)

@@ -37,9 +37,10 @@ template <typename T> __device__ __forceinline__ T ld_stream(const T* p) { retur
 template <typename T> __device__ __forceinline__ void st_stream(T* p, T v) { __stcs(p, v); }
 
 // The cells in sorted order (ascending (key, original index)) as the sort leaves them:
-//   packed   : one u64 per cell = (key bits [lo, lo+32) << 32) | original index -- used whenever all
-//              varying key bits fit in 32 (every grid up to 1024^3 and the AMR workloads); cbits holds
-//              the key bits outside that window, which are the same for all cells;
+//   packed   : one u64 per cell = (key bits [lo, lo + 64 - ib) << ib) | original index, ib = ceil(log2 n) index
+//              bits -- used whenever all varying key bits fit in the 64 - ib bits left (40 at 16.8 M cells: every
+//              grid up to 4096^3 and the AMR workloads); cbits holds the key bits outside that window, which are
+//              the same for all cells;
 //   generic  : keys[] + idx[];
 //   identity : all keys equal, nothing was sorted: keys[] as generated, idx(s) = s.
 struct SortedView {
@@ -48,25 +49,26 @@ struct SortedView {
     const u32* idx;
     u64 cbits;
     int lo;
+    int ib;
 };
 __device__ __forceinline__ u64 sv_key(const SortedView& v, i64 s)
 {
-    return v.packed ? (((v.packed[s] >> 32) << v.lo) | v.cbits) : v.keys[s];
+    return v.packed ? (((v.packed[s] >> v.ib) << v.lo) | v.cbits) : v.keys[s];
 }
 __device__ __forceinline__ u32 sv_idx(const SortedView& v, i64 s)
 {
-    return v.packed ? (u32)v.packed[s] : (v.idx ? v.idx[s] : (u32)s);
+    return v.packed ? (u32)(v.packed[s] & ((1ULL << v.ib) - 1ULL)) : (v.idx ? v.idx[s] : (u32)s);
 }
 
 // c(s): octree levels the keys of sorted cells s and s+1 share (s + 1 < n).  In the packed form only the
-// 32-bit key windows differ, so the highest differing key bit is lo + 31 - clz(xor of the windows).
+// key windows differ, so the highest differing key bit is lo + 63 - clz(xor of the windows).
+__device__ __forceinline__ int window_common_levels(u64 x, int lo)     // x = xor of two key windows
+{
+    return x == 0ULL ? kMaxLevel : (__clzll((long long)x) - 1 - lo) / 3;   // (62 - (lo + 63 - clz)) / 3
+}
 __device__ __forceinline__ int sv_common_levels(const SortedView& v, i64 s)
 {
-    if (v.packed) {
-        const u32* w = reinterpret_cast<const u32*>(v.packed);
-        const u32 x = w[2 * s + 1] ^ w[2 * s + 3];
-        return x == 0u ? kMaxLevel : (31 + __clz((int)x) - v.lo) / 3;     // (62 - (lo + 31 - clz)) / 3
-    }
+    if (v.packed) return window_common_levels((v.packed[s] ^ v.packed[s + 1]) >> v.ib, v.lo);
     return common_levels(v.keys[s], v.keys[s + 1]);
 }
 

@@ -69,7 +69,8 @@ struct SortPlan {
     int shift[kMaxPasses];           // bit position of each pass's digit in the 63-bit key
     u32 mask[kMaxPasses];
     int lo;                          // lowest varying key bit
-    bool packed;                     // all varying bits inside [lo, lo + 32)
+    int ib;                          // index bits of the packed word: ceil(log2 n)
+    bool packed;                     // all varying bits inside [lo, lo + 64 - ib)
 };
 
 // ghist[p * pass_stride + d] = number of keys whose digit of pass p is d
@@ -136,7 +137,7 @@ struct SortSmemVals { u32 vals[kSortTile]; };    // generic mode only: the value
 // What one pass reads and writes.
 //   kGenericFirst: reads keys, value = element index;  writes (key, value)
 //   kGeneric     : reads (key, value);                 writes (key, value)
-//   kPackedFirst : reads keys;  writes words (key bits [lo, lo+32) << 32 | element index)
+//   kPackedFirst : reads keys;  writes words (key bits [lo, lo + 64 - ib) << ib | element index)
 //   kPacked      : reads words; writes words
 enum SortMode { kGenericFirst = 0, kGeneric = 1, kPackedFirst = 2, kPacked = 3 };
 
@@ -147,7 +148,7 @@ template <int MODE>
 __global__ void __launch_bounds__(kSortThreads, (MODE >= kPackedFirst ? 4 : 3))
 radix_onesweep_kernel(const u64* __restrict__ kin, const u32* __restrict__ vin, u64* __restrict__ kout,
                       u32* __restrict__ vout, const u32* __restrict__ ghist /* this pass: [256] */,
-                      u32* __restrict__ status, u32* __restrict__ ticket, i64 n, int shift, u32 mask, int lo)
+                      u32* __restrict__ status, u32* __restrict__ ticket, i64 n, int shift, u32 mask, int lo, int ib)
 {
     constexpr bool kVals = MODE == kGenericFirst || MODE == kGeneric;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -244,8 +245,9 @@ radix_onesweep_kernel(const u64* __restrict__ kin, const u32* __restrict__ vin, 
         const u32 qs = q ^ ((q >> 5) & 31u);
         const u32 e32 = (u32)(wbase + i * 32 + lane);
         if (MODE == kPackedFirst) {                         // word = key window | element index
-            S.klo[qs] = e32;
-            S.khi[qs] = (u32)(key[i] >> lo);
+            const u64 word = ((key[i] >> lo) << ib) | (u64)e32;
+            S.klo[qs] = (u32)word;
+            S.khi[qs] = (u32)(word >> 32);
         } else {
             S.klo[qs] = (u32)key[i];
             S.khi[qs] = (u32)(key[i] >> 32);
@@ -256,7 +258,7 @@ radix_onesweep_kernel(const u64* __restrict__ kin, const u32* __restrict__ vin, 
     __syncthreads();
     const i64 left = n - base;
     const int nvalid = left < kSortTile ? (int)left : kSortTile;
-    const int dshift = MODE == kPackedFirst ? shift - lo + 32 : shift;   // the digit inside what was stored
+    const int dshift = MODE == kPackedFirst ? shift - lo + ib : shift;   // the digit inside what was stored
     #pragma unroll 4
     for (int q = tid; q < nvalid; q += kSortThreads) {
         const u32 qs = (u32)q ^ (((u32)q >> 5) & 31u);
@@ -269,16 +271,18 @@ radix_onesweep_kernel(const u64* __restrict__ kin, const u32* __restrict__ vin, 
 }
 
 // passes covering exactly the varying bits [lo_bit, hi_bit] in 8-bit digits
-inline SortPlan make_sort_plan(u64 varying)
+inline SortPlan make_sort_plan(u64 varying, i64 n)
 {
     SortPlan p;
     p.npasses = 0;
     p.lo = 0;
+    p.ib = 1;
+    while ((1LL << p.ib) < n) ++p.ib;
     p.packed = false;
     if (varying == 0) return p;
     int lo = __builtin_ctzll(varying), hi = 63 - __builtin_clzll(varying);
     p.lo = lo;
-    p.packed = hi - lo + 1 <= 32;
+    p.packed = hi - lo + 1 <= 64 - p.ib;
     for (int b = lo; b <= hi; b += 8) {
         int w = hi - b + 1 < 8 ? hi - b + 1 : 8;
         p.shift[p.npasses] = b;
@@ -319,17 +323,17 @@ inline cudaError_t radix_sort_pairs(u64* k0, u32* v0, u64* k1, u32* v1, i64 n, c
         if (plan.packed) {
             if (p == 0)
                 radix_onesweep_kernel<kPackedFirst><<<ntiles, kSortThreads, smem, st>>>(
-                    k0, nullptr, k1, nullptr, blk, status, ticket, n, plan.shift[p], plan.mask[p], plan.lo);
-            else   // the key window sits in the upper half of the word
+                    k0, nullptr, k1, nullptr, blk, status, ticket, n, plan.shift[p], plan.mask[p], plan.lo, plan.ib);
+            else   // the key window sits above the index bits of the word
                 radix_onesweep_kernel<kPacked><<<ntiles, kSortThreads, smem, st>>>(
-                    k0, nullptr, k1, nullptr, blk, status, ticket, n, plan.shift[p] - plan.lo + 32, plan.mask[p], plan.lo);
+                    k0, nullptr, k1, nullptr, blk, status, ticket, n, plan.shift[p] - plan.lo + plan.ib, plan.mask[p], plan.lo, plan.ib);
         } else {
             if (p == 0)
                 radix_onesweep_kernel<kGenericFirst><<<ntiles, kSortThreads, smem, st>>>(
-                    k0, nullptr, k1, v1, blk, status, ticket, n, plan.shift[p], plan.mask[p], plan.lo);
+                    k0, nullptr, k1, v1, blk, status, ticket, n, plan.shift[p], plan.mask[p], plan.lo, plan.ib);
             else
                 radix_onesweep_kernel<kGeneric><<<ntiles, kSortThreads, smem, st>>>(
-                    k0, v0, k1, v1, blk, status, ticket, n, plan.shift[p], plan.mask[p], plan.lo);
+                    k0, v0, k1, v1, blk, status, ticket, n, plan.shift[p], plan.mask[p], plan.lo, plan.ib);
         }
         mark("sort_pass", 24.0 * (double)n);          // 12 B read + 12 B written per pair and pass
         u64* tk = k0; k0 = k1; k1 = tk;

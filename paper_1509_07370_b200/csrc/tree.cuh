@@ -70,24 +70,24 @@ topo_count_kernel(const SortedView sv, i64 n, signed char* __restrict__ clev, u3
     int cprev;                                        // c(wbase - 1)
     const i64 last = n - 1;
     if (sv.packed) {
-        const u32* w = reinterpret_cast<const u32*>(sv.packed);
-        u32 x[kTopoItems];
+        const u64* w = sv.packed;
+        u64 x[kTopoItems];
         if (wbase + kTopoChunk < n) {                  // interior chunk: no clamping (warp-uniform)
-            const u32* wp = w + 2 * (wbase + lane) + 1;
+            const u64* wp = w + wbase + lane;
             #pragma unroll
-            for (int i = 0; i < kTopoItems; ++i) x[i] = wp[64 * i] ^ wp[64 * i + 2];
+            for (int i = 0; i < kTopoItems; ++i) x[i] = (wp[32 * i] ^ wp[32 * i + 1]) >> sv.ib;
         } else {
             #pragma unroll
             for (int i = 0; i < kTopoItems; ++i) {
                 const i64 s = wbase + 32 * i + lane;
                 const i64 s0 = s < last ? s : last, s1 = s + 1 < last ? s + 1 : last;
-                x[i] = w[2 * s0 + 1] ^ w[2 * s1 + 1];
+                x[i] = (w[s0] ^ w[s1]) >> sv.ib;
             }
         }
-        const u32 xp = wbase > 0 ? (w[2 * wbase - 1] ^ w[2 * wbase + 1]) : 0u;
+        const u64 xp = wbase > 0 ? ((w[wbase - 1] ^ w[wbase]) >> sv.ib) : 0ULL;
         #pragma unroll
-        for (int i = 0; i < kTopoItems; ++i) c[i] = x[i] == 0u ? kMaxLevel : (31 + __clz((int)x[i]) - sv.lo) / 3;
-        cprev = xp == 0u ? kMaxLevel : (31 + __clz((int)xp) - sv.lo) / 3;
+        for (int i = 0; i < kTopoItems; ++i) c[i] = window_common_levels(x[i], sv.lo);
+        cprev = window_common_levels(xp, sv.lo);
     } else {
         u64 x[kTopoItems];
         #pragma unroll

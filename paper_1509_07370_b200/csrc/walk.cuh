@@ -32,6 +32,7 @@
 // BH_OPT_GROUP = 1 (W5, the textbook per-target walk) is walk_single_kernel below.
 #pragma once
 #include "common.cuh"
+#include "ewald.cuh"
 #include "tree.cuh"
 
 namespace bh {
@@ -64,6 +65,7 @@ struct WalkParams {
     double negG;
     int stack_cap;            // entries per warp
     u32 ntargets;             // only cells with original index < ntargets are targets (bh_set_num_targets)
+    EwaldTab ew;              // PERIODIC instantiations only: the Ewald field array (ewald.cuh)
 };
 
 __host__ __device__ inline size_t walk_smem_per_warp(int stack_cap)
@@ -271,6 +273,67 @@ __device__ __forceinline__ void eval_c_g(const float4* __restrict__ L, const u32
     gB[0] += (double)gx.y; gB[1] += (double)gy.y; gB[2] += (double)gz.y;
 }
 
+// ---- PERIODIC (App. A): every entry contributes m (1/d + corr1(d_vec/L)/L) = m f_EF (Eq. A.1) -------------------
+// The unchecked lists hold entries already moved to the periodic image nearest the pair of groups, and only
+// entries for which that image is the minimum image for EVERY member, so plain differences are minimum-image
+// displacements.  One entry at a time: the table lookup (three 16-byte loads + nine FMAs) dominates.
+template <int CAP>
+__device__ __forceinline__ void eval_soa2_p(const float* __restrict__ L, int cnt, const float4 tA, const float4 tB,
+                                            const EwaldTab& T, double& accA, double& accB, bool doA, bool doB)
+{
+    float sa = 0.f, sb = 0.f;
+    for (int e = 0; e < cnt; ++e) {
+        const float x = L[e], y = L[CAP + e], z = L[2 * CAP + e], m = L[3 * CAP + e];
+        if (doA) {
+            const float dx = x - tA.x, dy = y - tA.y, dz = z - tA.z;
+            const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmaf_rn(dx, dx, kTinyD2)));
+            sa = __fmaf_rn(m, rsqrt_approx(d2) + ewald_corr(T, dx, dy, dz), sa);
+        }
+        if (doB) {
+            const float dx = x - tB.x, dy = y - tB.y, dz = z - tB.z;
+            const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmaf_rn(dx, dx, kTinyD2)));
+            sb = __fmaf_rn(m, rsqrt_approx(d2) + ewald_corr(T, dx, dy, dz), sb);
+        }
+    }
+    accA += (double)sa;
+    accB += (double)sb;
+}
+
+// checked list under periodic boundaries: explicit minimum image per target; the own cell and zero-distance
+// pairs keep their image / background part m corr1(0)/L (reading P5) and drop only 1/d
+__device__ __forceinline__ void eval_c_p(const float4* __restrict__ L, const u32* __restrict__ Lm, int cnt, const float4 tA,
+                                         const float4 tB, const EwaldTab& T, double& accA, double& accB, u32& evA, u32& evB)
+{
+    float sa = 0.f, sb = 0.f;
+    for (int e = 0; e < cnt; ++e) {
+        const float4 v = L[e];
+        const u32 mk = Lm[e];
+        evA += mk & 1u; evB += mk >> 1;
+        {
+            const float dx = wrap_mi(v.x - tA.x, T.L, T.invL), dy = wrap_mi(v.y - tA.y, T.L, T.invL), dz = wrap_mi(v.z - tA.z, T.L, T.invL);
+            const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx));
+            const float ri = d2 >= 1.17549435e-38f ? rsqrt_approx(d2) : 0.f;
+            if (mk & 1u) sa = __fmaf_rn(v.w, ri + ewald_corr(T, dx, dy, dz), sa);
+        }
+        {
+            const float dx = wrap_mi(v.x - tB.x, T.L, T.invL), dy = wrap_mi(v.y - tB.y, T.L, T.invL), dz = wrap_mi(v.z - tB.z, T.L, T.invL);
+            const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx));
+            const float ri = d2 >= 1.17549435e-38f ? rsqrt_approx(d2) : 0.f;
+            if (mk & 2u) sb = __fmaf_rn(v.w, ri + ewald_corr(T, dx, dy, dz), sb);
+        }
+    }
+    accA += (double)sa;
+    accB += (double)sb;
+}
+
+// packed minimum image: d - L rint(d / L), rint by the 1.5 * 2^23 trick (|d / L| is far below 2^22)
+__device__ __forceinline__ float2 wrap_mi2(float2 d, float L, float invL)
+{
+    const float2 big = splat2(12582912.f);
+    const float2 q = __fadd2_rn(__fadd2_rn(__fmul2_rn(d, splat2(invL)), big), splat2(-12582912.f));
+    return __ffma2_rn(splat2(-L), q, d);
+}
+
 template <int CAP>
 __device__ __forceinline__ void soa_store(float* L, int e, float4 r)
 {
@@ -325,7 +388,13 @@ __device__ __forceinline__ void box_d2(const float4 q, const Box2& b, float2& d2
 // SUBSET = true: only cells with original index < P.ntargets are targets (bh_set_num_targets); the
 //                default instantiation carries none of that code.
 // ACC = true   : bh_field -- additionally g = -grad Phi on the same lists (NEXT-4); its own register budget.
-template <bool COUNT, bool SUBSET = false, bool ACC = false>
+// PERIODIC     : periodic boundaries (App. A, NEXT-3; the cube of the build is the periodic box): every child record
+//                is first moved to the image nearest the centre of the pair's bounding box.  Where that image is the
+//                minimum image for every member (|q' - c|_a + half-width_a < L/2 on all axes) the step runs exactly as
+//                in the isolated case; a child on the seam (half a box away along some axis) takes the per-member test
+//                with an explicit minimum image per member and, if used, goes to the checked list, which wraps per
+//                target.  Every entry is evaluated as m (1/d + corr1/L) with the table lookup of ewald.cuh.
+template <bool COUNT, bool SUBSET = false, bool ACC = false, bool PERIODIC = false>
 __global__ void __launch_bounds__(kWalkWarps * 32, 24 / kWalkWarps)
 walk_pair_kernel(const WalkParams P)
 {
@@ -379,6 +448,18 @@ walk_pair_kernel(const WalkParams P)
     TA.x = splat2(-tA.x); TA.y = splat2(-tA.y); TA.z = splat2(-tA.z);
     TB.x = splat2(-tB.x); TB.y = splat2(-tB.y); TB.z = splat2(-tB.z);
 
+    // PERIODIC: centre and half-widths of the pair's bounding box, the reach within which the image nearest the
+    // centre is every member's minimum image (a relative 1e-5 of L/2 is kept clear for the fp32 roundings)
+    float pcx = 0.f, pcy = 0.f, pcz = 0.f, phx = 0.f, phy = 0.f, phz = 0.f, reach = 0.f;
+    if (PERIODIC) {
+        const float x0 = fminf(box.xl.x, box.xl.y), x1 = fmaxf(box.xh.x, box.xh.y);
+        const float y0 = fminf(box.yl.x, box.yl.y), y1 = fmaxf(box.yh.x, box.yh.y);
+        const float z0 = fminf(box.zl.x, box.zl.y), z1 = fmaxf(box.zh.x, box.zh.y);
+        pcx = 0.5f * (x0 + x1); pcy = 0.5f * (y0 + y1); pcz = 0.5f * (z0 + z1);
+        phx = 0.5f * (x1 - x0); phy = 0.5f * (y1 - y0); phz = 0.5f * (z1 - z0);
+        reach = 0.5f * P.ew.L * (1.0f - 1.0e-5f);
+    }
+
     double accA = 0.0, accB = 0.0;
     double grA[3] = {0.0, 0.0, 0.0}, grB[3] = {0.0, 0.0, 0.0};   // ACC: sums of w (r_j - r_t)
     int nU2 = 0, nUA = 0, nUB = 0, nC = 0;          // list fill (warp-uniform)
@@ -427,6 +508,15 @@ walk_pair_kernel(const WalkParams P)
         if (have) { r = __ldg(rec + slot); t = __ldg(aux + slot); }
         const bool internal = t.w > 0u;
         const bool leaf = have && !internal;
+        bool seam = false;                              // PERIODIC: the nearest image is not every member's minimum image
+        if (PERIODIC) {
+            // r - L rint((r - c)/L): a record that needs no shift stays bit-identical (the own-cell check relies on it)
+            r.x = __fmaf_rn(-P.ew.L, rintf((r.x - pcx) * P.ew.invL), r.x);
+            r.y = __fmaf_rn(-P.ew.L, rintf((r.y - pcy) * P.ew.invL), r.y);
+            r.z = __fmaf_rn(-P.ew.L, rintf((r.z - pcz) * P.ew.invL), r.z);
+            const float ix = r.x - pcx, iy = r.y - pcy, iz = r.z - pcz;
+            seam = have && (fabsf(ix) + phx > reach || fabsf(iy) + phy > reach || fabsf(iz) + phz > reach);
+        }
         // ---- opening test (W-rule 2, fp32 decision W8): r_c = l*(1/theta) [+ delta] ----
         float rc = __fmul_rn(__uint_as_float(t.x), inv_theta);
         if (mac94) rc = __fadd_rn(rc, __uint_as_float(t.y));
@@ -437,6 +527,7 @@ walk_pair_kernel(const WalkParams P)
         if (internal) {
             accm = ((d2min.x > rc2 ? 1u : 0u) | (d2min.y > rc2 ? 2u : 0u)) & msk;     // every member passes
             ambm = ((d2max.x > rc2 ? 1u : 0u) | (d2max.y > rc2 ? 2u : 0u)) & msk & ~accm;
+            if (PERIODIC && seam) { accm = 0u; ambm = msk; }                         // the box bounds do not hold on the seam
         }
         // ---- nodes a box cannot decide: per-member test + vote ----
         const u32 bAmb = __ballot_sync(0xffffffffu, ambm != 0u);
@@ -453,8 +544,11 @@ walk_pair_kernel(const WalkParams P)
             #pragma unroll 4
             for (int i = 0; i < na; ++i) {
                 const float4 q = amb[i];
-                const float2 dx = __fadd2_rn(splat2(q.x), npx), dy = __fadd2_rn(splat2(q.y), npy),
-                             dz = __fadd2_rn(splat2(q.z), npz);
+                float2 dx = __fadd2_rn(splat2(q.x), npx), dy = __fadd2_rn(splat2(q.y), npy),
+                       dz = __fadd2_rn(splat2(q.z), npz);
+                if (PERIODIC) {                           // the member's own minimum image (a no-op off the seam)
+                    dx = wrap_mi2(dx, P.ew.L, P.ew.invL); dy = wrap_mi2(dy, P.ew.L, P.ew.invL); dz = wrap_mi2(dz, P.ew.L, P.ew.invL);
+                }
                 const float2 d2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
                 failA = __funnelshift_l(__float_as_uint(d2.x) + __float_as_uint(q.w), failA, 1);
                 failB = __funnelshift_l(__float_as_uint(d2.y) + __float_as_uint(q.w), failB, 1);
@@ -481,8 +575,10 @@ walk_pair_kernel(const WalkParams P)
         }
         // ---- append accepted nodes and leaf cells to the lists ----
         // leaf cells inside a group's box may be a target's own cell or coincide with one
-        const bool danger = leaf && (((msk & 1u) && !(d2min.x > 0.f)) || ((msk & 2u) && !(d2min.y > 0.f)));
-        const u32 um = internal ? accm : (danger ? 0u : msk);           // 3: both groups, 1: A only, 2: B only
+        const u32 cmask = internal ? accm : msk;                        // groups that take this child as a list entry
+        const bool danger = (leaf && (((msk & 1u) && !(d2min.x > 0.f)) || ((msk & 2u) && !(d2min.y > 0.f)))) ||
+                            (PERIODIC && seam && cmask != 0u);           // seam entries are wrapped per target
+        const u32 um = danger ? 0u : cmask;                             // 3: both groups, 1: A only, 2: B only
         const u32 b1 = __ballot_sync(0xffffffffu, um & 1u);
         const u32 b2 = __ballot_sync(0xffffffffu, um & 2u);
         const u32 same = ((um & 1u) ? b1 : ~b1) & ((um & 2u) ? b2 : ~b2);   // lanes that append to the same list
@@ -494,7 +590,7 @@ walk_pair_kernel(const WalkParams P)
         nU2 += cU2; nUA += cUA; nUB += cUB;
         const u32 bC = __ballot_sync(0xffffffffu, danger);
         if (bC) {                                                       // rare: only next to the groups' own cells
-            if (danger) { const int at = nC + __popc(bC & lt); C[at] = r; Cm[at] = msk; }
+            if (danger) { const int at = nC + __popc(bC & lt); C[at] = r; Cm[at] = cmask; }
             nC += __popc(bC);
         }
         __syncwarp();
@@ -503,7 +599,8 @@ walk_pair_kernel(const WalkParams P)
             if (nU2 >= kU2Cap - kStepMax) {
                 soa_pad<kSoaCap>(U2, nU2);
                 __syncwarp();
-                if (ACC) eval_soa2_g<kSoaCap>(U2, nU2, TA, TB, accA, accB, grA, grB);
+                if (PERIODIC) eval_soa2_p<kSoaCap>(U2, nU2, tA, tB, P.ew, accA, accB, true, true);
+                else if (ACC) eval_soa2_g<kSoaCap>(U2, nU2, TA, TB, accA, accB, grA, grB);
                 else eval_soa2<kSoaCap>(U2, nU2, TA, TB, accA, accB);
                 evA += (u32)nU2; evB += (u32)nU2;
                 nU2 = 0;
@@ -511,19 +608,22 @@ walk_pair_kernel(const WalkParams P)
             if (nUA >= kU1Cap - kStepMax) {
                 soa_pad<kSoaCap>(UA, nUA);
                 __syncwarp();
-                accA += ACC ? eval_soa_g<kSoaCap>(UA, nUA, TA, grA) : eval_soa<kSoaCap>(UA, nUA, TA);
+                if (PERIODIC) eval_soa2_p<kSoaCap>(UA, nUA, tA, tB, P.ew, accA, accB, true, false);
+                else accA += ACC ? eval_soa_g<kSoaCap>(UA, nUA, TA, grA) : eval_soa<kSoaCap>(UA, nUA, TA);
                 evA += (u32)nUA;
                 nUA = 0;
             }
             if (nUB >= kU1Cap - kStepMax) {
                 soa_pad<kSoaCap>(UB, nUB);
                 __syncwarp();
-                accB += ACC ? eval_soa_g<kSoaCap>(UB, nUB, TB, grB) : eval_soa<kSoaCap>(UB, nUB, TB);
+                if (PERIODIC) eval_soa2_p<kSoaCap>(UB, nUB, tA, tB, P.ew, accA, accB, false, true);
+                else accB += ACC ? eval_soa_g<kSoaCap>(UB, nUB, TB, grB) : eval_soa<kSoaCap>(UB, nUB, TB);
                 evB += (u32)nUB;
                 nUB = 0;
             }
             if (nC >= kCCap - kStepMax) {
-                if (ACC) eval_c_g(C, Cm, nC, npx, npy, npz, accA, accB, grA, grB, evA, evB);
+                if (PERIODIC) eval_c_p(C, Cm, nC, tA, tB, P.ew, accA, accB, evA, evB);
+                else if (ACC) eval_c_g(C, Cm, nC, npx, npy, npz, accA, accB, grA, grB, evA, evB);
                 else eval_c(C, Cm, nC, npx, npy, npz, accA, accB, evA, evB);
                 nC = 0;
             }
@@ -544,21 +644,25 @@ walk_pair_kernel(const WalkParams P)
     if (nU2 > 0) {
         soa_pad<kSoaCap>(U2, nU2);
         __syncwarp();
-        if (ACC) eval_soa2_g<kSoaCap>(U2, nU2, TA, TB, accA, accB, grA, grB);
+        if (PERIODIC) eval_soa2_p<kSoaCap>(U2, nU2, tA, tB, P.ew, accA, accB, true, true);
+        else if (ACC) eval_soa2_g<kSoaCap>(U2, nU2, TA, TB, accA, accB, grA, grB);
         else eval_soa2<kSoaCap>(U2, nU2, TA, TB, accA, accB);
     }
     if (nUA > 0) {
         soa_pad<kSoaCap>(UA, nUA);
         __syncwarp();
-        accA += ACC ? eval_soa_g<kSoaCap>(UA, nUA, TA, grA) : eval_soa<kSoaCap>(UA, nUA, TA);
+        if (PERIODIC) eval_soa2_p<kSoaCap>(UA, nUA, tA, tB, P.ew, accA, accB, true, false);
+        else accA += ACC ? eval_soa_g<kSoaCap>(UA, nUA, TA, grA) : eval_soa<kSoaCap>(UA, nUA, TA);
     }
     if (nUB > 0) {
         soa_pad<kSoaCap>(UB, nUB);
         __syncwarp();
-        accB += ACC ? eval_soa_g<kSoaCap>(UB, nUB, TB, grB) : eval_soa<kSoaCap>(UB, nUB, TB);
+        if (PERIODIC) eval_soa2_p<kSoaCap>(UB, nUB, tA, tB, P.ew, accA, accB, false, true);
+        else accB += ACC ? eval_soa_g<kSoaCap>(UB, nUB, TB, grB) : eval_soa<kSoaCap>(UB, nUB, TB);
     }
     if (nC > 0) {
-        if (ACC) eval_c_g(C, Cm, nC, npx, npy, npz, accA, accB, grA, grB, evA, evB);
+        if (PERIODIC) eval_c_p(C, Cm, nC, tA, tB, P.ew, accA, accB, evA, evB);
+        else if (ACC) eval_c_g(C, Cm, nC, npx, npy, npz, accA, accB, grA, grB, evA, evB);
         else eval_c(C, Cm, nC, npx, npy, npz, accA, accB, evA, evB);
     }
     // the kernel answers for its own lists: entries it evaluated for each group (= accepted + leaf of W6)

@@ -1,0 +1,177 @@
+"""GPU parity for NEXT-3 (Appendix A): periodic boundaries -- the Ewald field
+array and the periodic group walk of libbh against the fp64 oracle (oracle/bh_oracle.c, orc_ewald_* and
+orc_potential_periodic, pinned in tests/test_oracle_ewald.py).
+
+Bars.  The field array (fp64 on both sides, different alpha and series lengths): 1e-11 absolute.  Phi: a
+periodic potential has zero mean -- its values are what is left of a cancellation -- so the relative error is
+taken against max(|Phi_i|, G M / L): 1e-4 max / 1e-6 median on the groups whose lists agree with
+the oracle's (criterion in fp64 there, fp32 in the kernel: flipped groups are counted, reported and held to the
+tree code's own error).  The periodic mode has no fp32-decision twin in the oracle, so there is no flip-free
+secondary comparison; the count-only repeat and the Phi kernel's own entry counts must still agree."""
+import numpy as np
+import pytest
+
+import bh_workloads as wl
+from tests import parity
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def bh():
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import paper_1509_07370_b200 as pkg
+    return pkg
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).cuda()
+
+
+N_TAB, NREF = 34, 2
+
+
+@pytest.fixture(scope="module")
+def table(oracle):
+    return oracle.EwaldTable(N=N_TAB, nref=NREF)
+
+
+def _ctx(bh, w, nref=NREF):
+    ctx = bh.Context(0)
+    ctx.set_periodic(True, N=N_TAB, nref=nref)
+    ctx.build(_dev(w.x), _dev(w.y), _dev(w.z), _dev(w.m), w.cube)
+    return ctx
+
+
+def test_field_array_equals_oracle(bh, oracle, table):
+    ctx = bh.Context(0)
+    ctx.set_periodic(True, N=N_TAB, nref=NREF)
+    got = ctx.ewald_table().cpu().numpy().reshape(-1)
+    assert got.shape == table.data.shape
+    assert np.max(np.abs(got - table.data)) <= 1e-11
+    assert abs(got[0] + 2.8372974795) <= 1e-9                      # the simple-cubic constant at u = 0
+
+
+def _check(ctx, ot, w, table, theta, mac=0, max_tol=1e-4, med_tol=1e-6):
+    ctx.set_mac(mac)
+    phi = ctx.potential(theta, w.G).cpu().numpy()
+    cnt = ctx.last_group_counts().cpu().numpy()
+    ev = ctx.last_group_evaluated().cpu().numpy().astype(np.int64)
+    ref, c64 = ot.potential_periodic(theta, table, G=w.G, mac=mac, want_counts=True)
+    assert np.array_equal(ev, cnt[:, 0] + cnt[:, 1])               # the Phi kernel's own lists = the count-only repeat
+    flipped = np.any(cnt != c64, axis=1)
+    perm = ot.sorted_keys_perm()[1].astype(np.int64)
+    inv = np.empty(w.n, dtype=np.int64)
+    inv[perm] = np.arange(w.n)
+    tflip = flipped[inv // 32]
+    scale = np.maximum(np.abs(ref), abs(w.G) * np.abs(w.m).sum() / w.cube[3])
+    rel = np.abs(phi - ref) / scale
+    keep = ~tflip
+    print(f"periodic parity {w.name} theta={theta} mac={mac}: {len(flipped)} groups, {int(flipped.sum())} flips fp32-vs-fp64, "
+          f"max rel {rel[keep].max():.2e}, median {np.median(rel[keep]):.2e}")
+    assert flipped.mean() <= parity.FLIP_CEILING + 1.0 / len(flipped)
+    assert rel[keep].max() <= max_tol and np.median(rel[keep]) <= med_tol, (rel[keep].max(), np.median(rel[keep]))
+    assert keep.all() or rel[~keep].max() <= parity.tree_tol(theta)
+    return phi
+
+
+CASES = [wl.turbulent_medium(16), wl.amr_collapsing_core(nroot=2, max_level=3), wl.random_points(4099, seed=2),
+         wl.clustered_points(3000, seed=3), wl.with_duplicates(wl.random_points(500, seed=4), 40, seed=4),
+         wl.random_points(33, seed=8), wl.random_points(2, seed=7)]
+
+
+@pytest.mark.parametrize("mac", [0, 1], ids=["eq3", "eq4"])
+@pytest.mark.parametrize("theta", [0.5, 0.3, 1.0])
+@pytest.mark.parametrize("w", CASES, ids=lambda w: w.name)
+def test_periodic_phi_vs_oracle(bh, oracle, table, w, theta, mac):
+    ctx = _ctx(bh, w)
+    ot = oracle.OracleTree(w.x, w.y, w.z, w.m, w.cube)
+    _check(ctx, ot, w, table, theta, mac)
+
+
+def test_uniform_periodic_grid_closed_form(bh):
+    """16^3 equal masses in a periodic box = a simple cubic lattice of spacing L/16: Phi_i = +2.8372974795 G m 16 / L
+    at every cell (theta = 0: every cell is summed through the table)."""
+    ng = 16
+    x, y, z = wl._grid_centres(ng)
+    L, m = 2.0, 0.37
+    w = wl.Workload("pgrid16", x * L - 1.0, y * L - 1.0, z * L - 1.0, np.full(x.size, m), cube=(-1.0, -1.0, -1.0, L))
+    ctx = bh.Context(0)
+    ctx.set_periodic(True, N=66, nref=1)
+    ctx.build(_dev(w.x), _dev(w.y), _dev(w.z), _dev(w.m), w.cube)
+    phi = ctx.potential(0.0, 1.0).cpu().numpy()
+    exact = 2.8372974795 * m * ng / L
+    assert np.max(np.abs(phi - exact)) <= 1e-4 * exact, (phi[:3], exact)
+    assert np.ptp(phi) <= 1e-5 * exact
+
+
+def test_translation_invariance_and_isolated_differs(bh, oracle, table):
+    w = wl.clustered_points(3000, seed=3)
+    L = float(w.cube[3])
+    ctx = _ctx(bh, w)
+    phi = ctx.potential(0.4, w.G).cpu().numpy()
+    pos = np.stack([w.x, w.y, w.z], 1)
+    p2 = np.mod(pos - w.cube[:3] + np.array([0.37, 0.81, 0.12]) * L, L) + w.cube[:3]
+    w2 = wl.Workload("shifted", p2[:, 0], p2[:, 1], p2[:, 2], w.m, cube=w.cube)
+    phi2 = _ctx(bh, w2).potential(0.4, w.G).cpu().numpy()
+    scale = w.G * w.m.sum() / L
+    # the groups and hence the lists change with the shift: agreement at the tree code's own error
+    assert np.max(np.abs(phi2 - phi) / np.maximum(np.abs(phi), scale)) <= 5e-3
+    ctx.set_periodic(False)
+    iso = ctx.potential(0.4, w.G).cpu().numpy()
+    assert np.max(np.abs(iso - phi)) > 1e-1 * scale
+    ref_iso = oracle.OracleTree(w.x, w.y, w.z, w.m, w.cube)
+    parity.check_walk(ctx, ref_iso, w, 0.4)                        # switching the option off restores the isolated walk
+
+
+def test_periodic_edge_cases(bh, oracle, table):
+    one = wl.random_points(1, seed=9)
+    ctx = _ctx(bh, one)
+    phi = ctx.potential(0.5, 1.0).cpu().numpy()
+    assert phi[0] == pytest.approx(2.8372974795 * one.m[0] / one.cube[3], rel=1e-9)      # its own images
+    w = wl.random_points(300, seed=10)
+    ctx = _ctx(bh, w)
+    ctx.set_group(1)
+    with pytest.raises(bh.BHError):
+        ctx.potential(0.5)                                          # no per-target mode under periodic boundaries
+    ctx.set_group(32)
+    with pytest.raises(bh.BHError):
+        ctx.field(0.5)
+    ctx.set_num_targets(100)
+    with pytest.raises(bh.BHError):
+        ctx.potential(0.5)
+    ctx.set_num_targets(-1)
+    with pytest.raises(bh.BHError):
+        ctx.set_option(bh.binding.BH_OPT_EWALD_N, 3)
+    ot = oracle.OracleTree(w.x, w.y, w.z, w.m, w.cube)
+    _check(ctx, ot, w, table, 0.5)
+
+
+def test_periodic_turb128_sampled(bh, oracle):
+    """A 2 M-cell periodic box (the turbulent medium is generated periodic): sampled groups against the oracle."""
+    w = wl.turbulent_medium(128)
+    tab = oracle.EwaldTable(N=66, nref=1)
+    ctx = bh.Context(0)
+    ctx.set_periodic(True, N=66, nref=1)
+    ctx.build(_dev(w.x), _dev(w.y), _dev(w.z), _dev(w.m), w.cube)
+    phi = ctx.potential(0.5, w.G).cpu().numpy()
+    cnt = ctx.last_group_counts().cpu().numpy()
+    ot = oracle.OracleTree(w.x, w.y, w.z, w.m, w.cube)
+    perm = ot.sorted_keys_perm()[1].astype(np.int64)
+    scale0 = w.G * w.m.sum() / w.cube[3]
+    buf = np.full(w.n, np.nan)
+    rels, flips, ng = [], 0, 0
+    for g0, g1 in parity.sample_runs((w.n + 31) // 32, 12, 8):
+        _, c64 = ot.potential_periodic(0.5, tab, G=w.G, groups=(g0, g1), want_counts=True, out=buf)
+        fl = np.any(cnt[g0:g1] != c64, axis=1)
+        flips += int(fl.sum()); ng += g1 - g0
+        for g in range(g0, g1):
+            if not fl[g - g0]:
+                tg = perm[32 * g:32 * g + 32]
+                rels.append(np.abs(phi[tg] - buf[tg]) / np.maximum(np.abs(buf[tg]), scale0))
+    rel = np.concatenate(rels)
+    print(f"periodic turb128: {ng} groups, {flips} flips, max rel {rel.max():.2e}, median {np.median(rel):.2e}")
+    assert flips <= 0.05 * ng + 1 and rel.max() <= 1e-4 and np.median(rel) <= 1e-6
