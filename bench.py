@@ -233,6 +233,44 @@ def run_reference(args):
     return 0
 
 
+def run_workloads_table(args):
+    """--workloads-table: the five BASELINE.json workloads (config 4 = theta sweep on the AMR grid) on one GPU, one
+    markdown row each: absolute numbers and achieved fraction of roofline (north_star)."""
+    import numpy as np
+    import torch
+    import bh_workloads as wl
+    import paper_1509_07370_b200 as bh
+    hbm_gbs, sm_max_mhz, _ = _peaks()
+    peak = st_sms(0) * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
+    rows = [("sphere32", 0.5), ("maclaurin128", 0.5), ("amr_core", 0.5), ("turb256", 0.5),
+            ("amr_core", 0.3), ("amr_core", 0.7), ("amr_core", 1.0)]
+    print("| workload | cells | theta | build ms | build B/cell | build % HBM | walk ms | interactions/target | interactions/s | walk % FP32 | cells/s (build+walk) |")
+    print("|---|---:|---:|---:|---:|---:|---:|---:|---:|---:|---:|")
+    cache = {}
+    for name, theta in rows:
+        if name not in cache:
+            w = wl.by_name(name)
+            cache = {name: (w, [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (w.x, w.y, w.z, w.m)])}
+        w, d = cache[name]
+        ctx = bh.Context(0)
+        phi = torch.empty(w.n, dtype=torch.float64, device="cuda")
+        tb, tw = [], []
+        for r in range(args.warmup + args.steps):
+            e = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+            e[0].record(); ctx.build(*d, w.cube); e[1].record(); ctx.potential(theta, w.G, out=phi); e[2].record()
+            torch.cuda.synchronize()
+            if r >= args.warmup:
+                tb.append(e[0].elapsed_time(e[1])); tw.append(e[1].elapsed_time(e[2]))
+        st = ctx.get_stats()
+        b, t = statistics.median(tb), statistics.median(tw)
+        bpc = build_bytes_per_cell(w.n, st.n_nodes, st.sort_passes)
+        print(f"| {name} | {w.n} | {theta} | {b:.3f} | {bpc:.1f} | {100 * bpc * w.n / (b * 1e-3) / 1e9 / hbm_gbs:.1f} | {t:.3f} | "
+              f"{st.interactions / w.n:.1f} | {st.interactions / (t * 1e-3):.3e} | "
+              f"{100 * st.interactions * FLOPS_PER_INTERACTION / (t * 1e-3) / 1e12 / peak:.1f} | {w.n / ((b + t) * 1e-3):.3e} |")
+        ctx.close()
+    return 0
+
+
 def run_ours(args):
     import numpy as np
     import torch
@@ -376,6 +414,25 @@ def run_ours(args):
     torch.cuda.synchronize()
     t_field = ra.elapsed_time(rb) / args.steps / 1e3
 
+    # ---- NEXT-3: the same cells in a PERIODIC box (App. A): minimum-image walk + Ewald field lookup per interaction ----
+    pctx = bh.Context(local)
+    pctx.set_periodic(True)
+    pctx.build(*d, w.cube)
+    pphi_dev = pctx.potential(w.theta, w.G)                # builds the field array (once per context) and warms up
+    torch.cuda.synchronize()
+    ra.record()
+    pphi_dev = pctx.potential(w.theta, w.G)
+    rb.record()
+    torch.cuda.synchronize()
+    t_periodic = ra.elapsed_time(rb) / 1e3
+    pst = pctx.get_stats()
+    periodic_info = {"ms_walk": t_periodic * 1e3, "interactions_per_s": world * pst.interactions / t_periodic,
+                     "interactions_per_target": pst.interactions / n, "ewald_grid_points_per_axis": 66, "ewald_nested_grids": 1,
+                     "slowdown_vs_isolated_walk": t_periodic / t_walk,
+                     "note": "every interaction adds a quadratic table lookup (3 x 16 B loads + 9 FMAs) to the 13-flop kernel"}
+    del pphi_dev
+    pctx.close()
+
     # ---- optional (--let-domains P): the locally-essential-tree solve of P x-slab domains, one after the other on
     # this GPU (paper_1509_07370_b200/let.py, let_potential_serial): what a P-GPU run computes, without the exchange ----
     let_info = None
@@ -452,6 +509,7 @@ def run_ours(args):
         "field": {"ms_walk": t_field * 1e3, "interactions_per_s": world * st.interactions / t_field,
                   "flops_per_interaction": 22, "frac_fp32": st.interactions * 22 / t_field / 1e12 / (
                       st_sms(local) * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12)},
+        "periodic": periodic_info,
         "essential_nodes": {"box": "face-neighbour cube of the same size", "theta": w.theta, "mac": "eq4",
                             "entries": n_ess, "ms": t_ess * 1e3},
         "build_passes_ms": {"keys": st.ms_keys, "sort": st.ms_sort, "count": st.ms_count,
@@ -548,11 +606,15 @@ def main():
     ap.add_argument("--theta", type=float, default=0.5)
     ap.add_argument("--ref-groups", type=int, default=4096, help="groups the oracle walks per step (sample)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--workloads-table", action="store_true",
+                    help="print one markdown row per BASELINE workload (build / walk times and roofline fractions) instead of the JSON line")
     ap.add_argument("--let-domains", type=int, default=0,
                     help="also run the locally-essential-tree solve of this many slab domains serially on the GPU")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.workloads_table:
+        return run_workloads_table(args)
     return run_ours(args)
 
 

@@ -282,6 +282,7 @@ __device__ __forceinline__ void eval_soa2_p(const float* __restrict__ L, int cnt
                                             const EwaldTab& T, double& accA, double& accB, bool doA, bool doB)
 {
     float sa = 0.f, sb = 0.f;
+    #pragma unroll 2
     for (int e = 0; e < cnt; ++e) {
         const float x = L[e], y = L[CAP + e], z = L[2 * CAP + e], m = L[3 * CAP + e];
         if (doA) {
