@@ -50,7 +50,6 @@ struct DeviceScalars {          // small device-resident results read back by th
 enum { EV_B0, EV_KEYS, EV_SORT, EV_PERM, EV_TOPO, EV_MOM, EV_W0, EV_W1,
        EV_H0, EV_HC0, EV_HXYZ, EV_HM, EV_HD0, EV_HD1, EV_HEND, EV_COUNT };   // EV_H*: bh_solve_host
 
-constexpr size_t kStageChunk = 16u << 20;      // pinned staging chunk of bh_solve_host for pageable callers
 
 }  // namespace
 
@@ -106,8 +105,6 @@ struct bh_ctx {
     cudaStream_t copy_stream = nullptr;   // bh_solve_host: the host->device copies run beside the build
     cudaEvent_t assign_wait = nullptr;    // set by bh_solve_host: the masses land after the positions; the first kernel
                                           // that reads m (the assigning kernel) waits for this event
-    void* pinned[2] = {nullptr, nullptr}; // two staging chunks for pageable host buffers
-    cudaEvent_t pinned_ev[2] = {nullptr, nullptr};
     bool host_timed = false;
 
     cudaEvent_t ev[EV_COUNT] = {nullptr};
@@ -304,10 +301,6 @@ int bh_destroy(bh_ctx* ctx)
     for (DevBuf* b : all) b->release();
     if (ctx->h_scalars) cudaFreeHost(ctx->h_scalars);
     if (ctx->copy_stream) { cudaStreamSynchronize(ctx->copy_stream); cudaStreamDestroy(ctx->copy_stream); }
-    for (int i = 0; i < 2; ++i) {
-        if (ctx->pinned[i]) cudaFreeHost(ctx->pinned[i]);
-        if (ctx->pinned_ev[i]) cudaEventDestroy(ctx->pinned_ev[i]);
-    }
     for (int i = 0; i < EV_COUNT; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
     for (int i = 0; i < bh_ctx::kMaxPasses; ++i) if (ctx->pev[i]) cudaEventDestroy(ctx->pev[i]);
     delete ctx;
@@ -821,57 +814,18 @@ int bh_potential_direct(bh_ctx* ctx, double G, const int64_t* targets, int64_t n
 
 namespace {
 
-bool is_pinned(const void* p)
-{
-    cudaPointerAttributes a;
-    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
-    return a.type == cudaMemoryTypeHost || a.type == cudaMemoryTypeManaged;
-}
-
-int ensure_pinned_chunks(bh_ctx* ctx)
-{
-    for (int i = 0; i < 2; ++i) {
-        if (!ctx->pinned[i]) BH_CUDA(cudaMallocHost(&ctx->pinned[i], kStageChunk));
-        if (!ctx->pinned_ev[i]) BH_CUDA(cudaEventCreateWithFlags(&ctx->pinned_ev[i], cudaEventDisableTiming));
-    }
-    return BH_OK;
-}
-
-// host -> device on `st`.  Pinned sources go in one asynchronous copy; pageable ones are staged through two
-// pinned chunks so that the CPU's memcpy of chunk k+1 runs beside the DMA of chunk k.
+// host -> device / device -> host on `st`.  Pinned buffers are copied by one asynchronous DMA; for pageable ones the
+// runtime stages the copy itself.  (Staging pageable buffers here through two pinned 16 MB chunks, the CPU's memcpy of
+// one chunk beside the DMA of the other, was measured against that on turb256: 78 ms per call against 71 ms -- the CPU
+// copy at ~11 GB/s bounds both, and the runtime's device -> host path is twice as fast -- so it was dropped.)
 int h2d(bh_ctx* ctx, void* dst, const void* src, size_t bytes, cudaStream_t st)
 {
-    if (is_pinned(src)) { BH_CUDA(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, st)); return BH_OK; }
-    { int rc = ensure_pinned_chunks(ctx); if (rc != BH_OK) return rc; }
-    int k = 0;
-    for (size_t off = 0; off < bytes; off += kStageChunk, k ^= 1) {
-        const size_t len = bytes - off < kStageChunk ? bytes - off : kStageChunk;
-        BH_CUDA(cudaEventSynchronize(ctx->pinned_ev[k]));            // the chunk's previous DMA is done
-        memcpy(ctx->pinned[k], static_cast<const char*>(src) + off, len);
-        BH_CUDA(cudaMemcpyAsync(static_cast<char*>(dst) + off, ctx->pinned[k], len, cudaMemcpyHostToDevice, st));
-        BH_CUDA(cudaEventRecord(ctx->pinned_ev[k], st));
-    }
+    BH_CUDA(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, st));
     return BH_OK;
 }
-
-// device -> host on `st`, complete on return for pageable destinations (staged the same way)
 int d2h(bh_ctx* ctx, void* dst, const void* src, size_t bytes, cudaStream_t st)
 {
-    if (is_pinned(dst)) { BH_CUDA(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, st)); return BH_OK; }
-    { int rc = ensure_pinned_chunks(ctx); if (rc != BH_OK) return rc; }
-    const size_t nchunk = (bytes + kStageChunk - 1) / kStageChunk;
-    for (size_t c = 0; c <= nchunk; ++c) {           // DMA of chunk c runs beside the CPU's memcpy of chunk c - 1
-        if (c < nchunk) {
-            const size_t off = c * kStageChunk, len = bytes - off < kStageChunk ? bytes - off : kStageChunk;
-            BH_CUDA(cudaMemcpyAsync(ctx->pinned[c & 1], static_cast<const char*>(src) + off, len, cudaMemcpyDeviceToHost, st));
-            BH_CUDA(cudaEventRecord(ctx->pinned_ev[c & 1], st));
-        }
-        if (c > 0) {
-            const size_t off = (c - 1) * kStageChunk, len = bytes - off < kStageChunk ? bytes - off : kStageChunk;
-            BH_CUDA(cudaEventSynchronize(ctx->pinned_ev[(c - 1) & 1]));
-            memcpy(static_cast<char*>(dst) + off, ctx->pinned[(c - 1) & 1], len);
-        }
-    }
+    BH_CUDA(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, st));
     return BH_OK;
 }
 
