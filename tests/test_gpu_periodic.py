@@ -87,6 +87,8 @@ CASES = [wl.turbulent_medium(16), wl.amr_collapsing_core(nroot=2, max_level=3), 
 @pytest.mark.parametrize("theta", [0.5, 0.3, 1.0])
 @pytest.mark.parametrize("w", CASES, ids=lambda w: w.name)
 def test_periodic_phi_vs_oracle(bh, oracle, table, w, theta, mac):
+    if w.n > 100000 and (theta != 0.5 or mac != 0):
+        pytest.skip("the oracle's periodic walk of the 233 k-cell AMR grid takes ~10 s: one (theta, criterion) there")
     ctx = _ctx(bh, w)
     ot = oracle.OracleTree(w.x, w.y, w.z, w.m, w.cube)
     _check(ctx, ot, w, table, theta, mac)
