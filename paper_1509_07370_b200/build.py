@@ -10,6 +10,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libbh.so")
+CHECKED_LIB = os.path.join(HERE, "libbh_checked.so")   # -DBH_CHECKED: device-side bounds checks (tests/test_gpu_checked.py)
 PEAK_LIB = os.path.join(HERE, "libbh_fma_peak.so")      # bench.py's measured FP32 denominator; not part of libbh
 PEAK_SRC = os.path.join(CSRC, "fma_peak.cu")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
@@ -44,6 +45,13 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_checked(force: bool = False) -> str:
+    """The same library with -DBH_CHECKED: every index the kernels compute is bounds-checked on the device."""
+    if force or not os.path.exists(CHECKED_LIB) or any(os.path.getmtime(s) > os.path.getmtime(CHECKED_LIB) for s in sources()):
+        subprocess.check_call([_nvcc()] + NVCC_FLAGS + ["-DBH_CHECKED", "-o", CHECKED_LIB, os.path.join(CSRC, "bh.cu")])
+    return CHECKED_LIB
+
+
 def build_fma_peak(force: bool = False) -> str:
     """The FMA-chain peak measurement bench.py reports beside the nominal FP32 peak (its own small library)."""
     if force or not os.path.exists(PEAK_LIB) or os.path.getmtime(PEAK_LIB) < os.path.getmtime(PEAK_SRC):
@@ -51,6 +59,14 @@ def build_fma_peak(force: bool = False) -> str:
     return PEAK_LIB
 
 
+if os.environ.get("BH_CHECKED") == "1":       # debugging aid: the binding loads the checked build instead
+    LIB = CHECKED_LIB
+    build = build_checked                         # noqa: F811
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
-    print(build_fma_peak(force="--force" in sys.argv))
+    if "--checked" in sys.argv:
+        print(build_checked(force="--force" in sys.argv))
+    else:
+        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+        print(build_fma_peak(force="--force" in sys.argv))

@@ -690,6 +690,7 @@ int launch_walk(bh_ctx* ctx, double theta, double G, double* phi, int group, int
     P.negG = -G;
     P.stack_cap = 0;
     P.ntargets = ctx->ntargets < 0 ? 0xffffffffu : (u32)(ctx->ntargets < n ? ctx->ntargets : n);
+    P.nslots = (u32)ctx->nslots;
     memset(&P.ew, 0, sizeof(P.ew));
     if (periodic) {
         P.ew.coef = ctx->ew_coef.as<float4>();

@@ -7,6 +7,17 @@
 #error "libbh is written for sm_100a (B200); compile with -gencode arch=compute_100a,code=sm_100a"
 #endif
 
+// Checked build (`python -m paper_1509_07370_b200.build --checked` -> libbh_checked.so, -DBH_CHECKED): bounds checks
+// of our own on every index the kernels compute -- stack and list fills of the walk, slots, node ids, sort positions.
+// compute-sanitizer is not available on this GPU pool, so tests/test_gpu_checked.py runs the small parity cases
+// through this library in a subprocess; a failed check traps the kernel and the call returns BH_ERR_CUDA.
+#ifdef BH_CHECKED
+#include <assert.h>
+#define BH_DCHECK(cond) assert(cond)
+#else
+#define BH_DCHECK(cond) ((void)0)
+#endif
+
 namespace bh {
 
 typedef unsigned long long u64;

@@ -242,6 +242,7 @@ radix_onesweep_kernel(const u64* __restrict__ kin, const u32* __restrict__ vin, 
     for (int i = 0; i < kSortItems; ++i) {
         const u32 d = (u32)(key[i] >> shift) & mask;
         const u32 q = S.dstart[d] + S.wcnt[warp][d] + rank[i];
+        BH_DCHECK(q < (u32)kSortTile);
         const u32 qs = q ^ ((q >> 5) & 31u);
         const u32 e32 = (u32)(wbase + i * 32 + lane);
         if (MODE == kPackedFirst) {                         // word = key window | element index
@@ -265,6 +266,7 @@ radix_onesweep_kernel(const u64* __restrict__ kin, const u32* __restrict__ vin, 
         const u64 k = ((u64)S.khi[qs] << 32) | S.klo[qs];
         const u32 d = (u32)(k >> dshift) & mask;
         const u32 g = S.gbase[d] + (u32)q;
+        BH_DCHECK((i64)g < n);
         kout[g] = k;
         if (kVals) vout[g] = svals[qs];
     }

@@ -222,6 +222,7 @@ topo_assign_kernel(const signed char* __restrict__ clev, i64 n, const SortedView
                 if (pend != 0xffffffffu) nfirst[pend] = slot;       // entity (l, s) is the first child of (l-1, s)
                 if (isint) {
                     const u32 b = baseI + __popc(balI & lt);
+                    BH_DCHECK(slot < nslots);
                     node_slot[b] = slot;
                     nlo[b] = (u32)s;
                     pend = b;
@@ -232,6 +233,7 @@ topo_assign_kernel(const signed char* __restrict__ clev, i64 n, const SortedView
             }
         }
         if (valid) {
+            BH_DCHECK(myslot < nslots && myslot > 0u);
             st_stream(leaf_slot + s, myslot);          // written once, read much later: keep L2 for the gathers
             double2* o64 = reinterpret_cast<double2*>(rec64 + myslot);
             st_stream(o64, make_double2(px, py));
@@ -292,6 +294,7 @@ __device__ __forceinline__ void moments_node(i64 b, i64 b1, int level, u32 slot_
     const double x0 = A.x0, y0 = A.y0, z0 = A.z0, L = A.L;
     const u32 first = nfirst[b];
     const u32 cnt = (b + 1 < b1 ? nfirst[b + 1] : slot_end) - first;
+    BH_DCHECK(cnt >= 1u && first + cnt <= slot_end && (level == kMaxLevel || cnt <= 8u));
     double M = 0.0, Sx = 0.0, Sy = 0.0, Sz = 0.0;
     for (u32 j = 0; j < cnt; ++j) {       // ascending octant order (M-rule 1); no fma contraction
         const double2* p = reinterpret_cast<const double2*>(rec64 + first + j);

@@ -65,6 +65,7 @@ struct WalkParams {
     double negG;
     int stack_cap;            // entries per warp
     u32 ntargets;             // only cells with original index < ntargets are targets (bh_set_num_targets)
+    u32 nslots;               // checked build: every slot read must be below this
     EwaldTab ew;              // PERIODIC instantiations only: the Ewald field array (ewald.cuh)
 };
 
@@ -506,6 +507,7 @@ walk_pair_kernel(const WalkParams P)
         const u32 slot = e.x + jj;
         float4 r = make_float4(0.f, 0.f, 0.f, 0.f);
         uint4 t = make_uint4(0u, 0u, 0u, 0u);           // {size, delta, first child, child count}
+        BH_DCHECK(!have || slot < P.nslots);
         if (have) { r = __ldg(rec + slot); t = __ldg(aux + slot); }
         const bool internal = t.w > 0u;
         const bool leaf = have && !internal;
@@ -538,6 +540,7 @@ walk_pair_kernel(const WalkParams P)
             if (ambm) amb[myr] = make_float4(r.x, r.y, r.z, __uint_as_float(~__float_as_uint(rc2)));
             __syncwarp();
             const int na = __popc(bAmb);
+            BH_DCHECK(na >= 1 && na <= 32);
             // failA / failB collect, one bit per undecided node (node i at bit na - 1 - i), whether this lane's
             // member of A / B does NOT pass it (the sign bit of the integer difference is shifted in); one
             // OR-reduction per group then replaces a vote per node
@@ -566,6 +569,7 @@ walk_pair_kernel(const WalkParams P)
         const u32 bOp = __ballot_sync(0xffffffffu, om != 0u);
         if (om) stack[sp + __popc(bOp & lt)] = make_uint2(t.z, t.w | (om << 30));
         sp += __popc(bOp);
+        BH_DCHECK(sp <= P.stack_cap);
         if (COUNT) {
             const bool bucket = internal && !(__uint_as_float(t.x) < __int_as_float(0x7f800000));
             cAccA += accm & 1u; cAccB += accm >> 1;
@@ -589,10 +593,12 @@ walk_pair_kernel(const WalkParams P)
             soa_store<kSoaCap>(U2, at, r);
         }
         nU2 += cU2; nUA += cUA; nUB += cUB;
+        BH_DCHECK(nU2 <= kU2Cap && nUA <= kU1Cap && nUB <= kU1Cap);
         const u32 bC = __ballot_sync(0xffffffffu, danger);
         if (bC) {                                                       // rare: only next to the groups' own cells
             if (danger) { const int at = nC + __popc(bC & lt); C[at] = r; Cm[at] = cmask; }
             nC += __popc(bC);
+            BH_DCHECK(nC <= kCCap);
         }
         __syncwarp();
         // ---- evaluate a list before the next step could overflow it ----
