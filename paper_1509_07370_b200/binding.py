@@ -215,6 +215,18 @@ class Context:
             res = out[: cnt.value]
             return res.clone() if cap > cnt.value + (cnt.value >> 2) + 4096 else res     # do not pin a much larger buffer
 
+    def essential_nodes_into(self, box_lo, box_hi, theta: float, out) -> int:
+        """bh_essential_nodes with a caller-owned destination: `out` is a [cap, 4] float64 CUDA tensor -- of this
+        process, or device memory of ANOTHER rank mapped into this one (CUDA IPC / symmetric memory over NVLink): the
+        gather kernel's 32-byte record stores then ARE the transfer.  Returns the number of entries; raises
+        BH_ERR_TOO_LARGE if they do not fit (the first cap entries are written)."""
+        lo = (C.c_double * 3)(*[float(v) for v in box_lo])
+        hi = (C.c_double * 3)(*[float(v) for v in box_hi])
+        cnt = C.c_int64(0)
+        self._check(self._L.bh_essential_nodes(self._h, lo, hi, float(theta), self._dev(out, self._torch.float64),
+                                               int(out.shape[0]), C.byref(cnt)))
+        return int(cnt.value)
+
     def set_num_targets(self, ntargets: int):
         """bh_set_num_targets: cells with original index < ntargets are targets, the rest sources only (-1: all)."""
         self._check(self._L.bh_set_num_targets(self._h, int(ntargets)))

@@ -79,8 +79,23 @@ def exchange_records(send: Sequence, group=None):
     return [t.to(dev) for t in recv]
 
 
+def exchange_counts(counts: Sequence[int], group=None, device=None):
+    """Peer-buffer exchange, the only collective left: counts[r] = entries this rank WROTE into rank r's inbox.
+    Returns received[s] = entries rank s wrote into ours.  The all-gather doubles as the barrier after which every
+    rank's stores are visible (each rank synchronises its stream before calling)."""
+    import torch
+    import torch.distributed as dist
+    world, rank = dist.get_world_size(group), dist.get_rank(group)
+    cdev = _comm_device(group, device if device is not None else torch.device("cpu"))
+    mine = torch.tensor([int(c) for c in counts], dtype=torch.int64, device=cdev)
+    allc = [torch.empty_like(mine) for _ in range(world)]
+    dist.all_gather(allc, mine, group=group)
+    return [int(allc[s][rank]) for s in range(world)]
+
+
 def let_potential(x, y, z, m, cube, theta: float, G: float = 1.0, group=None, mac: int = 1,
-                  select: Optional[Callable] = None, solve: Optional[Callable] = None, ctx=None):
+                  select: Optional[Callable] = None, solve: Optional[Callable] = None, ctx=None,
+                  peer_out: Optional[Sequence] = None, inbox: Optional[Sequence] = None):
     """Potential of this rank's cells under the mass of ALL ranks (steps 1-5 above).
 
     x, y, z, m : this rank's cells (CUDA float64 tensors on the product path).
@@ -89,6 +104,11 @@ def let_potential(x, y, z, m, cube, theta: float, G: float = 1.0, group=None, ma
     select(x, y, z, m, cube, boxes, theta, mac) -> list of [k, 4] record tensors, one per box (None to skip)
     solve(x, y, z, m, cube, n_targets, theta, G, mac) -> phi[n_targets]
     Both default to libbh through `ctx` (a Context; one is created on the current device if omitted).
+    peer_out / inbox (product path only): the FUSED selection + exchange.  inbox[s] is this rank's [cap, 4] float64
+    buffer for the records of rank s; peer_out[r] is rank r's inbox for THIS rank, mapped into this process (CUDA
+    IPC between processes, symmetric memory / P2P mappings over NVLink between GPUs).  bh_essential_nodes then
+    gathers the essential records of every remote box straight into the receiver's memory -- the kernel's stores
+    are the transfer -- and the only collective left is the all-gather of the counts (exchange_counts).
     Returns (phi of the own cells, info dict with the entry counts sent / received)."""
     import torch
     import torch.distributed as dist
@@ -118,6 +138,25 @@ def let_potential(x, y, z, m, cube, theta: float, G: float = 1.0, group=None, ma
         return solve(x, y, z, m, cube, n_own, theta, G, mac), info
     boxes = gather_boxes(domain_box(x, y, z) if n_own else ((1.0, 1.0, 1.0), (0.0, 0.0, 0.0)), group, x.device)
     want = [None if (r == rank or boxes[r][0][0] > boxes[r][1][0]) else boxes[r] for r in range(world)]
+    if peer_out is not None:
+        if ctx is None or inbox is None:
+            raise ValueError("the peer-buffer exchange needs ctx (libbh) and this rank's inbox buffers")
+        sent = [0] * world
+        if n_own:
+            ctx.set_num_targets(-1)
+            ctx.build(x, y, z, m, cube)
+            for r in range(world):
+                if want[r] is not None:
+                    sent[r] = ctx.essential_nodes_into(want[r][0], want[r][1], theta, peer_out[r])   # stores into rank r
+        torch.cuda.current_stream().synchronize()                    # this rank's stores have left
+        received = exchange_counts(sent, group, x.device)            # ... and after this, everybody's have arrived
+        info["sent"], info["received"] = sent, received
+        if n_own == 0:
+            return x.new_empty(0), info
+        ext = torch.cat([inbox[s][: received[s]] for s in range(world) if received[s] > 0] or [x.new_empty((0, 4))])
+        ux, uy, uz, um = (torch.cat([a, ext[:, k].contiguous()]) for k, a in enumerate((x, y, z, m)))
+        torch.cuda.current_stream().synchronize()   # the inbox has been read: peers may write the next solve's records
+        return solve(ux, uy, uz, um, cube, n_own, theta, G, mac), info
     if n_own:
         send = select(x, y, z, m, cube, want, theta, mac)
         send = [x.new_empty((0, 4)) if s is None else s for s in send]

@@ -249,3 +249,66 @@ def test_let_across_processes_with_product_kernels(bh, oracle, world, empty_rank
         assert (np.abs(phi[sub] - ex) / np.abs(ex)).max() < 1e-2
     if empty_rank is not None:
         assert got[empty_rank][1].shape == (0,) and sum(got[empty_rank][2]["sent"]) == 0
+
+
+# ---- the fused selection + exchange: bh_essential_nodes gathers straight into the RECEIVER's memory ----------------
+def _peer_worker(rank, world, port, q, mail, name):
+    """Every rank allocates one inbox per sender and hands it to that sender through a torch.multiprocessing queue
+    (CUDA IPC: the buffer is mapped into the sender's process); senders then select with the mapped buffer as `out`."""
+    import torch.distributed as dist
+    from paper_1509_07370_b200 import let, binding
+    dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=rank, world_size=world)
+    torch.cuda.set_device(0)
+    w = _LET_INPUTS[name]()
+    parts = _slabs(w, world)
+    i = parts[rank]
+    t = [torch.from_numpy(np.ascontiguousarray(a[i])).cuda() for a in (w.x, w.y, w.z, w.m)]
+    cap = w.n                                                        # an essential set never exceeds the sender's cells
+    inbox = [None if s == rank else torch.zeros((cap, 4), dtype=torch.float64, device="cuda") for s in range(world)]
+    for s in range(world):
+        if s != rank:
+            mail[s].put((rank, inbox[s]))                            # rank s will write its records for us in here
+    peer_out = [None] * world
+    for _ in range(world - 1):
+        r, buf = mail[rank].get(timeout=300)
+        peer_out[r] = buf
+    ctx = binding.Context(0)
+    ctx.set_mac(1)
+    phi, info = let.let_potential(*t, w.cube, 0.5, w.G, mac=1, ctx=ctx, peer_out=peer_out, inbox=inbox)
+    phi2, info2 = let.let_potential(*t, w.cube, 0.5, w.G, mac=1, ctx=ctx, peer_out=peer_out, inbox=inbox)   # buffers reused
+    assert torch.equal(phi, phi2) and info2["received"] == info["received"]
+    q.put((rank, phi.cpu().numpy(), info))
+    dist.barrier()
+    del peer_out
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world,name", [(2, "clustered"), (3, "amr")])
+def test_let_with_peer_mapped_inboxes(bh, oracle, world, name):
+    """The essential-node records go from the selecting kernel straight into the receiving process's device buffer
+    (mapped through CUDA IPC; over NVLink the same pointer arithmetic is a P2P store): no send / receive calls, one
+    all-gather of counts.  Same results as the oracle procedure."""
+    import torch.multiprocessing as mp
+    theta, mac = 0.5, 1
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    mail = [ctx.Queue() for _ in range(world)]
+    port = _free_port()
+    procs = [ctx.Process(target=_peer_worker, args=(r, world, port, q, mail, name)) for r in range(world)]
+    for p in procs:
+        p.start()
+    got = sorted((q.get(timeout=600) for _ in procs), key=lambda t: t[0])
+    for p in procs:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    w = _LET_INPUTS[name]()
+    parts = _slabs(w, world)
+    ophis, osent = _oracle_let(oracle, w, parts, theta, mac)
+    for r, (rank, phi, info) in enumerate(got):
+        assert info["sent"] == osent[r] and info["received"] == [osent[s][r] for s in range(world)]
+        op64, op32, flipped = ophis[r]
+        rel32 = parity._rel(phi, op32)
+        assert rel32.max() <= 1e-4 and np.median(rel32) <= 1e-6, (rel32.max(), np.median(rel32))
+        rel = np.abs(phi - op64) / np.abs(op64)
+        assert rel[~flipped].max() <= 1e-4 and np.median(rel[~flipped]) <= 1e-6
