@@ -244,8 +244,11 @@ def run_workloads_table(args):
     peak = st_sms(0) * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
     rows = [("sphere32", 0.5), ("maclaurin128", 0.5), ("amr_core", 0.5), ("turb256", 0.5),
             ("amr_core", 0.3), ("amr_core", 0.7), ("amr_core", 1.0)]
-    print("| workload | cells | theta | build ms | build B/cell | build % HBM | walk ms | interactions/target | interactions/s | walk % FP32 | cells/s (build+walk) |")
-    print("|---|---:|---:|---:|---:|---:|---:|---:|---:|---:|---:|")
+    import oracle as orc
+    orc.build_library()
+    print("| workload | cells | theta | build ms | build B/cell | build % HBM | walk ms | interactions/target | interactions/s | walk % FP32 "
+          f"| cells/s (build+walk) | oracle cells/s (1 core of {os.cpu_count()}, {cpu_model()}) | Phi max / median rel vs oracle (groups, flips) |")
+    print("|---|---:|---:|---:|---:|---:|---:|---:|---:|---:|---:|---:|---|")
     cache = {}
     for name, theta in rows:
         if name not in cache:
@@ -264,9 +267,17 @@ def run_workloads_table(args):
         st = ctx.get_stats()
         b, t = statistics.median(tb), statistics.median(tw)
         bpc = build_bytes_per_cell(w.n, st.n_nodes, st.sort_passes)
+        # the oracle on this box's host (one core), full build + a sample of the groups, and the parity of that sample
+        w.theta = theta
+        buf = np.full(w.n, np.nan)
+        sample = {}
+        tbo, two, _, _, walked = oracle_step(w, orc, min(args.ref_groups, 2048), buf, sample)
+        par = parity_key(w, phi.cpu().numpy(), ctx.last_group_counts().cpu().numpy(),
+                         ctx.last_group_evaluated().cpu().numpy().astype(np.int64), buf, sample)
         print(f"| {name} | {w.n} | {theta} | {b:.3f} | {bpc:.1f} | {100 * bpc * w.n / (b * 1e-3) / 1e9 / hbm_gbs:.1f} | {t:.3f} | "
               f"{st.interactions / w.n:.1f} | {st.interactions / (t * 1e-3):.3e} | "
-              f"{100 * st.interactions * FLOPS_PER_INTERACTION / (t * 1e-3) / 1e12 / peak:.1f} | {w.n / ((b + t) * 1e-3):.3e} |")
+              f"{100 * st.interactions * FLOPS_PER_INTERACTION / (t * 1e-3) / 1e12 / peak:.1f} | {w.n / ((b + t) * 1e-3):.3e} | "
+              f"{w.n / (tbo + two):.3e} | {par['max_rel']:.1e} / {par['median_rel']:.1e} ({par['groups']}, {par['flips_fp32_vs_fp64']}) |")
         ctx.close()
     return 0
 
