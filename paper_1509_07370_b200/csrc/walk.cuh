@@ -18,12 +18,19 @@
 //    member's fp32 d^2 from below (above).  Only nodes between the two bounds take the per-member
 //    test + __all_sync vote.
 //  * Accepted nodes and leaf cells go to interaction lists in shared memory: U2 (both groups),
-//    UA / UB (one group only) -- all SoA and evaluated two ENTRIES per packed instruction against a
+//    UA / UB (one group only) -- regions of ONE SoA block, so an append is four stores at one
+//    computed index whatever the list; evaluated two ENTRIES per packed instruction against a
 //    scalar target coordinate, U2 for the lane's two targets from the same loads -- and C (leaf
 //    cells inside a group's bounding box -- the only ones that can be a target's own cell or
 //    coincide with it -- evaluated with the zero-distance mask of W3).
 //  * The member votes of one step are batched: each lane collects its member's failures as a bit
-//    per undecided node and one OR-reduction per group replaces a vote per node.
+//    per undecided node (the sign bit of bits(d^2) + ~bits(r_c^2), moved in by a funnel shift) and
+//    one OR-reduction per group replaces a vote per node.
+//  * The kernel counts, per group, the list entries it evaluates (geval): the tests hold that count
+//    against the oracle's accepted + leaf, and it is the numerator of the reported roofline.
+//  * PERIODIC instantiation (App. A): records are moved to the periodic image nearest the pair, entries
+//    on the seam are voted and evaluated with a per-member minimum image, and every entry adds the
+//    Ewald correction looked up in the context's field array (ewald.cuh).
 //  * Partial sums are fp32 over one list flush (<= 128 entries, 4 accumulators) and are flushed
 //    into an fp64 sum per target, which keeps the summation error near 1e-7 relative.
 //  * Phi is written straight to the original cell order (step a7 is fused: no extra pass).

@@ -179,3 +179,22 @@ def test_periodic_turb128_sampled(bh, oracle):
     rel = np.concatenate(rels)
     print(f"periodic turb128: {ng} groups, {flips} flips, max rel {rel.max():.2e}, median {np.median(rel):.2e}")
     assert flips <= 0.05 * ng + 1 and rel.max() <= 1e-4 and np.median(rel) <= 1e-6
+
+
+def test_periodic_mass_refit_and_solve_host(bh, oracle, table):
+    """bh_update_masses and bh_solve_host under periodic boundaries: the same tree with new masses equals a rebuild
+    bit for bit and matches the oracle; the host-buffer call equals the device path."""
+    w = wl.clustered_points(3000, seed=3)
+    rng = np.random.Generator(np.random.PCG64(5))
+    m2 = w.m * rng.uniform(0.5, 2.0, w.n)
+    ctx = _ctx(bh, w)
+    ctx.potential(0.5, w.G)
+    ctx.update_masses(_dev(m2))
+    phi_u = ctx.potential(0.5, w.G).cpu().numpy()
+    w2 = wl.Workload(w.name + "_m2", w.x, w.y, w.z, m2, cube=w.cube)
+    ctx2 = _ctx(bh, w2)
+    assert np.array_equal(phi_u, ctx2.potential(0.5, w.G).cpu().numpy())
+    _check(ctx2, oracle.OracleTree(w.x, w.y, w.z, m2, w.cube), w2, table, 0.5)
+    c3 = bh.Context(0)
+    c3.set_periodic(True, N=N_TAB, nref=NREF)
+    assert np.array_equal(c3.solve_host(w.x, w.y, w.z, m2, w.cube, 0.5, w.G), phi_u)
