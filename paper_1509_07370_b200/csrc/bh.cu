@@ -362,10 +362,7 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
         ctx->launches_build = 0;
         ctx->npass = 0;
         BH_CUDA(cudaMemsetAsync(ds, 0, sizeof(DeviceScalars), st));
-        {   // key_and starts as all ones
-            const u64 ones = ~0ULL;
-            BH_CUDA(cudaMemcpyAsync(&ds->keyred.key_and, &ones, sizeof(u64), cudaMemcpyHostToDevice, st));
-        }
+        BH_CUDA(cudaMemsetAsync(&ds->keyred.key_and, 0xff, sizeof(u64), st));   // key_and starts as all ones
 
         // ---- a1: Morton keys ----
         const double s = 2097152.0 / cube[3];      // K1: s = 2^21 / L in fp64
