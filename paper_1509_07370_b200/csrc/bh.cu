@@ -65,7 +65,7 @@ struct bh_ctx {
     bool walk_periodic = false;           // ... of the last walk (the count pass repeats it)
     int ew_N = 66, ew_nref = 1;           // BH_OPT_EWALD_N / _NREF: points per axis and nested grids of the field array
     int ew_ready_N = 0, ew_ready_nref = 0;
-    DevBuf ew_table, ew_coef;             // grid values (fp64) and per-point quadratic coefficients (fp32)
+    DevBuf ew_table, ew_coef;             // grid values (fp64) and per-point quadratic records (EwaldRec)
     bool counts_valid = false;            // gcount holds the counters of the last walk
     double walk_theta = 0.0;              // arguments of the last bh_potential (the count pass repeats its walk)
     int walk_mac = BH_MAC_BH86;
@@ -634,10 +634,10 @@ int ensure_ewald(bh_ctx* ctx)
     const int N = ctx->ew_N, nref = ctx->ew_nref, M = N - 1;
     const i64 npts = (i64)nref * N * N * N, ncoef = (i64)nref * M * M * M;
     BH_CUDA(ctx->ew_table.ensure(sizeof(double) * npts));
-    BH_CUDA(ctx->ew_coef.ensure(sizeof(float4) * 3 * ncoef));
+    BH_CUDA(ctx->ew_coef.ensure(sizeof(EwaldRec) * ncoef));
     ewald_table_kernel<<<blocks_for(npts, 128), 128, 0, ctx->stream>>>(N, nref, ctx->ew_table.as<double>());
     BH_CUDA(cudaGetLastError());
-    ewald_coef_kernel<<<blocks_for(ncoef, 128), 128, 0, ctx->stream>>>(N, nref, ctx->ew_table.as<double>(), ctx->ew_coef.as<float4>());
+    ewald_coef_kernel<<<blocks_for(ncoef, 128), 128, 0, ctx->stream>>>(N, nref, ctx->ew_table.as<double>(), ctx->ew_coef.as<EwaldRec>());
     BH_CUDA(cudaGetLastError());
     ctx->ew_ready_N = N;
     ctx->ew_ready_nref = nref;
@@ -690,13 +690,18 @@ int launch_walk(bh_ctx* ctx, double theta, double G, double* phi, int group, int
     P.nslots = (u32)ctx->nslots;
     memset(&P.ew, 0, sizeof(P.ew));
     if (periodic) {
-        P.ew.coef = ctx->ew_coef.as<float4>();
+        P.ew.coef = ctx->ew_coef.as<EwaldRec>();
         P.ew.L = (float)ctx->cube[3];
         P.ew.invL = (float)(1.0 / ctx->cube[3]);
         P.ew.s0 = (float)(2.0 * (ctx->ew_N - 2) / ctx->cube[3]);
         P.ew.top = (float)(ctx->ew_N - 2);
         P.ew.M = ctx->ew_N - 1;
+        P.ew.MM = P.ew.M * P.ew.M;
+        P.ew.M3 = P.ew.MM * P.ew.M;
+        P.ew.cbias = 0x4b400000u * (u32)(P.ew.MM + P.ew.M + 1);
         P.ew.nref = ctx->ew_nref;
+        P.ew.inv_s2 = 1.f / ewald_s2(ctx->ew_N);
+        P.ew.ktop = 0x4b400000 + (ctx->ew_N - 2);
     }
     if (group == 32) {
         i64 cap = (i64)kStackPerLevel * (ctx->maxlevel + 2) + 32;

@@ -12,10 +12,13 @@
 //       reaches one point past the face of the minimum-image cell, grid k refines the corner around u = 0;
 //   P4  quadratic through the 3 points per axis around the NEAREST grid point (central differences);
 //   P5  minimum-image displacements everywhere; the own cell and zero-distance pairs contribute m corr1(0)/L.
-// What differs from the paper's layout: besides the grid values (fp64, kept for bh_export of the table) the
-// device keeps, per grid point, the TEN coefficients of its quadratic in fp32 (three float4): a lookup is three
-// 16-byte loads from one 48-byte record and nine FMAs instead of a 19-point gather.
+// What differs from the paper's layout: besides the grid values (fp64, kept for bh_ewald_table) the device keeps,
+// per grid point, the TEN coefficients of its quadratic in one 32-byte record: value and first differences in fp32,
+// the six second differences in fp16 scaled by a power of two (they multiply offsets |t| <= 1/2 twice: their
+// rounding stays below 1e-7 of 1/L).  A lookup is ONE 32-byte load of one aligned sector instead of a 19-point
+// gather -- the periodic walk is bound by L1 sectors per lookup (profiles/r2_periodic_ncu.md).
 #pragma once
+#include <cuda_fp16.h>
 #include "common.cuh"
 
 namespace bh {
@@ -75,10 +78,27 @@ __device__ __forceinline__ double ewald_tab_at(const double* t, int N, int i, in
     return t[((i64)k * N + j) * N + i];
 }
 
-// per grid point (i, j, k <= N - 2) the quadratic around it, in grid units d_a = |u_a|/h - i_a:
-//   c0 = (C0, Dx, Dy, Dz), c1 = (Dxx/2, Dyy/2, Dzz/2, Dxy), c2 = (Dxz, Dyz, 0, 0)
+// one grid point's quadratic, in grid units d_a = |u_a|/h - i_a:
+//   C0 + Dx dx + Dy dy + Dz dz + (hxx dx^2 + hyy dy^2 + hzz dz^2 + hxy dx dy + hxz dx dz + hyz dy dz) / S_lev,
+//   hxx = S_lev Dxx/2 etc.; S_lev = s2 * 4^lev with s2 the power of two below 1/h_0^2 (second differences are
+//   O(10 h^2): the scaled values sit in fp16's normal range)
+struct __align__(32) EwaldRec {
+    float c0, dx, dy, dz;
+    __half2 hxx_yy, hzz_xy, hxz_yz;
+    u32 pad;
+};
+
+__host__ __device__ inline float ewald_s2(int N)
+{
+    float s = 1.f;
+    const float lim = 4.f * (float)(N - 2) * (float)(N - 2);          // 1/h_0^2
+    while (2.f * s <= lim) s *= 2.f;
+    return s;
+}
+
+// per grid point (i, j, k <= N - 2) the quadratic around it
 __global__ void __launch_bounds__(128)
-ewald_coef_kernel(int N, int nref, const double* __restrict__ table, float4* __restrict__ coef)
+ewald_coef_kernel(int N, int nref, const double* __restrict__ table, EwaldRec* __restrict__ coef)
 {
     const int M = N - 1;
     const i64 total = (i64)nref * M * M * M;
@@ -97,47 +117,72 @@ ewald_coef_kernel(int N, int nref, const double* __restrict__ table, float4* __r
                                ewald_tab_at(t, N, i - 1, j, k + 1) + ewald_tab_at(t, N, i - 1, j, k - 1));
     const double Dyz = 0.25 * (ewald_tab_at(t, N, i, j + 1, k + 1) - ewald_tab_at(t, N, i, j + 1, k - 1) -
                                ewald_tab_at(t, N, i, j - 1, k + 1) + ewald_tab_at(t, N, i, j - 1, k - 1));
-    coef[3 * id + 0] = make_float4((float)C0, (float)(0.5 * (xp - xm)), (float)(0.5 * (yp - ym)), (float)(0.5 * (zp - zm)));
-    coef[3 * id + 1] = make_float4((float)(0.5 * (xp - 2.0 * C0 + xm)), (float)(0.5 * (yp - 2.0 * C0 + ym)),
-                                   (float)(0.5 * (zp - 2.0 * C0 + zm)), (float)Dxy);
-    coef[3 * id + 2] = make_float4((float)Dxz, (float)Dyz, 0.f, 0.f);
+    const double S = (double)ewald_s2(N) * (double)(1 << (2 * lev));
+    EwaldRec r;
+    r.c0 = (float)C0; r.dx = (float)(0.5 * (xp - xm)); r.dy = (float)(0.5 * (yp - ym)); r.dz = (float)(0.5 * (zp - zm));
+    r.hxx_yy = __floats2half2_rn((float)(S * 0.5 * (xp - 2.0 * C0 + xm)), (float)(S * 0.5 * (yp - 2.0 * C0 + ym)));
+    r.hzz_xy = __floats2half2_rn((float)(S * 0.5 * (zp - 2.0 * C0 + zm)), (float)(S * Dxy));
+    r.hxz_yz = __floats2half2_rn((float)(S * Dxz), (float)(S * Dyz));
+    r.pad = 0u;
+    coef[id] = r;
 }
 
 // what the walk needs of the table
 struct EwaldTab {
-    const float4* coef;   // [nref][M][M][M][3], M = N - 1
+    const EwaldRec* coef; // [nref][M][M][M], M = N - 1
     float s0;             // grid-0 units per unit length: 2 (N - 2) / L
     float invL;
     float L;
     float top;            // (float)(N - 2): the largest nearest-point index
-    int M;
+    int M, MM, M3;        // M = N - 1 and its powers
     int nref;
+    float inv_s2;         // 1 / ewald_s2(N)
+    int ktop;             // bit pattern of 1.5 * 2^23 + (N - 2): the clamp of the nearest-point index
+    u32 cbias;            // bits(1.5 * 2^23) * (M^2 + M + 1) mod 2^32
 };
 
-// corr1(r/L)/L for a minimum-image displacement (dx, dy, dz), |d_a| <= L/2 (+ rounding), fp32
+// corr1(r/L) for a minimum-image displacement (dx, dy, dz), |d_a| <= L/2 (+ rounding), fp32; the caller divides by L
 __device__ __forceinline__ float ewald_corr(const EwaldTab& T, float dx, float dy, float dz)
 {
-    float ax = fabsf(dx) * T.s0, ay = fabsf(dy) * T.s0, az = fabsf(dz) * T.s0;
-    int lev = 0;
+    float s = T.s0, inv_s = T.inv_s2;
+    u32 off = T.cbias;
     if (T.nref > 1) {
         // finest grid with max_a |u_a| 2^lev <= N - 2: floor(log2(top / m)) from the difference of the bit patterns
-        const float m = fmaxf(fmaxf(ax, ay), fmaxf(az, 1.0e-30f));
+        const float m = fmaxf(fmaxf(fabsf(dx), fabsf(dy)), fmaxf(fabsf(dz), 1.0e-30f)) * T.s0;
         const int e = (int)(__float_as_uint(T.top) - __float_as_uint(m)) >> 23;
-        lev = min(T.nref - 1, max(e, 0));
-        const float sc = __int_as_float((127 + lev) << 23);
-        ax *= sc; ay *= sc; az *= sc;
+        const int lev = min(T.nref - 1, max(e, 0));
+        s *= __int_as_float((127 + lev) << 23);
+        inv_s *= __int_as_float((127 - 2 * lev) << 23);
+        off -= (u32)lev * (u32)T.M3;
     }
-    const float fx = fminf(rintf(ax), T.top), fy = fminf(rintf(ay), T.top), fz = fminf(rintf(az), T.top);
-    const float tx = ax - fx, ty = ay - fy, tz = az - fz;
-    const int idx = ((lev * T.M + (int)fz) * T.M + (int)fy) * T.M + (int)fx;
-    const float4 c0 = __ldg(T.coef + 3 * idx), c1 = __ldg(T.coef + 3 * idx + 1), c2 = __ldg(T.coef + 3 * idx + 2);
-    const float v = c0.x + tx * (c0.y + tx * c1.x + ty * c1.w + tz * c2.x) + ty * (c0.z + ty * c1.y + tz * c2.y) +
-                    tz * (c0.w + tz * c1.z);
-    return v * T.invL;
+    // nearest grid point without the conversion pipe: x + 1.5 * 2^23 rounds x to the nearest (even on ties) integer for
+    // 0 <= x < 2^22 and leaves it in the low mantissa bits; the clamp to N - 2 is an integer minimum on the bit
+    // pattern; the offset from that point comes out of one fma (no rounding of |d| s in between)
+    const float big = 12582912.f;
+    const int bx = min((int)__float_as_uint(__fmaf_rn(fabsf(dx), s, big)), T.ktop);
+    const int by = min((int)__float_as_uint(__fmaf_rn(fabsf(dy), s, big)), T.ktop);
+    const int bz = min((int)__float_as_uint(__fmaf_rn(fabsf(dz), s, big)), T.ktop);
+    const float tx = __fmaf_rn(fabsf(dx), s, big - __uint_as_float((u32)bx));
+    const float ty = __fmaf_rn(fabsf(dy), s, big - __uint_as_float((u32)by));
+    const float tz = __fmaf_rn(fabsf(dz), s, big - __uint_as_float((u32)bz));
+    // the index in wrapping u32 arithmetic: cbias = bits(big) * (M^2 + M + 1) takes the three exponent fields out
+    const u32 idx = (u32)bz * (u32)T.MM + ((u32)by * (u32)T.M + ((u32)bx - off));
+    u32 w0, w1, w2, w3, w4, w5, w6, w7;
+    asm("ld.global.nc.v8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+        : "=r"(w0), "=r"(w1), "=r"(w2), "=r"(w3), "=r"(w4), "=r"(w5), "=r"(w6), "=r"(w7) : "l"(T.coef + idx));
+    (void)w7;
+    const float2 xxyy = __half22float2(*reinterpret_cast<const __half2*>(&w4));
+    const float2 zzxy = __half22float2(*reinterpret_cast<const __half2*>(&w5));
+    const float2 xzyz = __half22float2(*reinterpret_cast<const __half2*>(&w6));
+    const float q = tx * (xxyy.x * tx + zzxy.y * ty + xzyz.x * tz) + ty * (xxyy.y * ty + xzyz.y * tz) + tz * (zzxy.x * tz);
+    return __uint_as_float(w0) + tx * __uint_as_float(w1) + ty * __uint_as_float(w2) + tz * __uint_as_float(w3) + q * inv_s;
 }
 
 // minimum image of a displacement, fp32: d - L rint(d / L)
-__device__ __forceinline__ float wrap_mi(float d, float L, float invL) { return __fmaf_rn(-L, rintf(d * invL), d); }
+// rint(v) for |v| < 2^22 on the FMA pipe (1.5 * 2^23 trick) instead of FRND on the conversion pipe
+__device__ __forceinline__ float rint_magic(float v) { return (v + 12582912.f) - 12582912.f; }
+
+__device__ __forceinline__ float wrap_mi(float d, float L, float invL) { return __fmaf_rn(-L, rint_magic(d * invL), d); }
 
 // n = 1 under periodic boundaries: the lone cell still feels its own images, Phi = -G m corr1(0)/L
 __global__ void periodic_single_kernel(const double4* __restrict__ rec64, const double* __restrict__ table, double L,

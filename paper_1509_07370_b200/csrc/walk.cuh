@@ -289,6 +289,8 @@ template <int CAP>
 __device__ __forceinline__ void eval_soa2_p(const float* __restrict__ L, int cnt, const float4 tA, const float4 tB,
                                             const EwaldTab& T, double& accA, double& accB, bool doA, bool doB)
 {
+    // 1/d and corr1/L are added per entry BEFORE the sum: far entries nearly cancel (f_EF is small where 1/d is
+    // not), two separate fp32 sums would each carry the rounding of a total ~100 x larger than their difference
     float sa = 0.f, sb = 0.f;
     #pragma unroll 2
     for (int e = 0; e < cnt; ++e) {
@@ -296,12 +298,12 @@ __device__ __forceinline__ void eval_soa2_p(const float* __restrict__ L, int cnt
         if (doA) {
             const float dx = x - tA.x, dy = y - tA.y, dz = z - tA.z;
             const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmaf_rn(dx, dx, kTinyD2)));
-            sa = __fmaf_rn(m, rsqrt_approx(d2) + ewald_corr(T, dx, dy, dz), sa);
+            sa = __fmaf_rn(m, __fmaf_rn(ewald_corr(T, dx, dy, dz), T.invL, rsqrt_approx(d2)), sa);
         }
         if (doB) {
             const float dx = x - tB.x, dy = y - tB.y, dz = z - tB.z;
             const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmaf_rn(dx, dx, kTinyD2)));
-            sb = __fmaf_rn(m, rsqrt_approx(d2) + ewald_corr(T, dx, dy, dz), sb);
+            sb = __fmaf_rn(m, __fmaf_rn(ewald_corr(T, dx, dy, dz), T.invL, rsqrt_approx(d2)), sb);
         }
     }
     accA += (double)sa;
@@ -322,13 +324,13 @@ __device__ __forceinline__ void eval_c_p(const float4* __restrict__ L, const u32
             const float dx = wrap_mi(v.x - tA.x, T.L, T.invL), dy = wrap_mi(v.y - tA.y, T.L, T.invL), dz = wrap_mi(v.z - tA.z, T.L, T.invL);
             const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx));
             const float ri = d2 >= 1.17549435e-38f ? rsqrt_approx(d2) : 0.f;
-            if (mk & 1u) sa = __fmaf_rn(v.w, ri + ewald_corr(T, dx, dy, dz), sa);
+            if (mk & 1u) sa = __fmaf_rn(v.w, __fmaf_rn(ewald_corr(T, dx, dy, dz), T.invL, ri), sa);
         }
         {
             const float dx = wrap_mi(v.x - tB.x, T.L, T.invL), dy = wrap_mi(v.y - tB.y, T.L, T.invL), dz = wrap_mi(v.z - tB.z, T.L, T.invL);
             const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx));
             const float ri = d2 >= 1.17549435e-38f ? rsqrt_approx(d2) : 0.f;
-            if (mk & 2u) sb = __fmaf_rn(v.w, ri + ewald_corr(T, dx, dy, dz), sb);
+            if (mk & 2u) sb = __fmaf_rn(v.w, __fmaf_rn(ewald_corr(T, dx, dy, dz), T.invL, ri), sb);
         }
     }
     accA += (double)sa;
@@ -521,9 +523,9 @@ walk_pair_kernel(const WalkParams P)
         bool seam = false;                              // PERIODIC: the nearest image is not every member's minimum image
         if (PERIODIC) {
             // r - L rint((r - c)/L): a record that needs no shift stays bit-identical (the own-cell check relies on it)
-            r.x = __fmaf_rn(-P.ew.L, rintf((r.x - pcx) * P.ew.invL), r.x);
-            r.y = __fmaf_rn(-P.ew.L, rintf((r.y - pcy) * P.ew.invL), r.y);
-            r.z = __fmaf_rn(-P.ew.L, rintf((r.z - pcz) * P.ew.invL), r.z);
+            r.x = __fmaf_rn(-P.ew.L, rint_magic((r.x - pcx) * P.ew.invL), r.x);
+            r.y = __fmaf_rn(-P.ew.L, rint_magic((r.y - pcy) * P.ew.invL), r.y);
+            r.z = __fmaf_rn(-P.ew.L, rint_magic((r.z - pcz) * P.ew.invL), r.z);
             const float ix = r.x - pcx, iy = r.y - pcy, iz = r.z - pcz;
             seam = have && (fabsf(ix) + phx > reach || fabsf(iy) + phy > reach || fabsf(iz) + phz > reach);
         }
