@@ -141,12 +141,15 @@ struct EwaldTab {
     u32 cbias;            // bits(1.5 * 2^23) * (M^2 + M + 1) mod 2^32
 };
 
-// corr1(r/L) for a minimum-image displacement (dx, dy, dz), |d_a| <= L/2 (+ rounding), fp32; the caller divides by L
+// corr1(r/L) for a minimum-image displacement (dx, dy, dz), |d_a| <= L/2 (+ rounding), fp32; the caller divides by L.
+// NESTED = false: one grid (nref = 1, the default) -- the level selection is compiled out (as predicated
+// instructions it cost a fifth of the lookup's issue slots).
+template <bool NESTED>
 __device__ __forceinline__ float ewald_corr(const EwaldTab& T, float dx, float dy, float dz)
 {
     float s = T.s0, inv_s = T.inv_s2;
     u32 off = T.cbias;
-    if (T.nref > 1) {
+    if (NESTED) {
         // finest grid with max_a |u_a| 2^lev <= N - 2: floor(log2(top / m)) from the difference of the bit patterns
         const float m = fmaxf(fmaxf(fabsf(dx), fabsf(dy)), fmaxf(fabsf(dz), 1.0e-30f)) * T.s0;
         const int e = (int)(__float_as_uint(T.top) - __float_as_uint(m)) >> 23;
@@ -156,26 +159,32 @@ __device__ __forceinline__ float ewald_corr(const EwaldTab& T, float dx, float d
         off -= (u32)lev * (u32)T.M3;
     }
     // nearest grid point without the conversion pipe: x + 1.5 * 2^23 rounds x to the nearest (even on ties) integer for
-    // 0 <= x < 2^22 and leaves it in the low mantissa bits; the clamp to N - 2 is an integer minimum on the bit
-    // pattern; the offset from that point comes out of one fma (no rounding of |d| s in between)
+    // 0 <= x < 2^22 and leaves it in the low mantissa bits; the offset from that point comes out of one fma (no
+    // rounding of |d| s in between).
+    // No clamp: |d_a| s <= (N - 2)(1 + a few ulp) rounds to at most N - 2, the last point that has a record.
     const float big = 12582912.f;
-    const int bx = min((int)__float_as_uint(__fmaf_rn(fabsf(dx), s, big)), T.ktop);
-    const int by = min((int)__float_as_uint(__fmaf_rn(fabsf(dy), s, big)), T.ktop);
-    const int bz = min((int)__float_as_uint(__fmaf_rn(fabsf(dz), s, big)), T.ktop);
+    const int bx = (int)__float_as_uint(__fmaf_rn(fabsf(dx), s, big));
+    const int by = (int)__float_as_uint(__fmaf_rn(fabsf(dy), s, big));
+    const int bz = (int)__float_as_uint(__fmaf_rn(fabsf(dz), s, big));
+    BH_DCHECK(bx <= T.ktop && by <= T.ktop && bz <= T.ktop);
     const float tx = __fmaf_rn(fabsf(dx), s, big - __uint_as_float((u32)bx));
     const float ty = __fmaf_rn(fabsf(dy), s, big - __uint_as_float((u32)by));
     const float tz = __fmaf_rn(fabsf(dz), s, big - __uint_as_float((u32)bz));
     // the index in wrapping u32 arithmetic: cbias = bits(big) * (M^2 + M + 1) takes the three exponent fields out
     const u32 idx = (u32)bz * (u32)T.MM + ((u32)by * (u32)T.M + ((u32)bx - off));
-    u32 w0, w1, w2, w3, w4, w5, w6, w7;
+    u32 w0, w1, w2, w3, w4, w5, w6;
+    [[maybe_unused]] u32 w7;                            // the record's padding word
     asm("ld.global.nc.v8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
         : "=r"(w0), "=r"(w1), "=r"(w2), "=r"(w3), "=r"(w4), "=r"(w5), "=r"(w6), "=r"(w7) : "l"(T.coef + idx));
-    (void)w7;
     const float2 xxyy = __half22float2(*reinterpret_cast<const __half2*>(&w4));
     const float2 zzxy = __half22float2(*reinterpret_cast<const __half2*>(&w5));
     const float2 xzyz = __half22float2(*reinterpret_cast<const __half2*>(&w6));
-    const float q = tx * (xxyy.x * tx + zzxy.y * ty + xzyz.x * tz) + ty * (xxyy.y * ty + xzyz.y * tz) + tz * (zzxy.x * tz);
-    return __uint_as_float(w0) + tx * __uint_as_float(w1) + ty * __uint_as_float(w2) + tz * __uint_as_float(w3) + q * inv_s;
+    // explicit fmas: the same bits whatever the compiler would contract (the checked build must agree, test_gpu_checked)
+    const float qx = __fmaf_rn(xzyz.x, tz, __fmaf_rn(zzxy.y, ty, xxyy.x * tx));
+    const float qy = __fmaf_rn(xzyz.y, tz, xxyy.y * ty);
+    const float q = __fmaf_rn(tx, qx, __fmaf_rn(ty, qy, tz * (zzxy.x * tz)));
+    const float lin = __fmaf_rn(tz, __uint_as_float(w3), __fmaf_rn(ty, __uint_as_float(w2), __fmaf_rn(tx, __uint_as_float(w1), __uint_as_float(w0))));
+    return __fmaf_rn(q, inv_s, lin);
 }
 
 // minimum image of a displacement, fp32: d - L rint(d / L)

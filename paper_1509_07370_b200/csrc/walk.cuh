@@ -284,26 +284,26 @@ __device__ __forceinline__ void eval_c_g(const float4* __restrict__ L, const u32
 // ---- PERIODIC (App. A): every entry contributes m (1/d + corr1(d_vec/L)/L) = m f_EF (Eq. A.1) -------------------
 // The unchecked lists hold entries already moved to the periodic image nearest the pair of groups, and only
 // entries for which that image is the minimum image for EVERY member, so plain differences are minimum-image
-// displacements.  One entry at a time: the table lookup (three 16-byte loads + nine FMAs) dominates.
-template <int CAP>
-__device__ __forceinline__ void eval_soa2_p(const float* __restrict__ L, int cnt, const float4 tA, const float4 tB,
+// displacements.  One entry at a time: the table lookup (one 32-byte record, ewald.cuh) dominates.
+template <int CAP, bool NESTED>
+__device__ __forceinline__ void eval_soa2_pn(const float* __restrict__ L, int cnt, const float4 tA, const float4 tB,
                                             const EwaldTab& T, double& accA, double& accB, bool doA, bool doB)
 {
     // 1/d and corr1/L are added per entry BEFORE the sum: far entries nearly cancel (f_EF is small where 1/d is
     // not), two separate fp32 sums would each carry the rounding of a total ~100 x larger than their difference
     float sa = 0.f, sb = 0.f;
-    #pragma unroll 2
+    #pragma unroll 1
     for (int e = 0; e < cnt; ++e) {
         const float x = L[e], y = L[CAP + e], z = L[2 * CAP + e], m = L[3 * CAP + e];
         if (doA) {
             const float dx = x - tA.x, dy = y - tA.y, dz = z - tA.z;
             const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmaf_rn(dx, dx, kTinyD2)));
-            sa = __fmaf_rn(m, __fmaf_rn(ewald_corr(T, dx, dy, dz), T.invL, rsqrt_approx(d2)), sa);
+            sa = __fmaf_rn(m, __fmaf_rn(ewald_corr<NESTED>(T, dx, dy, dz), T.invL, rsqrt_approx(d2)), sa);
         }
         if (doB) {
             const float dx = x - tB.x, dy = y - tB.y, dz = z - tB.z;
             const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmaf_rn(dx, dx, kTinyD2)));
-            sb = __fmaf_rn(m, __fmaf_rn(ewald_corr(T, dx, dy, dz), T.invL, rsqrt_approx(d2)), sb);
+            sb = __fmaf_rn(m, __fmaf_rn(ewald_corr<NESTED>(T, dx, dy, dz), T.invL, rsqrt_approx(d2)), sb);
         }
     }
     accA += (double)sa;
@@ -312,7 +312,8 @@ __device__ __forceinline__ void eval_soa2_p(const float* __restrict__ L, int cnt
 
 // checked list under periodic boundaries: explicit minimum image per target; the own cell and zero-distance
 // pairs keep their image / background part m corr1(0)/L (reading P5) and drop only 1/d
-__device__ __forceinline__ void eval_c_p(const float4* __restrict__ L, const u32* __restrict__ Lm, int cnt, const float4 tA,
+template <bool NESTED>
+__device__ __forceinline__ void eval_c_pn(const float4* __restrict__ L, const u32* __restrict__ Lm, int cnt, const float4 tA,
                                          const float4 tB, const EwaldTab& T, double& accA, double& accB, u32& evA, u32& evB)
 {
     float sa = 0.f, sb = 0.f;
@@ -324,17 +325,33 @@ __device__ __forceinline__ void eval_c_p(const float4* __restrict__ L, const u32
             const float dx = wrap_mi(v.x - tA.x, T.L, T.invL), dy = wrap_mi(v.y - tA.y, T.L, T.invL), dz = wrap_mi(v.z - tA.z, T.L, T.invL);
             const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx));
             const float ri = d2 >= 1.17549435e-38f ? rsqrt_approx(d2) : 0.f;
-            if (mk & 1u) sa = __fmaf_rn(v.w, __fmaf_rn(ewald_corr(T, dx, dy, dz), T.invL, ri), sa);
+            if (mk & 1u) sa = __fmaf_rn(v.w, __fmaf_rn(ewald_corr<NESTED>(T, dx, dy, dz), T.invL, ri), sa);
         }
         {
             const float dx = wrap_mi(v.x - tB.x, T.L, T.invL), dy = wrap_mi(v.y - tB.y, T.L, T.invL), dz = wrap_mi(v.z - tB.z, T.L, T.invL);
             const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx));
             const float ri = d2 >= 1.17549435e-38f ? rsqrt_approx(d2) : 0.f;
-            if (mk & 2u) sb = __fmaf_rn(v.w, __fmaf_rn(ewald_corr(T, dx, dy, dz), T.invL, ri), sb);
+            if (mk & 2u) sb = __fmaf_rn(v.w, __fmaf_rn(ewald_corr<NESTED>(T, dx, dy, dz), T.invL, ri), sb);
         }
     }
     accA += (double)sa;
     accB += (double)sb;
+}
+
+// one grid (the default) or nested grids: chosen once per list, not per interaction
+template <int CAP>
+__device__ __forceinline__ void eval_soa2_p(const float* __restrict__ L, int cnt, const float4 tA, const float4 tB,
+                                            const EwaldTab& T, double& accA, double& accB, bool doA, bool doB)
+{
+    if (T.nref > 1) eval_soa2_pn<CAP, true>(L, cnt, tA, tB, T, accA, accB, doA, doB);
+    else eval_soa2_pn<CAP, false>(L, cnt, tA, tB, T, accA, accB, doA, doB);
+}
+
+__device__ __forceinline__ void eval_c_p(const float4* __restrict__ L, const u32* __restrict__ Lm, int cnt, const float4 tA,
+                                         const float4 tB, const EwaldTab& T, double& accA, double& accB, u32& evA, u32& evB)
+{
+    if (T.nref > 1) eval_c_pn<true>(L, Lm, cnt, tA, tB, T, accA, accB, evA, evB);
+    else eval_c_pn<false>(L, Lm, cnt, tA, tB, T, accA, accB, evA, evB);
 }
 
 // packed minimum image: d - L rint(d / L), rint by the 1.5 * 2^23 trick (|d / L| is far below 2^22)
