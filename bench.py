@@ -440,7 +440,7 @@ def run_ours(args):
     periodic_info = {"ms_walk": t_periodic * 1e3, "interactions_per_s": world * pst.interactions / t_periodic,
                      "interactions_per_target": pst.interactions / n, "ewald_grid_points_per_axis": 66, "ewald_nested_grids": 1,
                      "slowdown_vs_isolated_walk": t_periodic / t_walk,
-                     "note": "every interaction adds a quadratic table lookup (one 32 B record, ~55 instructions) to the 13-flop kernel"}
+                     "note": "every interaction adds a quadratic table lookup (one 32 B record, ~48 instructions) to the 13-flop kernel"}
     del pphi_dev
     pctx.close()
 
