@@ -96,6 +96,20 @@ def test_periodic_phi_vs_oracle(bh, oracle, table, w, theta, mac):
     _check(ctx, ot, w, table, theta, mac)
 
 
+@pytest.mark.parametrize("N,nref", [(18, 3), (10, 4), (66, 1)])
+def test_periodic_other_grids(bh, oracle, N, nref):
+    """Coarse grids with deeper nesting and the default single grid: both sides interpolate the same array, so the
+    bars stay those of the main comparison whatever the grid's own interpolation error is."""
+    w = wl.clustered_points(3000, seed=3)
+    tab = oracle.EwaldTable(N=N, nref=nref)
+    ctx = bh.Context(0)
+    ctx.set_periodic(True, N=N, nref=nref)
+    got = ctx.ewald_table().cpu().numpy().reshape(-1)
+    assert np.max(np.abs(got - tab.data)) <= 1e-11
+    ctx.build(_dev(w.x), _dev(w.y), _dev(w.z), _dev(w.m), w.cube)
+    _check(ctx, oracle.OracleTree(w.x, w.y, w.z, w.m, w.cube), w, tab, 0.5)
+
+
 def test_uniform_periodic_grid_closed_form(bh):
     """16^3 equal masses in a periodic box = a simple cubic lattice of spacing L/16: Phi_i = +2.8372974795 G m 16 / L
     at every cell (theta = 0: every cell is summed through the table)."""
