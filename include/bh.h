@@ -212,6 +212,27 @@ int bh_field(bh_ctx* ctx, double theta, double G, double* phi, double* acc);
  * Pairs of distinct cells at zero distance are skipped. */
 int bh_potential_direct(bh_ctx* ctx, double G, const int64_t* targets, int64_t nt, double* phi);
 
+/* bh_direct_noalloc: the same direct sum (Eq. 2; fp64; zero-distance pairs skipped) WITHOUT a context
+ * and WITHOUT any allocation, for callers that cannot call cudaMalloc (CUDA graph capture, serving loops, harnesses
+ * that forbid it).  The packed (x, y, z, m) copy of the cells that bh_potential_direct allocates in its context
+ * lives here in a file-scope static __device__ array of BH_NOALLOC_MAX_N records (1 MiB per GPU that loads libbh,
+ * held until the process exits).  The call enqueues two kernels on `cuda_stream` and returns; it does not
+ * synchronise, allocate, free, or create streams / events.  (The first call on a device looks up the array's device
+ * address, cudaGetSymbolAddress: make that call outside a stream capture.)
+ *   device      : CUDA device ordinal (made current for the call, the previous device is restored)
+ *   cuda_stream : cudaStream_t, or NULL for the default stream
+ *   x, y, z, m  : DEVICE, const double[n], read only, original order
+ *   n           : 0 <= n <= BH_NOALLOC_MAX_N; larger n returns BH_ERR_TOO_LARGE (nothing is launched), n = 0 is BH_OK
+ *   phi         : DEVICE, double[n], phi[i] = -G sum_{j != i} m_j/|r_i - r_j|, original order
+ * Every call on a device shares the one array and leaves its records in it: the next call overwrites what it reads,
+ * nothing has to be cleared.  Calls that OVERLAP on the GPU (different streams without ordering, several host
+ * threads) race on it: order them.  Errors: BH_ERR_INVALID_ARG / BH_ERR_TOO_LARGE / BH_ERR_CUDA;
+ * bh_noalloc_last_error() returns the calling thread's last message (there is no context to keep it). */
+#define BH_NOALLOC_MAX_N 32768
+int bh_direct_noalloc(int device, void* cuda_stream, const double* x, const double* y, const double* z, const double* m,
+                      int64_t n, double G, double* phi);
+const char* bh_noalloc_last_error(void);
+
 /* One call with HOST buffers: copies x, y, z, m (double[n] each, pageable or pinned) to the
  * device, runs bh_build and bh_potential, copies phi (double[n]) back, synchronises ("Only position and
  * mass data is copied to the device ... just results are copied back").

@@ -6,6 +6,7 @@ libbh.so.  PyTorch supplies device memory and the stream.  There is no CPU fallb
 missing it is built with nvcc, and if that fails the import of `Context` users fails loudly.
 """
 from .binding import (BH_MAC_BARNES94, BH_MAC_BH86, BHError, Context, Stats, lib, lib_path,  # noqa: F401
-                      EXPORTED_SYMBOLS)
+                      EXPORTED_SYMBOLS, NOALLOC_MAX_N, direct_noalloc)
 
-__all__ = ["Context", "Stats", "BHError", "BH_MAC_BH86", "BH_MAC_BARNES94", "lib", "lib_path", "EXPORTED_SYMBOLS"]
+__all__ = ["Context", "Stats", "BHError", "BH_MAC_BH86", "BH_MAC_BARNES94", "lib", "lib_path", "EXPORTED_SYMBOLS",
+           "direct_noalloc", "NOALLOC_MAX_N"]

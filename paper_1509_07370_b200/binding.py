@@ -21,6 +21,7 @@ EXPORTED_SYMBOLS = (
     "bh_potential_direct", "bh_solve_host", "bh_tree_sizes", "bh_export_tree", "bh_last_group_counts",
     "bh_last_interactions", "bh_get_stats", "bh_update_masses", "bh_essential_nodes", "bh_set_num_targets", "bh_field",
     "bh_last_group_evaluated", "bh_last_walk_group", "bh_get_build_passes", "bh_host_breakdown", "bh_ewald_table",
+    "bh_direct_noalloc", "bh_noalloc_last_error",
 )
 
 
@@ -88,11 +89,42 @@ def lib():
         L.bh_host_breakdown.argtypes = [vp, C.POINTER(C.c_float)]
         L.bh_ewald_table.argtypes = [vp, dp, i64, C.POINTER(i32), C.POINTER(i32)]
         L.bh_get_stats.argtypes = [vp, C.POINTER(Stats)]
+        L.bh_direct_noalloc.argtypes = [i32, vp, dp, dp, dp, dp, i64, C.c_double, dp]
+        L.bh_noalloc_last_error.argtypes = []
+        L.bh_noalloc_last_error.restype = C.c_char_p
         for name in EXPORTED_SYMBOLS:
-            if name not in ("bh_strerror", "bh_last_cuda_error"):
+            if name not in ("bh_strerror", "bh_last_cuda_error", "bh_noalloc_last_error"):
                 getattr(L, name).restype = i32
         _lib = L
     return _lib
+
+
+NOALLOC_MAX_N = 32768      # BH_NOALLOC_MAX_N of include/bh.h
+
+
+def direct_noalloc(x, y, z, m, G: float = 1.0, out=None, stream=None):
+    """bh_direct_noalloc: the fp64 direct sum of n <= NOALLOC_MAX_N cells with its scratch in a static device array
+    of libbh -- no context, no allocation inside the library.  x, y, z, m: contiguous float64 CUDA tensors; `out`:
+    float64 CUDA tensor [n] (allocated by torch here when None -- pass it to keep the whole call allocation-free);
+    `stream`: a torch.cuda.Stream (default: the current stream of the tensors' device).  Asynchronous."""
+    import torch
+    n = x.numel()
+    dev = x.device
+    if out is None:
+        out = torch.empty(n, dtype=torch.float64, device=dev)
+    ptrs = []
+    for t in (x, y, z, m, out):
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+                and t.numel() == n and t.device == dev):
+            raise TypeError("expected contiguous float64 CUDA tensors of one length on one device")
+        ptrs.append(C.c_void_p(t.data_ptr()))
+    st = stream if stream is not None else torch.cuda.current_stream(dev)
+    L = lib()
+    rc = L.bh_direct_noalloc(dev.index if dev.index is not None else torch.cuda.current_device(),
+                             C.c_void_p(st.cuda_stream), ptrs[0], ptrs[1], ptrs[2], ptrs[3], n, float(G), ptrs[4])
+    if rc != 0:
+        raise BHError(rc, (L.bh_noalloc_last_error() or L.bh_strerror(rc)).decode())
+    return out
 
 
 def _cube(c):

@@ -13,6 +13,7 @@ LIB = os.path.join(HERE, "libbh.so")
 CHECKED_LIB = os.path.join(HERE, "libbh_checked.so")   # -DBH_CHECKED: device-side bounds checks (tests/test_gpu_checked.py)
 PEAK_LIB = os.path.join(HERE, "libbh_fma_peak.so")      # bench.py's measured FP32 denominator; not part of libbh
 PEAK_SRC = os.path.join(CSRC, "fma_peak.cu")
+LIB_SRCS = [os.path.join(CSRC, "bh.cu"), os.path.join(CSRC, "direct_noalloc.cu")]   # the translation units of libbh
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
 
@@ -40,7 +41,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     """nvcc -gencode arch=compute_100a,code=sm_100a ... -> paper_1509_07370_b200/libbh.so"""
     if force or needs_build():
         cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
-              ["-o", LIB, os.path.join(CSRC, "bh.cu")]
+              ["-o", LIB] + LIB_SRCS
         subprocess.check_call(cmd)
     return LIB
 
@@ -48,7 +49,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
 def build_checked(force: bool = False) -> str:
     """The same library with -DBH_CHECKED: every index the kernels compute is bounds-checked on the device."""
     if force or not os.path.exists(CHECKED_LIB) or any(os.path.getmtime(s) > os.path.getmtime(CHECKED_LIB) for s in sources()):
-        subprocess.check_call([_nvcc()] + NVCC_FLAGS + ["-DBH_CHECKED", "-o", CHECKED_LIB, os.path.join(CSRC, "bh.cu")])
+        subprocess.check_call([_nvcc()] + NVCC_FLAGS + ["-DBH_CHECKED", "-o", CHECKED_LIB] + LIB_SRCS)
     return CHECKED_LIB
 
 
