@@ -492,6 +492,35 @@ def run_ours(args):
     torch.cuda.synchronize()
     e2e_pageable_t = time.perf_counter() - t1
 
+    # independent problems (a serving loop, not a time-stepping solver: a step there needs Phi before its next
+    # positions exist): two contexts on two streams, one host thread each -- the copies of one call run under the
+    # kernels of the other.  ctypes releases the GIL for the duration of bh_solve_host.
+    import threading
+    pair_ctx = [bh.Context(local, stream=torch.cuda.Stream(device=local)) for _ in range(2)]
+    pair_out = [torch.empty(n, dtype=torch.float64).pin_memory() for _ in range(2)]
+
+    def _serve(k, steps):
+        for _ in range(steps):
+            pair_ctx[k].solve_host(hx[0], hx[1], hx[2], hx[3], w.cube, w.theta, w.G, out=pair_out[k].numpy())
+
+    for k in range(2):
+        _serve(k, 1)                                           # first build of each context: allocations
+    torch.cuda.synchronize()
+    workers = [threading.Thread(target=_serve, args=(k, e2e_steps)) for k in range(2)]
+    t1 = time.perf_counter()
+    for th in workers:
+        th.start()
+    for th in workers:
+        th.join()
+    torch.cuda.synchronize()
+    e2e_pair_t = time.perf_counter() - t1
+    e2e_pair_t = ranks.max_over_ranks([e2e_pair_t], dev)[0]
+    e2e_pair_equal = bool(np.array_equal(pair_out[0].numpy(), phi_host.numpy()) and
+                          np.array_equal(pair_out[1].numpy(), phi_host.numpy()))
+    for c in pair_ctx:
+        c.close()
+    del pair_out
+
     if rank != 0:
         if dist:
             dist.destroy_process_group()
@@ -549,7 +578,11 @@ def run_ours(args):
                 "d2h_bytes_per_step": 8 * n, "steps": e2e_steps, "api": "bh_solve_host (pinned host buffers)",
                 "ms_per_step": e2e_t / e2e_steps * 1e3, "split_last_call": e2e_split,
                 "pageable_buffers": {"value": n / e2e_pageable_t, "ms_per_step": e2e_pageable_t * 1e3,
-                                     "note": "ordinary (pageable) numpy arrays: the CUDA runtime stages the copies, no overlap with the kernels"}},
+                                     "note": "ordinary (pageable) numpy arrays: the CUDA runtime stages the copies, no overlap with the kernels"},
+                "two_contexts_two_threads": {"value": ranks.whole_job_rate(n, 2 * e2e_steps, e2e_pair_t, world),
+                                             "ms_per_step": e2e_pair_t / (2 * e2e_steps) * 1e3, "calls": 2 * e2e_steps,
+                                             "phi_equal_to_single_context": e2e_pair_equal,
+                                             "note": "independent problems: bh_solve_host from two host threads, each with its own context and stream; one call's copies run under the other's kernels"}},
         "gpu_launches": launches_per_step * args.steps,
     }
     if let_info is not None:
