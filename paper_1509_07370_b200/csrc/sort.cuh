@@ -31,23 +31,35 @@ __device__ __forceinline__ u32 ld_status(const u32* p)
 // (warp-uniform; must contain every bit on which the warp's digits differ).  Eight ballots when all
 // bits vary (match.any slows down with every distinct value instead); cells that are neighbours in
 // memory share most key bits, so a warp of grid data in original order needs only 2-3.
+// one bit of the match: bit -> predicate, ballot, all-ones mask of the own bit, differ |= ballot ^ mask
+// (written out in PTX: the compiler's own forms take five or six instructions per bit)
+template <int B>
+__device__ __forceinline__ void differ_step(u32& differ, u32 d)
+{
+    asm volatile("{\n\t.reg .pred p;\n\t.reg .b32 bal, t, s;\n\t"
+                 "and.b32 t, %1, %2;\n\tsetp.ne.u32 p, t, 0;\n\t"
+                 "vote.sync.ballot.b32 bal, p, 0xffffffff;\n\t"
+                 "selp.b32 s, -1, 0, p;\n\t"
+                 "lop3.b32 %0, %0, bal, s, 0xf6;\n\t}"
+                 : "+r"(differ) : "r"(d), "n"(1 << B));
+}
+
 __device__ __forceinline__ u32 digit_peers_on(u32 d, u32 vary)
 {
     u32 differ = 0u;                             // lanes whose digit differs from this lane's in some bit
     if (vary == 0xffu) {
-        #pragma unroll
-        for (int b = 0; b < 8; ++b) {
-            const int s = (int)(d << (31 - b)) >> 31;            // all ones iff bit b of d is set
-            const u32 bal = __ballot_sync(0xffffffffu, s < 0);
-            differ |= bal ^ (u32)s;
-        }
+        differ_step<0>(differ, d); differ_step<1>(differ, d); differ_step<2>(differ, d); differ_step<3>(differ, d);
+        differ_step<4>(differ, d); differ_step<5>(differ, d); differ_step<6>(differ, d); differ_step<7>(differ, d);
     } else {
         while (vary) {
-            const int b = __ffs(vary) - 1;
-            vary &= vary - 1u;
-            const int s = (int)(d << (31 - b)) >> 31;
-            const u32 bal = __ballot_sync(0xffffffffu, s < 0);
-            differ |= bal ^ (u32)s;
+            const u32 m = vary & (0u - vary);                    // lowest bit still to match
+            vary ^= m;
+            asm volatile("{\n\t.reg .pred p;\n\t.reg .b32 bal, t, s;\n\t"
+                         "and.b32 t, %1, %2;\n\tsetp.ne.u32 p, t, 0;\n\t"
+                         "vote.sync.ballot.b32 bal, p, 0xffffffff;\n\t"
+                         "selp.b32 s, -1, 0, p;\n\t"
+                         "lop3.b32 %0, %0, bal, s, 0xf6;\n\t}"
+                         : "+r"(differ) : "r"(d), "r"(m));
         }
     }
     return ~differ;
@@ -200,17 +212,40 @@ radix_onesweep_kernel(const u64* __restrict__ kin, const u32* __restrict__ vin, 
         }
     }
     __syncthreads();
-    {   // thread d: exclusive scan of digit d over the warps, then over the digits
-        const int d = tid;
-        u32 run = 0;
-        #pragma unroll
-        for (int w = 0; w < kSortThreads / 32; ++w) { u32 c = S.wcnt[w][d]; S.wcnt[w][d] = run; run += c; }
-        // publish this tile's count of digit d, then look back for the pairs of digit d in earlier tiles
-        volatile u32* st = status + (size_t)tile * kRadix + d;
-        if (tile == 0) *st = kFlagPrefix | run; else *st = kFlagAgg | run;
-        u32 total;
-        const u32 ex = block_excl_scan_256(run, total, S.s_warp);          // tile-local start of digit d
-        const u32 gstart = block_excl_scan_256(ghist[d], total, S.s_warp);  // global start of digit d
+    // thread d: exclusive scan of digit d over the warps, then over the digits
+    const int dg = tid;
+    u32 run = 0;
+    #pragma unroll
+    for (int w = 0; w < kSortThreads / 32; ++w) { u32 c = S.wcnt[w][dg]; S.wcnt[w][dg] = run; run += c; }
+    // publish this tile's count of digit d; the look-back for the pairs of digit d in earlier tiles comes AFTER the
+    // exchange through shared memory: by then more of the earlier tiles have published their prefixes
+    volatile u32* st = status + (size_t)tile * kRadix + dg;
+    if (tile == 0) *st = kFlagPrefix | run; else *st = kFlagAgg | run;
+    u32 total;
+    const u32 ex = block_excl_scan_256(run, total, S.s_warp);          // tile-local start of digit d
+    const u32 gstart = block_excl_scan_256(ghist[dg], total, S.s_warp);  // global start of digit d
+    S.dstart[dg] = ex;
+    __syncthreads();
+    #pragma unroll
+    for (int i = 0; i < kSortItems; ++i) {
+        const u32 d = (u32)(key[i] >> shift) & mask;
+        const u32 q = S.dstart[d] + S.wcnt[warp][d] + rank[i];
+        BH_DCHECK(q < (u32)kSortTile);
+        const u32 qs = q ^ ((q >> 5) & 31u);
+        const u32 e32 = (u32)(wbase + i * 32 + lane);
+        if (MODE == kPackedFirst) {                         // word = key window | element index
+            const u64 word = ((key[i] >> lo) << ib) | (u64)e32;
+            S.klo[qs] = (u32)word;
+            S.khi[qs] = (u32)(word >> 32);
+        } else {
+            S.klo[qs] = (u32)key[i];
+            S.khi[qs] = (u32)(key[i] >> 32);
+        }
+        if (MODE == kGenericFirst) svals[qs] = e32;
+        if (MODE == kGeneric) svals[qs] = val[i];
+    }
+    {
+        const int d = dg;
         u32 before = 0;
         if (tile > 0) {
             // look-back in windows of kLookWin tiles: the window's status words are fetched together
@@ -234,27 +269,7 @@ radix_onesweep_kernel(const u64* __restrict__ kin, const u32* __restrict__ vin, 
             }
             *st = kFlagPrefix | (before + run);
         }
-        S.dstart[d] = ex;
         S.gbase[d] = gstart + before - ex;
-    }
-    __syncthreads();
-    #pragma unroll
-    for (int i = 0; i < kSortItems; ++i) {
-        const u32 d = (u32)(key[i] >> shift) & mask;
-        const u32 q = S.dstart[d] + S.wcnt[warp][d] + rank[i];
-        BH_DCHECK(q < (u32)kSortTile);
-        const u32 qs = q ^ ((q >> 5) & 31u);
-        const u32 e32 = (u32)(wbase + i * 32 + lane);
-        if (MODE == kPackedFirst) {                         // word = key window | element index
-            const u64 word = ((key[i] >> lo) << ib) | (u64)e32;
-            S.klo[qs] = (u32)word;
-            S.khi[qs] = (u32)(word >> 32);
-        } else {
-            S.klo[qs] = (u32)key[i];
-            S.khi[qs] = (u32)(key[i] >> 32);
-        }
-        if (MODE == kGenericFirst) svals[qs] = e32;
-        if (MODE == kGeneric) svals[qs] = val[i];
     }
     __syncthreads();
     const i64 left = n - base;
