@@ -78,7 +78,9 @@ typedef struct bh_stats {
                                   counted by the Phi kernel itself at every list flush (the roofline numerator) */
     /* device time in ms of the passes of the last bh_build / bh_potential (CUDA events) */
     /* device ms of the last build: keys (a1), sort (a2), count = c(s) + level histograms + scan (a4),
-     * assign = entity numbering + cells moved into their slots (a4 + a3), moments (a5), whole build */
+     * assign = entity numbering + cells moved into their slots (a4 + a3), moments (a5), whole build.
+     * The five phase times are filled only for a build made under BH_OPT_PASS_TIMING (else 0): an event between
+     * two kernels would break the chain of dependent launches bh_build issues; ms_build_total is always there. */
     float ms_keys, ms_sort, ms_count, ms_assign, ms_moments, ms_build_total;
     float ms_walk;
     int32_t launches_build;    /* kernels the last bh_build launched                                   */

@@ -109,6 +109,7 @@ struct bh_ctx {
 
     cudaEvent_t ev[EV_COUNT] = {nullptr};
     bool ev_build = false, ev_walk = false;
+    bool ev_phases = false;               // the per-phase events of the last build were recorded (BH_OPT_PASS_TIMING)
     int launches_build = 0, launches_walk = 0;
 
     // BH_OPT_PASS_TIMING: one event after every kernel of bh_build (a reporting mode: the events add gaps)
@@ -185,8 +186,7 @@ int launch_moments(bh_ctx* ctx)
             lvl_bytes = 32.0 * (kids - inner) + 72.0 * (double)(b1 - b0);
         }
         if ((!small || l < 0) && sl.nlev > 0) {          // flush the pending run of small levels
-            moments_small_kernel<<<1, kMomSmallThreads, 0, st>>>(sl, MA);
-            BH_CUDA(cudaGetLastError());
+            BH_CUDA(launch_chain(moments_small_kernel, dim3(1), dim3(kMomSmallThreads), 0, st, sl, MA));
             ctx->launches_build += 1;
             char nm[24];
             snprintf(nm, sizeof(nm), "moments_L%d-%d", sl.level[sl.nlev - 1], sl.level[0]);
@@ -201,8 +201,8 @@ int launch_moments(bh_ctx* ctx)
             ++sl.nlev;
             small_bytes += lvl_bytes;
         } else {
-            moments_kernel<<<blocks_for(b1 - b0, 128), 128, 0, st>>>(b0, b1, l, ctx->lv.slot_base[l + 2], MA);
-            BH_CUDA(cudaGetLastError());
+            BH_CUDA(launch_chain(moments_kernel, dim3(blocks_for(b1 - b0, 128)), dim3(128), 0, st, b0, b1, l,
+                                 ctx->lv.slot_base[l + 2], MA));
             ctx->launches_build += 1;
             char nm[24];
             snprintf(nm, sizeof(nm), "moments_L%d", l);
@@ -361,6 +361,13 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
         const bool speculate = attempt == 0 && ctx->plan_hint_valid;
         ctx->launches_build = 0;
         ctx->npass = 0;
+        // A speculated plan is known before the keys exist: every memset is issued first, and the kernels from the
+        // keys to the level totals form one chain of dependent launches (launch_chain / chain_enter, common.cuh)
+        // with no copy or memset in between; the key reduction is then read back together with the level totals.
+        KeyReduce kr = ctx->plan_hint;
+        SortPlan plan = make_sort_plan(kr.key_or ^ kr.key_and, n);
+        if (speculate && plan.npasses > 0)
+            BH_CUDA(cudaMemsetAsync(ctx->hist.p, 0, sizeof(u32) * sort_pass_words(n) * (size_t)plan.npasses, st));
         BH_CUDA(cudaMemsetAsync(ds, 0, sizeof(DeviceScalars), st));
         BH_CUDA(cudaMemsetAsync(&ds->keyred.key_and, 0xff, sizeof(u64), st));   // key_and starts as all ones
 
@@ -368,26 +375,25 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
         const double s = 2097152.0 / cube[3];      // K1: s = 2^21 / L in fp64
         {
             const int grid = persistent_grid(ctx, 8);
-            if (aligned16(x) && aligned16(y) && aligned16(z))
-                morton_keys_kernel<2><<<grid, 256, 0, st>>>(x, y, z, n, cube[0], cube[1], cube[2], s,
-                                                            ctx->keysA.as<u64>(), &ds->keyred);
-            else
-                morton_keys_kernel<1><<<grid, 256, 0, st>>>(x, y, z, n, cube[0], cube[1], cube[2], s,
-                                                            ctx->keysA.as<u64>(), &ds->keyred);
-            BH_CUDA(cudaGetLastError());
+            if (aligned16(x) && aligned16(y) && aligned16(z)) {
+                BH_CUDA(launch_chain(morton_keys_kernel<2>, dim3(grid), dim3(256), 0, st, x, y, z, n, cube[0], cube[1],
+                                     cube[2], s, ctx->keysA.as<u64>(), &ds->keyred));
+            } else {
+                BH_CUDA(launch_chain(morton_keys_kernel<1>, dim3(grid), dim3(256), 0, st, x, y, z, n, cube[0], cube[1],
+                                     cube[2], s, ctx->keysA.as<u64>(), &ds->keyred));
+            }
         }
         ctx->launches_build += 1;
         pass_mark(ctx, "keys", 36.0 * (double)n);
-        BH_CUDA(cudaEventRecord(ctx->ev[EV_KEYS], st));
+        if (ctx->pass_timing) BH_CUDA(cudaEventRecord(ctx->ev[EV_KEYS], st));   // an event between two kernels breaks their chain
 
         // read-back 1: which key bits vary (decides the radix passes) and the clamp count
-        BH_CUDA(cudaMemcpyAsync(&ctx->h_scalars->keyred, &ds->keyred, sizeof(KeyReduce), cudaMemcpyDeviceToHost, st));
-        KeyReduce kr = ctx->plan_hint;
         if (!speculate) {
+            BH_CUDA(cudaMemcpyAsync(&ctx->h_scalars->keyred, &ds->keyred, sizeof(KeyReduce), cudaMemcpyDeviceToHost, st));
             BH_CUDA(cudaStreamSynchronize(st));
             kr = ctx->h_scalars->keyred;
+            plan = make_sort_plan(kr.key_or ^ kr.key_and, n);
         }
-        const SortPlan plan = make_sort_plan(kr.key_or ^ kr.key_and, n);
         ctx->sort_passes = plan.npasses;
 
         // ---- a2: radix sort of (key, index) ----
@@ -396,7 +402,7 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
             BH_CUDA(ctx->idxB.ensure(sizeof(u32) * n));
         }
         BH_CUDA(radix_sort_pairs(ctx->keysA.as<u64>(), ctx->idxA.as<u32>(), ctx->keysB.as<u64>(), ctx->idxB.as<u32>(), n,
-                                 plan, ctx->hist.as<u32>(), persistent_grid(ctx, 8), st,
+                                 plan, ctx->hist.as<u32>(), /*scratch_is_clear=*/speculate, persistent_grid(ctx, 8), st,
                                  [ctx](const char* nm, double b) { pass_mark(ctx, nm, b); }));
         ctx->launches_build += plan.npasses ? 1 + plan.npasses : 0;   // histogram + one kernel per pass
         {
@@ -414,7 +420,7 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
                 sv.idx = odd ? ctx->idxB.as<u32>() : ctx->idxA.as<u32>();
             }
         }
-        BH_CUDA(cudaEventRecord(ctx->ev[EV_SORT], st));
+        if (ctx->pass_timing) BH_CUDA(cudaEventRecord(ctx->ev[EV_SORT], st));
 
         // ---- a4: topology (a3, the permutation of the cell data, is fused into the assigning kernel) ----
         ctx->nn = 0; ctx->nslots = 0; ctx->depth = 0; ctx->maxlevel = 0; ctx->max_bucket = 1;
@@ -423,18 +429,20 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
             nchunks = topo_chunks(n);
             tgrid = blocks_for(nchunks, kTopoThreads / 32);
             u32* hist = ctx->hist.as<u32>();
-            topo_count_kernel<<<tgrid, kTopoThreads, 0, st>>>(ctx->sv, n, ctx->clev.as<signed char>(), hist, nchunks);
-            BH_CUDA(cudaGetLastError());
+            BH_CUDA(launch_chain(topo_count_kernel, dim3(tgrid), dim3(kTopoThreads), 0, st, ctx->sv, n,
+                                 ctx->clev.as<signed char>(), hist, nchunks));
             pass_mark(ctx, "topo_count", 8.0 * (double)n);
             BH_CUDA(exclusive_scan_u32(hist, hist, (i64)kTopoDigits * nchunks, ctx->scan_scratch.as<u32>(),
                                        &ds->scan_total, st));
-            topo_totals_kernel<<<1, 64, 0, st>>>(hist, nchunks, &ds->scan_total, ds->topo_rows);
-            BH_CUDA(cudaGetLastError());
+            BH_CUDA(launch_chain(topo_totals_kernel, dim3(1), dim3(64), 0, st, hist, nchunks, &ds->scan_total,
+                                 ds->topo_rows));
             pass_mark(ctx, "topo_scan", 0.0);
             // read-back 2: entities and nodes per level (sizes every node / slot array)
             BH_CUDA(cudaMemcpyAsync(ctx->h_scalars->topo_rows, ds->topo_rows, sizeof(u32) * (kTopoDigits + 1),
                                     cudaMemcpyDeviceToHost, st));
         }
+        if (speculate)     // the key reduction of THIS build, checked against the speculated one below
+            BH_CUDA(cudaMemcpyAsync(&ctx->h_scalars->keyred, &ds->keyred, sizeof(KeyReduce), cudaMemcpyDeviceToHost, st));
         BH_CUDA(cudaEventRecord(ctx->ev[EV_PERM], st));
         // aux must be zero on every leaf slot; only the node slots of the previous build are not.  Clearing
         // them runs on the device while the host waits for the read-back and prepares the next launches.
@@ -498,14 +506,13 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
 
         pass_mark(ctx, "aux_clear+readback", 0.0);      // node-slot aux clearing and the idle wait for the level totals
         if (ctx->assign_wait) BH_CUDA(cudaStreamWaitEvent(st, ctx->assign_wait, 0));   // bh_solve_host: m is still landing
-        topo_assign_kernel<<<tgrid, kTopoThreads, 0, st>>>(
-            ctx->clev.as<signed char>(), n, ctx->sv, x, y, z, m, hist, nchunks, (u32)nslots,
-            ctx->leaf_slot.as<u32>(), ctx->node_slot.as<u32>(), ctx->nfirst.as<u32>(), ctx->nlo.as<u32>(),
-            ctx->rec64.as<double4>(), ctx->rec.as<float4>());
-        BH_CUDA(cudaGetLastError());
+        BH_CUDA(launch_chain(topo_assign_kernel, dim3(tgrid), dim3(kTopoThreads), 0, st,
+                             ctx->clev.as<signed char>(), n, ctx->sv, x, y, z, m, hist, nchunks, (u32)nslots,
+                             ctx->leaf_slot.as<u32>(), ctx->node_slot.as<u32>(), ctx->nfirst.as<u32>(), ctx->nlo.as<u32>(),
+                             ctx->rec64.as<double4>(), ctx->rec.as<float4>()));
         pass_mark(ctx, "assign_permute", 84.0 * (double)n + 24.0 * (double)nn);   // a3 84 B/cell + a4 24 B/node
         ctx->launches_build += 1 + 3 + 1 + 1;   // count, scan, totals, assign
-        BH_CUDA(cudaEventRecord(ctx->ev[EV_TOPO], st));
+        if (ctx->pass_timing) BH_CUDA(cudaEventRecord(ctx->ev[EV_TOPO], st));
 
         // ---- a5: moments ----
         { int rc = launch_moments(ctx); if (rc != BH_OK) return rc; }
@@ -521,6 +528,7 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
     }
     BH_CUDA(cudaEventRecord(ctx->ev[EV_MOM], st));
     ctx->ev_build = true;
+    ctx->ev_phases = ctx->pass_timing || n < 2;
     ctx->built = true;
     return BH_OK;
 }
@@ -537,6 +545,7 @@ int bh_update_masses(bh_ctx* ctx, const double* m)
     ctx->launches_build = 0;
     BH_CUDA(cudaEventRecord(ctx->ev[EV_B0], st));
     for (int k = EV_KEYS; k <= EV_TOPO; ++k) BH_CUDA(cudaEventRecord(ctx->ev[k], st));
+    ctx->ev_phases = true;
     if (ctx->n >= 2) {
         mass_update_kernel<<<blocks_for(ctx->n, 256), 256, 0, st>>>(ctx->sv, ctx->leaf_slot.as<u32>(), m, ctx->n,
                                                                    ctx->rec64.as<double4>(), ctx->rec.as<float4>());
@@ -1028,11 +1037,15 @@ int bh_get_stats(bh_ctx* ctx, bh_stats* out)
         out->walk_group = ctx->walk_group;
     }
     if (ctx->ev_build) {
-        cudaEventElapsedTime(&out->ms_keys, ctx->ev[EV_B0], ctx->ev[EV_KEYS]);
-        cudaEventElapsedTime(&out->ms_sort, ctx->ev[EV_KEYS], ctx->ev[EV_SORT]);
-        cudaEventElapsedTime(&out->ms_count, ctx->ev[EV_SORT], ctx->ev[EV_PERM]);
-        cudaEventElapsedTime(&out->ms_assign, ctx->ev[EV_PERM], ctx->ev[EV_TOPO]);
-        cudaEventElapsedTime(&out->ms_moments, ctx->ev[EV_TOPO], ctx->ev[EV_MOM]);
+        // the per-phase events sit between kernels and would break the chain of dependent launches, so an
+        // ordinary build records only its two ends; BH_OPT_PASS_TIMING turns the phases (and the passes) on
+        if (ctx->ev_phases) {
+            cudaEventElapsedTime(&out->ms_keys, ctx->ev[EV_B0], ctx->ev[EV_KEYS]);
+            cudaEventElapsedTime(&out->ms_sort, ctx->ev[EV_KEYS], ctx->ev[EV_SORT]);
+            cudaEventElapsedTime(&out->ms_count, ctx->ev[EV_SORT], ctx->ev[EV_PERM]);
+            cudaEventElapsedTime(&out->ms_assign, ctx->ev[EV_PERM], ctx->ev[EV_TOPO]);
+            cudaEventElapsedTime(&out->ms_moments, ctx->ev[EV_TOPO], ctx->ev[EV_MOM]);
+        }
         cudaEventElapsedTime(&out->ms_build_total, ctx->ev[EV_B0], ctx->ev[EV_MOM]);
     }
     if (ctx->ev_walk) cudaEventElapsedTime(&out->ms_walk, ctx->ev[EV_W0], ctx->ev[EV_W1]);

@@ -43,6 +43,36 @@ __device__ __forceinline__ int common_levels(u64 a, u64 b)
     return x == 0 ? kMaxLevel : (__clzll((long long)x) - 1) / 3;
 }
 
+// Programmatic dependent launch for the chains of short kernels in bh_build (histogram -> sort passes -> count ->
+// scan -> totals; assign -> moments level by level): a kernel launched with launch_chain() may be made resident
+// while its predecessor in the stream drains, and starts its work at chain_enter(), which returns once the
+// predecessor has completed and its writes are visible -- the launch latency and the ramp-up of every kernel
+// overlap the tail of the one before.  chain_enter() must come before the first global access; in a kernel
+// launched the ordinary way it returns at once.
+__device__ __forceinline__ void chain_enter()
+{
+#ifndef BH_NO_PDL
+    asm volatile("griddepcontrol.launch_dependents;\n\tgriddepcontrol.wait;" ::: "memory");
+#endif
+}
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_chain(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                                Args&&... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+#ifndef BH_NO_PDL
+    cfg.numAttrs = 1;
+#else
+    cfg.numAttrs = 0;
+#endif
+    return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+
 // streaming (evict-first) global accesses for data touched once per pass
 template <typename T> __device__ __forceinline__ T ld_stream(const T* p) { return __ldcs(p); }
 template <typename T> __device__ __forceinline__ void st_stream(T* p, T v) { __stcs(p, v); }

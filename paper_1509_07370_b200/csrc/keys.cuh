@@ -52,6 +52,7 @@ morton_keys_kernel(const double* __restrict__ x, const double* __restrict__ y, c
                    i64 n, double x0, double y0, double z0, double s,
                    u64* __restrict__ keys, KeyReduce* __restrict__ red)
 {
+    chain_enter();
     u64 k_or = 0, k_and = ~0ULL;
     u32 n_cl = 0;
     const i64 stride = (i64)gridDim.x * blockDim.x;

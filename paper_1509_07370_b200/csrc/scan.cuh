@@ -52,6 +52,7 @@ __device__ __forceinline__ uint4 load4_guard(const u32* in, i64 e, i64 n)
 __global__ void __launch_bounds__(kScanThreads)
 scan_reduce_kernel(const u32* __restrict__ in, i64 n, u32* __restrict__ block_sums)
 {
+    chain_enter();
     const i64 base = (i64)blockIdx.x * kScanChunk;
     u32 s = 0;
     #pragma unroll
@@ -76,6 +77,7 @@ scan_reduce_kernel(const u32* __restrict__ in, i64 n, u32* __restrict__ block_su
 __global__ void __launch_bounds__(kScanThreads)
 scan_spine_kernel(u32* __restrict__ block_sums, i64 nb, u32* __restrict__ total_out)
 {
+    chain_enter();
     __shared__ u32 s_warp[9];
     u32 carry = 0;
     for (i64 base = 0; base < nb; base += kScanThreads) {
@@ -92,6 +94,7 @@ scan_spine_kernel(u32* __restrict__ block_sums, i64 nb, u32* __restrict__ total_
 __global__ void __launch_bounds__(kScanThreads)
 scan_down_kernel(const u32* in, u32* out, i64 n, const u32* __restrict__ block_sums)   // in may alias out
 {
+    chain_enter();
     __shared__ u32 s_warp[9];
     const i64 base = (i64)blockIdx.x * kScanChunk;
     u32 carry = block_sums[blockIdx.x];
@@ -120,9 +123,12 @@ inline cudaError_t exclusive_scan_u32(const u32* in, u32* out, i64 n, u32* scrat
 {
     if (n <= 0) return cudaSuccess;
     const i64 nb = (n + kScanChunk - 1) / kScanChunk;
-    scan_reduce_kernel<<<(unsigned)nb, kScanThreads, 0, st>>>(in, n, scratch);
-    scan_spine_kernel<<<1, kScanThreads, 0, st>>>(scratch, nb, total_out);
-    scan_down_kernel<<<(unsigned)nb, kScanThreads, 0, st>>>(in, out, n, scratch);
+    cudaError_t e = launch_chain(scan_reduce_kernel, dim3((unsigned)nb), dim3(kScanThreads), 0, st, in, n, scratch);
+    if (e != cudaSuccess) return e;
+    e = launch_chain(scan_spine_kernel, dim3(1), dim3(kScanThreads), 0, st, scratch, nb, total_out);
+    if (e != cudaSuccess) return e;
+    e = launch_chain(scan_down_kernel, dim3((unsigned)nb), dim3(kScanThreads), 0, st, in, out, n, scratch);
+    if (e != cudaSuccess) return e;
     return cudaGetLastError();
 }
 inline size_t scan_scratch_elems(i64 n) { return (size_t)((n + kScanChunk - 1) / kScanChunk) + 1; }

@@ -90,6 +90,7 @@ __global__ void __launch_bounds__(kSortThreads)
 radix_hist_strided_kernel(const u64* __restrict__ keys, i64 n, const SortPlan plan, u32* __restrict__ ghist,
                           u32 pass_stride)
 {
+    chain_enter();
     __shared__ u32 h[kMaxPasses * kRadix];
     for (int i = threadIdx.x; i < plan.npasses * kRadix; i += kSortThreads) h[i] = 0;
     __syncthreads();
@@ -162,6 +163,7 @@ radix_onesweep_kernel(const u64* __restrict__ kin, const u32* __restrict__ vin, 
                       u32* __restrict__ vout, const u32* __restrict__ ghist /* this pass: [256] */,
                       u32* __restrict__ status, u32* __restrict__ ticket, i64 n, int shift, u32 mask, int lo, int ib)
 {
+    chain_enter();
     constexpr bool kVals = MODE == kGenericFirst || MODE == kGeneric;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     SortSmem& S = *reinterpret_cast<SortSmem*>(smem_raw);
@@ -318,19 +320,21 @@ inline size_t sort_smem_bytes(bool packed) { return sizeof(SortSmem) + (packed ?
 // Sorts the n keys in k0 (values = their indices 0..n-1, implicit) in plan.npasses >= 1 passes, ping-ponging
 // between (k0, v0) and (k1, v1); pass p writes to buffer 1 if p is even, else to buffer 0, so the result
 // is in buffer (npasses & 1).  Packed plans never touch v0 / v1 (may be null).
-// scratch holds plan.npasses * sort_pass_words(n) u32.
+// scratch holds plan.npasses * sort_pass_words(n) u32, all zero on entry if scratch_is_clear (else cleared here).
 // `mark(name, algorithmic bytes)` is called after every launch (bh_build's optional per-pass timing).
 template <class Mark>
 inline cudaError_t radix_sort_pairs(u64* k0, u32* v0, u64* k1, u32* v1, i64 n, const SortPlan& plan, u32* scratch,
-                                    int hist_grid, cudaStream_t st, Mark&& mark)
+                                    bool scratch_is_clear, int hist_grid, cudaStream_t st, Mark&& mark)
 {
     if (plan.npasses == 0) return cudaSuccess;
     const size_t pw = sort_pass_words(n);
     const int ntiles = (int)sort_tiles(n);
-    cudaError_t e = cudaMemsetAsync(scratch, 0, sizeof(u32) * pw * plan.npasses, st);
+    cudaError_t e = cudaSuccess;
+    if (!scratch_is_clear) e = cudaMemsetAsync(scratch, 0, sizeof(u32) * pw * plan.npasses, st);
     if (e != cudaSuccess) return e;
     // all histograms in one read; each pass's 256 counters sit at the head of its scratch block
-    radix_hist_strided_kernel<<<hist_grid, kSortThreads, 0, st>>>(k0, n, plan, scratch, (u32)pw);
+    e = launch_chain(radix_hist_strided_kernel, dim3(hist_grid), dim3(kSortThreads), 0, st, k0, n, plan, scratch, (u32)pw);
+    if (e != cudaSuccess) return e;
     mark("sort_hist", 8.0 * (double)n);
     const size_t smem = sort_smem_bytes(plan.packed);
     for (int p = 0; p < plan.npasses; ++p) {
@@ -339,19 +343,20 @@ inline cudaError_t radix_sort_pairs(u64* k0, u32* v0, u64* k1, u32* v1, i64 n, c
         u32* ticket = status + (size_t)ntiles * kRadix;
         if (plan.packed) {
             if (p == 0)
-                radix_onesweep_kernel<kPackedFirst><<<ntiles, kSortThreads, smem, st>>>(
-                    k0, nullptr, k1, nullptr, blk, status, ticket, n, plan.shift[p], plan.mask[p], plan.lo, plan.ib);
+                e = launch_chain(radix_onesweep_kernel<kPackedFirst>, dim3(ntiles), dim3(kSortThreads), smem, st,
+                                 k0, nullptr, k1, nullptr, blk, status, ticket, n, plan.shift[p], plan.mask[p], plan.lo, plan.ib);
             else   // the key window sits above the index bits of the word
-                radix_onesweep_kernel<kPacked><<<ntiles, kSortThreads, smem, st>>>(
-                    k0, nullptr, k1, nullptr, blk, status, ticket, n, plan.shift[p] - plan.lo + plan.ib, plan.mask[p], plan.lo, plan.ib);
+                e = launch_chain(radix_onesweep_kernel<kPacked>, dim3(ntiles), dim3(kSortThreads), smem, st,
+                                 k0, nullptr, k1, nullptr, blk, status, ticket, n, plan.shift[p] - plan.lo + plan.ib, plan.mask[p], plan.lo, plan.ib);
         } else {
             if (p == 0)
-                radix_onesweep_kernel<kGenericFirst><<<ntiles, kSortThreads, smem, st>>>(
-                    k0, nullptr, k1, v1, blk, status, ticket, n, plan.shift[p], plan.mask[p], plan.lo, plan.ib);
+                e = launch_chain(radix_onesweep_kernel<kGenericFirst>, dim3(ntiles), dim3(kSortThreads), smem, st,
+                                 k0, nullptr, k1, v1, blk, status, ticket, n, plan.shift[p], plan.mask[p], plan.lo, plan.ib);
             else
-                radix_onesweep_kernel<kGeneric><<<ntiles, kSortThreads, smem, st>>>(
-                    k0, v0, k1, v1, blk, status, ticket, n, plan.shift[p], plan.mask[p], plan.lo, plan.ib);
+                e = launch_chain(radix_onesweep_kernel<kGeneric>, dim3(ntiles), dim3(kSortThreads), smem, st,
+                                 k0, v0, k1, v1, blk, status, ticket, n, plan.shift[p], plan.mask[p], plan.lo, plan.ib);
         }
+        if (e != cudaSuccess) return e;
         mark("sort_pass", 24.0 * (double)n);          // 12 B read + 12 B written per pair and pass
         u64* tk = k0; k0 = k1; k1 = tk;
         u32* tv = v0; v0 = v1; v1 = tv;

@@ -59,6 +59,7 @@ __global__ void __launch_bounds__(kTopoThreads)
 topo_count_kernel(const SortedView sv, i64 n, signed char* __restrict__ clev, u32* __restrict__ hist,
                   i64 nchunks)
 {
+    chain_enter();
     const u32 lane = lane_id();
     const int warp = threadIdx.x >> 5;
     const i64 chunk = (i64)blockIdx.x * (kTopoThreads / 32) + warp;
@@ -154,6 +155,7 @@ topo_count_kernel(const SortedView sv, i64 n, signed char* __restrict__ clev, u3
 __global__ void topo_totals_kernel(const u32* __restrict__ scanned, i64 nchunks, const u32* __restrict__ total,
                                    u32* __restrict__ out /* [kTopoDigits + 1] */)
 {
+    chain_enter();
     const int d = threadIdx.x;
     if (d < kTopoDigits) out[d] = scanned[(i64)d * nchunks];
     else if (d == kTopoDigits) out[d] = *total;
@@ -173,6 +175,7 @@ topo_assign_kernel(const signed char* __restrict__ clev, i64 n, const SortedView
                    u32* __restrict__ leaf_slot, u32* __restrict__ node_slot, u32* __restrict__ nfirst,
                    u32* __restrict__ nlo, double4* __restrict__ rec64, float4* __restrict__ rec)
 {
+    chain_enter();
     const u32 lane = lane_id();
     const u32 lt = (1u << lane) - 1u;
     const i64 chunk = (i64)blockIdx.x * (kTopoThreads / 32) + (threadIdx.x >> 5);
@@ -247,6 +250,7 @@ topo_assign_kernel(const signed char* __restrict__ clev, i64 n, const SortedView
 __global__ void __launch_bounds__(256)
 aux_clear_kernel(const u32* __restrict__ node_slot, i64 nn, WalkAux* __restrict__ aux)
 {
+    chain_enter();
     const i64 b = (i64)blockIdx.x * blockDim.x + threadIdx.x;
     if (b < nn) reinterpret_cast<uint4*>(aux)[node_slot[b]] = make_uint4(0u, 0u, 0u, 0u);
 }
@@ -335,6 +339,7 @@ __device__ __forceinline__ void moments_node(i64 b, i64 b1, int level, u32 slot_
 __global__ void __launch_bounds__(128)
 moments_kernel(i64 b0, i64 b1, int level, u32 slot_end, const MomentArgs A)
 {
+    chain_enter();
     const i64 b = b0 + (i64)blockIdx.x * blockDim.x + threadIdx.x;
     if (b < b1) moments_node(b, b1, level, slot_end, A);
 }
@@ -351,6 +356,7 @@ struct SmallLevels {
 __global__ void __launch_bounds__(kMomSmallThreads)
 moments_small_kernel(const SmallLevels sl, const MomentArgs A)
 {
+    chain_enter();
     for (int k = 0; k < sl.nlev; ++k) {
         for (i64 b = (i64)sl.b0[k] + threadIdx.x; b < (i64)sl.b1[k]; b += kMomSmallThreads)
             moments_node(b, sl.b1[k], sl.level[k], sl.slot_end[k], A);
