@@ -44,6 +44,7 @@ struct DeviceScalars {          // small device-resident results read back by th
     u32 topo_rows[kTopoDigits + 1];   // row starts of the scanned level histogram + grand total
     u32 scan_total;
     u32 max_bucket;
+    u32 spec_ok;                      // gate of the kernels enqueued on speculated level totals (topo_totals_kernel)
     unsigned long long totals[6];     // sums of the four twin counters, twin interactions, the Phi kernel's own interactions
 };
 
@@ -92,6 +93,8 @@ struct bh_ctx {
     DevBuf rec64, rec, aux;
     KeyReduce plan_hint = {};             // key OR / AND of the last build: the next build sorts on them
     bool plan_hint_valid = false;         // without waiting for its own (checked at the second read-back)
+    u32 rows_hint[kTopoDigits + 1] = {0}; // level totals (scanned row starts) of the last build: the next build of as
+    i64 rows_hint_n = -1;                 // many cells enqueues assign + moments on them before its own arrive
     i64 aux_dirty_nn = -1;                // aux is zero except on node_slot[0, aux_dirty_nn); -1: unknown, clear all
     // walk
     i64 ntargets = -1;                    // bh_set_num_targets: cells [0, ntargets) are targets; -1 = all
@@ -161,7 +164,7 @@ int persistent_grid(const bh_ctx* ctx, int per_sm)
 
 
 // a5: moments of every level, deepest first; runs of small levels share one single-block launch
-int launch_moments(bh_ctx* ctx)
+int launch_moments(bh_ctx* ctx, const u32* gate = nullptr)
 {
     cudaStream_t st = ctx->stream;
     DeviceScalars* ds = ctx->scalars.as<DeviceScalars>();
@@ -171,6 +174,7 @@ int launch_moments(bh_ctx* ctx)
     MA.delta64 = ctx->delta64.as<double>(); MA.rec = ctx->rec.as<float4>(); MA.aux = ctx->aux.as<WalkAux>();
     MA.max_bucket = &ds->max_bucket;
     MA.x0 = ctx->cube[0]; MA.y0 = ctx->cube[1]; MA.z0 = ctx->cube[2]; MA.L = ctx->cube[3];
+    MA.gate = gate;
     SmallLevels sl;
     sl.nlev = 0;
     double small_bytes = 0.0;
@@ -357,6 +361,66 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
     i64 nchunks = 0;
     unsigned tgrid = 0;
     int aux_cleared = 0;
+    int launches_front = 0;
+    bool spec_rows = false;
+    // Everything after the level totals: sizes, assign + permute (a4 + a3), moments (a5).  `rows` are the scanned
+    // row starts -- this build's own, read back, or (gate != null) the previous build's, enqueued before this build's
+    // arrive; the kernels then run only if the device finds the two equal (topo_totals_kernel sets *gate).
+    auto finish = [&](const u32* rows, const u32* gate) -> int {
+        u32* hist = ctx->hist.as<u32>();
+        ctx->launches_build = launches_front + aux_cleared + 1 + 3 + 1 + 1;   // keys + sort; count, scan, totals, assign
+        // The device scan runs in u32.  Every histogram row sums to at most n < 2^30, so consecutive row
+        // starts differ by less than 2^30 and the true 64-bit starts follow from the differences mod 2^32.
+        unsigned long long true_rows[kTopoDigits + 1];
+        true_rows[0] = rows[0];
+        for (int d = 1; d <= kTopoDigits; ++d) true_rows[d] = true_rows[d - 1] + (u32)(rows[d] - rows[d - 1]);
+        if (true_rows[kSlotLevels] >= (1ULL << 32)) {          // slots are u32: n + n_nodes must stay below 2^32
+            snprintf(ctx->cuda_msg, sizeof(ctx->cuda_msg), "n + n_nodes = %llu needs more than 32-bit slots",
+                     true_rows[kSlotLevels]);
+            return BH_ERR_TOO_LARGE;
+        }
+        const i64 nslots = (i64)true_rows[kSlotLevels];       // entities of all levels = n + n_nodes
+        const i64 nn = (i64)(true_rows[kTopoDigits] - true_rows[kSlotLevels]);
+        for (int l = 0; l <= kSlotLevels; ++l) ctx->lv.slot_base[l] = rows[l];
+        for (int l = 0; l <= kNumLevels; ++l) ctx->lv.node_base[l] = (u32)(rows[kSlotLevels + l] - nslots);
+        ctx->maxlevel = 0; ctx->depth = 0;
+        for (int l = 0; l < kNumLevels; ++l)
+            if (ctx->lv.node_base[l + 1] > ctx->lv.node_base[l]) { ctx->maxlevel = l; if (l < kMaxLevel) ctx->depth = l; }
+        ctx->nn = nn;
+        ctx->nslots = nslots;
+        if (nslots != n + nn) {
+            snprintf(ctx->cuda_msg, sizeof(ctx->cuda_msg), "topology: %lld entities for %lld cells + %lld nodes",
+                     (long long)nslots, (long long)n, (long long)nn);
+            return BH_ERR_CUDA;
+        }
+
+        {
+            const bool grow = sizeof(WalkAux) * (size_t)nslots > ctx->aux.cap;
+            BH_CUDA(ctx->aux.ensure(sizeof(WalkAux) * nslots));
+            if (grow || ctx->aux_dirty_nn < 0) BH_CUDA(cudaMemsetAsync(ctx->aux.p, 0, ctx->aux.cap, st));
+            ctx->aux_dirty_nn = -1;                            // unknown until this build's moments are launched
+        }
+        BH_CUDA(ctx->nlo.ensure(sizeof(u32) * nn));
+        BH_CUDA(ctx->nfirst.ensure(sizeof(u32) * (nn + 4)));
+        BH_CUDA(ctx->node_slot.ensure(sizeof(u32) * nn));
+        BH_CUDA(ctx->delta64.ensure(sizeof(double) * nn));
+        BH_CUDA(ctx->rec64.ensure(sizeof(double4) * nslots));
+        BH_CUDA(ctx->rec.ensure(sizeof(float4) * nslots));
+
+        pass_mark(ctx, "aux_clear+readback", 0.0);      // node-slot aux clearing and the idle wait for the level totals
+        if (ctx->assign_wait) BH_CUDA(cudaStreamWaitEvent(st, ctx->assign_wait, 0));   // bh_solve_host: m is still landing
+        BH_CUDA(launch_chain(topo_assign_kernel, dim3(tgrid), dim3(kTopoThreads), 0, st,
+                             ctx->clev.as<signed char>(), n, ctx->sv, x, y, z, m, hist, nchunks, (u32)nslots,
+                             ctx->leaf_slot.as<u32>(), ctx->node_slot.as<u32>(), ctx->nfirst.as<u32>(), ctx->nlo.as<u32>(),
+                             ctx->rec64.as<double4>(), ctx->rec.as<float4>(), gate));
+        pass_mark(ctx, "assign_permute", 84.0 * (double)n + 24.0 * (double)nn);   // a3 84 B/cell + a4 24 B/node
+        if (ctx->pass_timing) BH_CUDA(cudaEventRecord(ctx->ev[EV_TOPO], st));
+
+        // ---- a5: moments ----
+        { int rc = launch_moments(ctx, gate); if (rc != BH_OK) return rc; }
+        ctx->aux_dirty_nn = nn;
+        return BH_OK;
+    };
     for (int attempt = 0;; ++attempt) {
         const bool speculate = attempt == 0 && ctx->plan_hint_valid;
         ctx->launches_build = 0;
@@ -405,6 +469,7 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
                                  plan, ctx->hist.as<u32>(), /*scratch_is_clear=*/speculate, persistent_grid(ctx, 8), st,
                                  [ctx](const char* nm, double b) { pass_mark(ctx, nm, b); }));
         ctx->launches_build += plan.npasses ? 1 + plan.npasses : 0;   // histogram + one kernel per pass
+        launches_front = ctx->launches_build;
         {
             const bool odd = plan.npasses & 1;
             const u64* kres = odd ? ctx->keysB.as<u64>() : ctx->keysA.as<u64>();
@@ -434,14 +499,20 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
             pass_mark(ctx, "topo_count", 8.0 * (double)n);
             BH_CUDA(exclusive_scan_u32(hist, hist, (i64)kTopoDigits * nchunks, ctx->scan_scratch.as<u32>(),
                                        &ds->scan_total, st));
+            // the level totals of the previous build are expected again if that build had as many cells and this
+            // one already speculates its sort plan (the same mesh as last time)
+            spec_rows = speculate && ctx->rows_hint_n == n;
+            TotalsHint hint;
+            memcpy(hint.rows, ctx->rows_hint, sizeof(hint.rows));
+            hint.key_or = kr.key_or; hint.key_and = kr.key_and; hint.check = spec_rows ? 1 : 0;
             BH_CUDA(launch_chain(topo_totals_kernel, dim3(1), dim3(64), 0, st, hist, nchunks, &ds->scan_total,
-                                 ds->topo_rows));
+                                 ctx->h_scalars->topo_rows, hint, &ds->keyred,
+                                 speculate ? &ctx->h_scalars->keyred : nullptr, &ds->spec_ok));
             pass_mark(ctx, "topo_scan", 0.0);
-            // read-back 2: entities and nodes per level (sizes every node / slot array)
-            BH_CUDA(cudaMemcpyAsync(ctx->h_scalars->topo_rows, ds->topo_rows, sizeof(u32) * (kTopoDigits + 1),
-                                    cudaMemcpyDeviceToHost, st));
-        }
-        if (speculate)     // the key reduction of THIS build, checked against the speculated one below
+            // read-back 2: entities and nodes per level (sizes every node / slot array) and, under a speculated
+            // plan, the key reduction of THIS build -- written by the kernel itself into the pinned host mirror
+            // (device-accessible under unified addressing), so no copy stands on the stream
+        } else if (speculate)
             BH_CUDA(cudaMemcpyAsync(&ctx->h_scalars->keyred, &ds->keyred, sizeof(KeyReduce), cudaMemcpyDeviceToHost, st));
         BH_CUDA(cudaEventRecord(ctx->ev[EV_PERM], st));
         // aux must be zero on every leaf slot; only the node slots of the previous build are not.  Clearing
@@ -453,6 +524,9 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
             ctx->aux_dirty_nn = 0;
             aux_cleared = 1;
         }
+        // speculated level totals: assign and the moments are enqueued now, on the previous build's totals and
+        // behind a device-side gate, and the host's wait for the read-back below runs under them
+        if (spec_rows) { int rc = finish(ctx->rows_hint, &ds->spec_ok); if (rc != BH_OK) return rc; }
         BH_CUDA(cudaEventSynchronize(ctx->ev[EV_PERM]));
         {
             const KeyReduce& real = ctx->h_scalars->keyred;
@@ -461,62 +535,16 @@ int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, con
             ctx->plan_hint_valid = true;
             ctx->n_clamped = (i64)real.n_clamped;
             if (hit) break;
+            if (spec_rows) ctx->aux_dirty_nn = 0;    // the gate was closed (the key reduction differs): aux is untouched
+            spec_rows = false;
         }
     }   // attempt
     if (n >= 2) {
-        u32* hist = ctx->hist.as<u32>();
-        const u32* rows = ctx->h_scalars->topo_rows;
-        // The device scan runs in u32.  Every histogram row sums to at most n < 2^30, so consecutive row
-        // starts differ by less than 2^30 and the true 64-bit starts follow from the differences mod 2^32.
-        unsigned long long true_rows[kTopoDigits + 1];
-        true_rows[0] = rows[0];
-        for (int d = 1; d <= kTopoDigits; ++d) true_rows[d] = true_rows[d - 1] + (u32)(rows[d] - rows[d - 1]);
-        if (true_rows[kSlotLevels] >= (1ULL << 32)) {          // slots are u32: n + n_nodes must stay below 2^32
-            snprintf(ctx->cuda_msg, sizeof(ctx->cuda_msg), "n + n_nodes = %llu needs more than 32-bit slots",
-                     true_rows[kSlotLevels]);
-            return BH_ERR_TOO_LARGE;
-        }
-        const i64 nslots = (i64)true_rows[kSlotLevels];       // entities of all levels = n + n_nodes
-        const i64 nn = (i64)(true_rows[kTopoDigits] - true_rows[kSlotLevels]);
-        for (int l = 0; l <= kSlotLevels; ++l) ctx->lv.slot_base[l] = rows[l];
-        for (int l = 0; l <= kNumLevels; ++l) ctx->lv.node_base[l] = (u32)(rows[kSlotLevels + l] - nslots);
-        for (int l = 0; l < kNumLevels; ++l)
-            if (ctx->lv.node_base[l + 1] > ctx->lv.node_base[l]) { ctx->maxlevel = l; if (l < kMaxLevel) ctx->depth = l; }
-        ctx->nn = nn;
-        ctx->nslots = nslots;
-        if (nslots != n + nn) {
-            snprintf(ctx->cuda_msg, sizeof(ctx->cuda_msg), "topology: %lld entities for %lld cells + %lld nodes",
-                     (long long)nslots, (long long)n, (long long)nn);
-            return BH_ERR_CUDA;
-        }
-
-        {
-            const bool grow = sizeof(WalkAux) * (size_t)nslots > ctx->aux.cap;
-            BH_CUDA(ctx->aux.ensure(sizeof(WalkAux) * nslots));
-            if (grow || ctx->aux_dirty_nn < 0) BH_CUDA(cudaMemsetAsync(ctx->aux.p, 0, ctx->aux.cap, st));
-            ctx->aux_dirty_nn = -1;                            // unknown until this build's moments are launched
-            ctx->launches_build += aux_cleared;
-        }
-        BH_CUDA(ctx->nlo.ensure(sizeof(u32) * nn));
-        BH_CUDA(ctx->nfirst.ensure(sizeof(u32) * (nn + 4)));
-        BH_CUDA(ctx->node_slot.ensure(sizeof(u32) * nn));
-        BH_CUDA(ctx->delta64.ensure(sizeof(double) * nn));
-        BH_CUDA(ctx->rec64.ensure(sizeof(double4) * nslots));
-        BH_CUDA(ctx->rec.ensure(sizeof(float4) * nslots));
-
-        pass_mark(ctx, "aux_clear+readback", 0.0);      // node-slot aux clearing and the idle wait for the level totals
-        if (ctx->assign_wait) BH_CUDA(cudaStreamWaitEvent(st, ctx->assign_wait, 0));   // bh_solve_host: m is still landing
-        BH_CUDA(launch_chain(topo_assign_kernel, dim3(tgrid), dim3(kTopoThreads), 0, st,
-                             ctx->clev.as<signed char>(), n, ctx->sv, x, y, z, m, hist, nchunks, (u32)nslots,
-                             ctx->leaf_slot.as<u32>(), ctx->node_slot.as<u32>(), ctx->nfirst.as<u32>(), ctx->nlo.as<u32>(),
-                             ctx->rec64.as<double4>(), ctx->rec.as<float4>()));
-        pass_mark(ctx, "assign_permute", 84.0 * (double)n + 24.0 * (double)nn);   // a3 84 B/cell + a4 24 B/node
-        ctx->launches_build += 1 + 3 + 1 + 1;   // count, scan, totals, assign
-        if (ctx->pass_timing) BH_CUDA(cudaEventRecord(ctx->ev[EV_TOPO], st));
-
-        // ---- a5: moments ----
-        { int rc = launch_moments(ctx); if (rc != BH_OK) return rc; }
-        ctx->aux_dirty_nn = nn;
+        const bool hit_rows = spec_rows && memcmp(ctx->h_scalars->topo_rows, ctx->rows_hint, sizeof(ctx->rows_hint)) == 0;
+        if (spec_rows && !hit_rows) ctx->aux_dirty_nn = 0;     // the gated kernels wrote nothing: aux is still all zero
+        if (!hit_rows) { int rc = finish(ctx->h_scalars->topo_rows, nullptr); if (rc != BH_OK) return rc; }
+        memcpy(ctx->rows_hint, ctx->h_scalars->topo_rows, sizeof(ctx->rows_hint));
+        ctx->rows_hint_n = n;
     } else {
         // n = 1: no tree (T-rule 1); the lone cell's record is kept for bh_essential_nodes
         if (ctx->assign_wait) BH_CUDA(cudaStreamWaitEvent(st, ctx->assign_wait, 0));
@@ -582,7 +610,6 @@ int bh_essential_nodes(bh_ctx* ctx, const double box_lo[3], const double box_hi[
         BH_CUDA(cudaMemcpyAsync(out, ctx->rec64.p, sizeof(double) * 4, cudaMemcpyDeviceToDevice, st));
         return BH_OK;
     }
-    DeviceScalars* ds = ctx->scalars.as<DeviceScalars>();
     const i64 nslots = ctx->nslots;
     const i64 nblk = (nslots + kEssTile - 1) / kEssTile;
     BH_CUDA(ctx->ess_state.ensure((size_t)nslots + 16));
@@ -603,8 +630,7 @@ int bh_essential_nodes(bh_ctx* ctx, const double box_lo[3], const double box_hi[
         const i64 b0 = last ? 0 : ctx->lv.node_base[l], b1 = last ? 0 : ctx->lv.node_base[l + 1];
         const bool small = !last && b1 - b0 <= kEssSmallNodes;
         if ((!small || last) && sl.nlev > 0) {
-            ess_small_kernel<<<1, 1024, 0, st>>>(sl, A);
-            BH_CUDA(cudaGetLastError());
+            BH_CUDA(launch_chain(ess_small_kernel, dim3(1), dim3(1024), 0, st, sl, A));
             sl.nlev = 0;
         }
         if (last || b1 == b0) continue;
@@ -613,19 +639,17 @@ int bh_essential_nodes(bh_ctx* ctx, const double box_lo[3], const double box_hi[
             sl.slot_end[sl.nlev] = ctx->lv.slot_base[l + 2];
             ++sl.nlev;
         } else {
-            ess_level_kernel<<<blocks_for(b1 - b0, 256), 256, 0, st>>>(b0, b1, l, ctx->lv.slot_base[l + 2], A);
-            BH_CUDA(cudaGetLastError());
+            BH_CUDA(launch_chain(ess_level_kernel, dim3(blocks_for(b1 - b0, 256)), dim3(256), 0, st, b0, b1, l,
+                                 ctx->lv.slot_base[l + 2], A));
         }
     }
     u32* blk = ctx->ess_emit.as<u32>();
-    ess_count_kernel<<<(unsigned)nblk, kEssThreads, 0, st>>>(A.state, nslots, blk);
-    BH_CUDA(cudaGetLastError());
-    BH_CUDA(exclusive_scan_u32(blk, blk, nblk, ctx->scan_scratch.as<u32>(), &ds->scan_total, st));
-    if (cap > 0) {
-        ess_gather_kernel<<<(unsigned)nblk, kEssThreads, 0, st>>>(A.state, nslots, blk, ctx->rec64.as<double4>(), out, cap);
-        BH_CUDA(cudaGetLastError());
-    }
-    BH_CUDA(cudaMemcpyAsync(&ctx->h_scalars->scan_total, &ds->scan_total, sizeof(u32), cudaMemcpyDeviceToHost, st));
+    BH_CUDA(launch_chain(ess_count_kernel, dim3((unsigned)nblk), dim3(kEssThreads), 0, st, A.state, nslots, blk));
+    // the number of entries goes straight into the pinned host mirror (device-accessible): no copy on the stream
+    BH_CUDA(exclusive_scan_u32(blk, blk, nblk, ctx->scan_scratch.as<u32>(), &ctx->h_scalars->scan_total, st));
+    if (cap > 0)
+        BH_CUDA(launch_chain(ess_gather_kernel, dim3((unsigned)nblk), dim3(kEssThreads), 0, st, A.state, nslots, blk,
+                             ctx->rec64.as<double4>(), out, cap));
     BH_CUDA(cudaStreamSynchronize(st));
     *count = (int64_t)ctx->h_scalars->scan_total;
     return *count > cap ? BH_ERR_TOO_LARGE : BH_OK;

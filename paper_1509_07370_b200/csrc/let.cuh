@@ -60,6 +60,7 @@ __device__ __forceinline__ void ess_node(i64 b, i64 b1, int level, u32 slot_end,
 __global__ void __launch_bounds__(256)
 ess_level_kernel(i64 b0, i64 b1, int level, u32 slot_end, const EssArgs A)
 {
+    chain_enter();
     const i64 b = b0 + (i64)blockIdx.x * blockDim.x + threadIdx.x;
     if (b < b1) ess_node(b, b1, level, slot_end, A);
 }
@@ -69,6 +70,7 @@ constexpr int kEssSmallNodes = 1024;
 __global__ void __launch_bounds__(1024)
 ess_small_kernel(const SmallLevels sl, const EssArgs A)
 {
+    chain_enter();
     for (int k = 0; k < sl.nlev; ++k) {
         for (i64 b = (i64)sl.b0[k] + threadIdx.x; b < (i64)sl.b1[k]; b += blockDim.x)
             ess_node(b, sl.b1[k], sl.level[k], sl.slot_end[k], A);
@@ -99,6 +101,7 @@ __device__ __forceinline__ u32 ess_twos(u32 w) { return (w >> 1) & 0x01010101u; 
 __global__ void __launch_bounds__(kEssThreads)
 ess_count_kernel(const unsigned char* __restrict__ state, i64 nslots, u32* __restrict__ block_count)
 {
+    chain_enter();
     __shared__ u32 s_warp[9];
     const i64 s0 = ((i64)blockIdx.x * kEssThreads + threadIdx.x) * 16;
     const uint4 v = ess_load_flags(state, s0, nslots);
@@ -112,6 +115,7 @@ __global__ void __launch_bounds__(kEssThreads)
 ess_gather_kernel(const unsigned char* __restrict__ state, i64 nslots, const u32* __restrict__ block_base,
                   const double4* __restrict__ rec64, double* __restrict__ out, i64 cap)
 {
+    chain_enter();
     __shared__ u32 s_warp[9];
     const i64 s0 = ((i64)blockIdx.x * kEssThreads + threadIdx.x) * 16;
     const uint4 v = ess_load_flags(state, s0, nslots);

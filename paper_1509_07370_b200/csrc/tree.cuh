@@ -24,6 +24,7 @@
 // deepest level up, each node from its children in ascending octant order in fp64 (M-rules).
 #pragma once
 #include "common.cuh"
+#include "keys.cuh"
 
 namespace bh {
 
@@ -151,14 +152,34 @@ topo_count_kernel(const SortedView sv, i64 n, signed char* __restrict__ clev, u3
     if (lane < (u32)kNumLevels) hist[(i64)(kSlotLevels + lane) * nchunks + chunk] = myI;
 }
 
-// row starts of the scanned histogram (+ the grand total) for the host: out[d] = scanned[d * nchunks]
+// row starts of the scanned histogram (+ the grand total) for the host: out[d] = scanned[d * nchunks].
+// A build that speculates the level totals (bh_build: the same mesh as last time) has already been told the totals it
+// expects: `*gate` = 1 if the rows and the key reduction just computed equal the expected ones, else 0 -- the
+// kernels enqueued behind this one on that assumption (assign, moments) return at once when it is 0.
+struct TotalsHint {
+    u32 rows[kTopoDigits + 1];
+    u64 key_or, key_and;
+    int check;                       // 0: nothing was speculated, *gate = 0
+};
 __global__ void topo_totals_kernel(const u32* __restrict__ scanned, i64 nchunks, const u32* __restrict__ total,
-                                   u32* __restrict__ out /* [kTopoDigits + 1] */)
+                                   u32* __restrict__ out /* [kTopoDigits + 1], pinned host memory */, const TotalsHint hint,
+                                   const KeyReduce* __restrict__ red, KeyReduce* __restrict__ red_out /* host, or null */,
+                                   u32* __restrict__ gate)
 {
     chain_enter();
     const int d = threadIdx.x;
-    if (d < kTopoDigits) out[d] = scanned[(i64)d * nchunks];
-    else if (d == kTopoDigits) out[d] = *total;
+    u32 v = 0u;
+    if (d < kTopoDigits) v = scanned[(i64)d * nchunks];
+    else if (d == kTopoDigits) v = *total;
+    if (d <= kTopoDigits) out[d] = v;          // straight into the host's pinned mirror: no copy on the stream
+    bool same = d > kTopoDigits || v == hint.rows[d];
+    if (d == 0) {
+        const KeyReduce r = *red;
+        if (red_out) *red_out = r;
+        same = same && r.key_or == hint.key_or && r.key_and == hint.key_and;
+    }
+    const int all = __syncthreads_and(same);
+    if (d == 0) *gate = (hint.check && all) ? 1u : 0u;
 }
 
 // ---- a4.2 + a3: number every entity, link the nodes, move every cell into its slot ------------------
@@ -173,9 +194,11 @@ topo_assign_kernel(const signed char* __restrict__ clev, i64 n, const SortedView
                    const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
                    const double* __restrict__ m, const u32* __restrict__ scanned, i64 nchunks, u32 nslots,
                    u32* __restrict__ leaf_slot, u32* __restrict__ node_slot, u32* __restrict__ nfirst,
-                   u32* __restrict__ nlo, double4* __restrict__ rec64, float4* __restrict__ rec)
+                   u32* __restrict__ nlo, double4* __restrict__ rec64, float4* __restrict__ rec,
+                   const u32* __restrict__ gate /* null, or: run only if *gate != 0 (speculated level totals) */)
 {
     chain_enter();
+    if (gate && *gate == 0u) return;
     const u32 lane = lane_id();
     const u32 lt = (1u << lane) - 1u;
     const i64 chunk = (i64)blockIdx.x * (kTopoThreads / 32) + (threadIdx.x >> 5);
@@ -288,6 +311,7 @@ struct MomentArgs {
     SortedView sv; const u32* nlo; const u32* nfirst; const u32* node_slot;
     double4* rec64; double* delta64; float4* rec; WalkAux* aux; u32* max_bucket;
     double x0, y0, z0, L;
+    const u32* gate;                 // null, or: run only if *gate != 0 (speculated level totals)
 };
 
 __device__ __forceinline__ void moments_node(i64 b, i64 b1, int level, u32 slot_end, const MomentArgs& A)
@@ -340,6 +364,7 @@ __global__ void __launch_bounds__(128)
 moments_kernel(i64 b0, i64 b1, int level, u32 slot_end, const MomentArgs A)
 {
     chain_enter();
+    if (A.gate && *A.gate == 0u) return;
     const i64 b = b0 + (i64)blockIdx.x * blockDim.x + threadIdx.x;
     if (b < b1) moments_node(b, b1, level, slot_end, A);
 }
@@ -357,6 +382,7 @@ __global__ void __launch_bounds__(kMomSmallThreads)
 moments_small_kernel(const SmallLevels sl, const MomentArgs A)
 {
     chain_enter();
+    if (A.gate && *A.gate == 0u) return;
     for (int k = 0; k < sl.nlev; ++k) {
         for (i64 b = (i64)sl.b0[k] + threadIdx.x; b < (i64)sl.b1[k]; b += kMomSmallThreads)
             moments_node(b, sl.b1[k], sl.level[k], sl.slot_end[k], A);
