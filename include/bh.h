@@ -121,9 +121,13 @@ int bh_set_option(bh_ctx* ctx, int key, int value);
  * identical keys form a level-21 bucket leaf; DESIGN.md T-rules), the cell data being gathered into
  * tree order in the same pass -> bottom-up level-by-level M, R (Eq. 5), delta = |R - geometric
  * centre| in fp64 (DESIGN.md M-rules).
- * Synchronises the stream internally to read back (a) which key bits vary and (b) the node count per
- * level -- once when the keys vary on the same bits as in the previous build of this context (the sort
- * is then started on that assumption and checked afterwards), twice otherwise. */
+ * Waits on the device internally for (a) which key bits vary and (b) the node count per level -- once when the
+ * keys vary on the same bits as in the previous build of this context (the sort is then started on that
+ * assumption and checked afterwards), twice otherwise.  A build of as many cells as the previous one also
+ * enqueues its last kernels on the previous level totals before that wait (they run only if the device finds the
+ * totals unchanged, else they are repeated), so the wait runs under them.  The kernels are issued as chains of
+ * programmatic dependent launches on the context's stream; to work enqueued before or after the call they behave
+ * like ordinary stream-ordered launches. */
 int bh_build(bh_ctx* ctx, const double* x, const double* y, const double* z, const double* m,
              int64_t n, const double cube[4]);
 
