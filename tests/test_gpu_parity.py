@@ -292,6 +292,35 @@ def test_context_reuse_across_inputs(bh, oracle):
         parity.check_walk(ctx, ot, w, w.theta)
 
 
+def test_speculated_level_totals_hit_and_miss(bh, oracle):
+    """Same n, same varying key bits, another topology: the second build starts its sort on the first one's plan
+    (a hit) and enqueues assign + moments on the first one's level totals (a miss: the device-side gate stays
+    closed, the kernels return, the host repeats them on the true totals); a third build of the same cells hits
+    both.  Every build must equal the oracle's tree, moments and Phi, and the repeated build the one before it
+    bit for bit."""
+    a, b = wl.random_points(20000, seed=11), wl.random_points(20000, seed=12)
+    ka = np.bitwise_or.reduce(oracle.OracleTree(a.x, a.y, a.z, a.m, a.cube).sorted_keys_perm()[0])
+    kb = np.bitwise_or.reduce(oracle.OracleTree(b.x, b.y, b.z, b.m, b.cube).sorted_keys_perm()[0])
+    assert ka == kb                                   # the premise: the sort plan of one serves the other
+    ctx = bh.Context(0)
+    prev = None
+    for w in (a, b, b, a, a):
+        ctx.build(_dev(w.x), _dev(w.y), _dev(w.z), _dev(w.m), w.cube)
+        t = _tree_np(ctx)
+        ot = oracle.OracleTree(w.x, w.y, w.z, w.m, w.cube)
+        ok, op = ot.sorted_keys_perm()
+        assert np.array_equal(t["keys"], ok) and np.array_equal(t["perm"], op)
+        on = ot.nodes()
+        for k in ("level", "prefix", "lo", "hi", "nchild"):
+            assert np.array_equal(t[k].astype(np.int64), on[k].astype(np.int64)), k
+        assert np.array_equal(t["M"], on["M"])
+        phi = ctx.potential(0.5, w.G).cpu().numpy()
+        parity.check_walk(ctx, ot, w, 0.5, phi=phi)
+        if prev is not None and prev[0] is w:
+            assert np.array_equal(phi, prev[1])
+        prev = (w, phi)
+
+
 def test_measured_fma_peak_is_near_nominal(bh):
     """The measured denominator of the walk's roofline (bench.py's aid, its own small library -- not libbh):
     register-resident FMA chains reach most of SMs x 128 lanes x 2 x clock and never exceed it."""
