@@ -128,7 +128,7 @@ namespace {
 
 int cuda_fail(bh_ctx* c, cudaError_t e, const char* where)
 {
-    if (c) snprintf(c->cuda_msg, sizeof(c->cuda_msg), "%s: %s", where, cudaGetErrorString(e));
+    if (c) snprintf(c->cuda_msg, sizeof(c->cuda_msg), "%.160s: %.80s", where, cudaGetErrorString(e));
     cudaGetLastError();   // clear sticky-free errors
     return e == cudaErrorMemoryAllocation ? BH_ERR_OOM : BH_ERR_CUDA;
 }
