@@ -41,7 +41,8 @@ struct DevBuf {                 // grow-only device buffer
 
 struct DeviceScalars {          // small device-resident results read back by the host
     KeyReduce keyred;
-    u32 topo_rows[kTopoDigits + 1];   // row starts of the scanned level histogram + grand total
+    u32 topo_rows[kTopoDigits + 1];   // row starts of the scanned level histogram + grand total (filled in the host mirror only:
+                                      // topo_totals_kernel writes them there itself)
     u32 scan_total;
     u32 max_bucket;
     u32 spec_ok;                      // gate of the kernels enqueued on speculated level totals (topo_totals_kernel)
