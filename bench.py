@@ -545,7 +545,10 @@ def run_ours(args):
         "ms_build_miss": ms_build_miss,
         "build_notes": "ms_build: the timed steps (same mesh every step: the sort plan speculated from the previous build "
                        "hits, one host round trip); ms_build_miss: previous build on another mesh (plan miss: keys, sort and "
-                       "count run twice, two round trips); ms_build_cold: first build of a fresh context (allocations inside)",
+                       "count run twice, two round trips); ms_build_cold: first build of a fresh context (allocations inside); "
+                       "build_passes: a build under BH_OPT_PASS_TIMING, one event after every kernel -- the events stand "
+                       "between the kernels, so that build runs without the overlap of dependent launches and its passes add "
+                       "up to more than ms_build",
         "build_passes": passes,
         "field": {"ms_walk": t_field * 1e3, "interactions_per_s": world * st.interactions / t_field,
                   "flops_per_interaction": 22, "frac_fp32": st.interactions * 22 / t_field / 1e12 / (
